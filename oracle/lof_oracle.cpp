@@ -1,0 +1,240 @@
+// lof_oracle.cpp — ORACLE (test infrastructure, not the product).  See lof_oracle.h.
+// Plain single-threaded C++17, fp64 arithmetic, written from PAPER.md (arXiv 1701.08197).
+// Shares no code with the CUDA path.  "parity unpinned" for readings F7, F8, F10, S1-S4,
+// H3'-H6' against the authors' code (not available); see DESIGN.md §3.
+#include "lof_oracle.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+extern "C" {
+
+// PAPER.md:41  factor_I = startThreshold * p^(log2 I) / I.  For I = 2^k this is
+// startThreshold * (p/2)^k; computed by repeated multiplication (reading F1).
+void lofo_factor_table(double start_threshold, double p, uint32_t n_out, double* out) {
+  double f = start_threshold;
+  for (uint32_t k = 0; k < n_out; ++k) {
+    out[k] = f;
+    f = f * (p / 2.0);
+  }
+}
+
+// PAPER.md:41  threshold_I = median + stddev * factor_I * sensitivity.
+void lofo_threshold_table(double median, double stddev, double start_threshold, double p,
+                          double sensitivity, uint32_t n_out, double* out) {
+  std::vector<double> factor(n_out);
+  lofo_factor_table(start_threshold, p, n_out, factor.data());
+  for (uint32_t k = 0; k < n_out; ++k) out[k] = median + stddev * factor[k] * sensitivity;
+}
+
+// O1-O3 (PAPER.md:41 uses median and stddev; :120 "means, medians, standard deviations").
+void lofo_statistics(const float* x, uint64_t n, lofo_stream_stats* out) {
+  out->median = 0.f; out->mean = 0.0; out->stddev = 0.0; out->n_flagged = 0; out->n_nonfinite = 0;
+  if (n == 0) return;
+  uint32_t bad = 0;
+  for (uint64_t i = 0; i < n; ++i) if (!std::isfinite(x[i])) ++bad;
+  out->n_nonfinite = bad;
+  if (bad) return;                                   // reading S6: other fields unspecified
+  double sum = 0.0;
+  for (uint64_t i = 0; i < n; ++i) sum += (double)x[i];
+  const double mean = sum / (double)n;
+  double ss = 0.0;
+  for (uint64_t i = 0; i < n; ++i) { const double d = (double)x[i] - mean; ss += d * d; }
+  out->mean = mean;
+  out->stddev = std::sqrt(ss / (double)n);           // population, about the mean (S2)
+  std::vector<float> v(x, x + n);
+  std::nth_element(v.begin(), v.begin() + n / 2, v.end());   // O(N) selection
+  out->median = v[n / 2];                            // rank floor(N/2), 0-based (S3)
+}
+
+static inline void mark_margin(uint8_t* margin, int64_t ms, uint64_t t0, uint64_t I, double S,
+                               double lim, double rel) {
+  if (!margin) return;
+  if (std::fabs(S - lim) <= rel * std::fabs(lim))
+    for (uint64_t j = 0; j < I; ++j) margin[(int64_t)(t0 + j) * ms] = 1;
+}
+
+// PAPER.md:37-47, Fig. 1: window I = 1, 2, 4, ...; a window is flagged when its sum, with
+// already-flagged samples replaced by threshold_I (F7), exceeds I*threshold_I (F4, strict F6).
+// Flags are frozen at the start of each iteration (F8).  The literal double loop.
+void lofo_sumthreshold_1d_literal(const float* x, uint64_t n, int64_t stride, uint8_t* mask,
+                                  int64_t ms, const double* thresholds, uint32_t n_levels,
+                                  uint8_t* margin, double margin_rel) {
+  std::vector<uint8_t> P(n);
+  for (uint32_t k = 0; k < n_levels; ++k) {
+    const uint64_t I = (uint64_t)1 << k;
+    if (I > n) break;                                // F9: window larger than the axis is skipped
+    const double T = thresholds[k];
+    const double lim = (double)I * T;
+    for (uint64_t i = 0; i < n; ++i) P[i] = mask[(int64_t)i * ms];
+    for (uint64_t t0 = 0; t0 + I <= n; ++t0) {
+      double S = 0.0;
+      for (uint64_t j = 0; j < I; ++j)
+        S += P[t0 + j] ? T : (double)x[(int64_t)(t0 + j) * stride];
+      mark_margin(margin, ms, t0, I, S, lim, margin_rel);
+      if (S > lim)
+        for (uint64_t j = 0; j < I; ++j) mask[(int64_t)(t0 + j) * ms] = 1;
+    }
+  }
+}
+
+// Same iteration in O(n): S - I*T = sum over the window of (v - T), v the substituted value,
+// i.e. 0 for a flagged sample and x - T otherwise; taken as differences of an fp64 prefix
+// array of those terms (a constant line gives exactly 0, keeping F6's "constant input yields
+// no flags").  Checked against the literal loop in tests/test_oracle_pins.py (pin P2).
+void lofo_sumthreshold_1d_fast(const float* x, uint64_t n, int64_t stride, uint8_t* mask,
+                               int64_t ms, const double* thresholds, uint32_t n_levels,
+                               uint8_t* margin, double margin_rel) {
+  std::vector<double> pre(n + 1);
+  std::vector<int32_t> diff(n + 1);
+  for (uint32_t k = 0; k < n_levels; ++k) {
+    const uint64_t I = (uint64_t)1 << k;
+    if (I > n) break;
+    const double T = thresholds[k];
+    const double lim = (double)I * T;
+    pre[0] = 0.0;
+    for (uint64_t i = 0; i < n; ++i)
+      pre[i + 1] = pre[i] + (mask[(int64_t)i * ms] ? 0.0 : (double)x[(int64_t)i * stride] - T);
+    std::fill(diff.begin(), diff.end(), 0);
+    for (uint64_t t0 = 0; t0 + I <= n; ++t0) {
+      const double excess = pre[t0 + I] - pre[t0];          // S - I*T
+      mark_margin(margin, ms, t0, I, excess + lim, lim, margin_rel);
+      if (excess > 0.0) { diff[t0] += 1; diff[t0 + I] -= 1; }
+    }
+    int32_t cover = 0;
+    for (uint64_t i = 0; i < n; ++i) {
+      cover += diff[i];
+      if (cover > 0) mask[(int64_t)i * ms] = 1;
+    }
+  }
+}
+
+void lofo_power_from_ci16(const int16_t* volt, uint64_t n, float* power) {
+  for (uint64_t i = 0; i < n; ++i) {
+    const int32_t re = volt[2 * i], im = volt[2 * i + 1];
+    power[i] = (float)(uint32_t)(re * re + im * im);   // integer-exact (S5)
+  }
+}
+
+
+// O1-O9 for a whole block (PAPER.md:37-47 per line; frequency first then time, PAPER.md:83,
+// :180; the time run starts from and substitutes the frequency run's flags, reading F10;
+// statistics over all samples of the stream before any flagging, reading S1).
+int lofo_flag_block(const lofo_params* prm, const float* power, uint32_t* flags,
+                    lofo_stream_stats* stats, double* rowsum, uint32_t* rowcnt,
+                    uint8_t* mask_freq, uint8_t* margin, double margin_rel, int use_literal) {
+  const uint64_t S = prm->n_streams, C = prm->n_channels, T = prm->n_time;
+  if (!S || !C || !T || !prm->max_window || (prm->max_window & (prm->max_window - 1))) return -1;
+  uint32_t n_levels = 0;
+  while (((uint32_t)1 << n_levels) <= prm->max_window) ++n_levels;     // I = 1 .. max_window
+  const uint64_t words = (T + 31) / 32;
+  auto run = use_literal ? lofo_sumthreshold_1d_literal : lofo_sumthreshold_1d_fast;
+  std::vector<uint8_t> M(C * T);
+  std::vector<double> thr(n_levels);
+  for (uint64_t s = 0; s < S; ++s) {
+    const float* X = power + s * C * T;
+    lofo_stream_stats st;
+    lofo_statistics(X, C * T, &st);                                     // O1-O3
+    uint8_t* mg = margin ? margin + s * C * T : nullptr;
+    if (mg) std::memset(mg, 0, C * T);
+    if (st.n_nonfinite) {                                               // reading S6
+      std::fill(M.begin(), M.end(), (uint8_t)1);
+    } else {
+      lofo_threshold_table((double)st.median, st.stddev, prm->start_threshold, prm->p,
+                           prm->sensitivity, n_levels, thr.data());     // O4
+      std::fill(M.begin(), M.end(), (uint8_t)0);                        // O5
+      if (prm->directions & 1u)                                         // O6: along channels
+        for (uint64_t t = 0; t < T; ++t)
+          run(X + t, C, (int64_t)T, M.data() + t, (int64_t)T, thr.data(), n_levels,
+              mg ? mg + t : nullptr, margin_rel);
+      if (mask_freq) std::memcpy(mask_freq + s * C * T, M.data(), C * T);
+      if (prm->directions & 2u)                                         // O7: along time
+        for (uint64_t c = 0; c < C; ++c)
+          run(X + c * T, T, 1, M.data() + c * T, 1, thr.data(), n_levels,
+              mg ? mg + c * T : nullptr, margin_rel);
+    }
+    if (st.n_nonfinite && mask_freq) std::memset(mask_freq + s * C * T, 1, C * T);
+    uint64_t nf = 0;
+    for (uint64_t c = 0; c < C; ++c) {                                  // O8, O9
+      uint32_t* fw = flags + (s * C + c) * words;
+      for (uint64_t w = 0; w < words; ++w) fw[w] = 0;
+      double rs = 0.0; uint32_t rc = 0;
+      for (uint64_t t = 0; t < T; ++t) {
+        if (M[c * T + t]) { fw[t >> 5] |= (uint32_t)1 << (t & 31); ++nf; }
+        else { rs += (double)X[c * T + t]; ++rc; }
+      }
+      if (rowsum) rowsum[s * C + c] = rs;
+      if (rowcnt) rowcnt[s * C + c] = rc;
+    }
+    st.n_flagged = nf;
+    if (stats) stats[s] = st;
+  }
+  return 0;
+}
+
+// ---- history flagger (PAPER.md:87-116 pseudocode; buffer of 32-bit means) ----
+struct lofo_history {
+  lofo_params prm;
+  std::vector<float> ring;        // [S][C][H]
+  std::vector<uint32_t> head, count;
+};
+
+lofo_history* lofo_history_create(const lofo_params* prm) {
+  lofo_history* h = new lofo_history;
+  h->prm = *prm;
+  const uint64_t rows = (uint64_t)prm->n_streams * prm->n_channels;
+  h->ring.assign(rows * prm->history_length, 0.f);
+  h->head.assign(rows, 0);
+  h->count.assign(rows, 0);
+  return h;
+}
+void lofo_history_destroy(lofo_history* h) { delete h; }
+void lofo_history_reset(lofo_history* h) {
+  std::fill(h->ring.begin(), h->ring.end(), 0.f);
+  std::fill(h->head.begin(), h->head.end(), 0u);
+  std::fill(h->count.begin(), h->count.end(), 0u);
+}
+
+void lofo_history_update(lofo_history* h, const double* rowsum, const uint32_t* rowcnt,
+                         uint32_t* flags, uint8_t* row_flagged, uint8_t* near, double near_rel) {
+  const lofo_params& P = h->prm;
+  const uint64_t rows = (uint64_t)P.n_streams * P.n_channels, T = P.n_time, H = P.history_length;
+  const uint64_t words = (T + 31) / 32;
+  const double sens = P.history_sensitivity > 0.0 ? P.history_sensitivity : P.sensitivity;
+  for (uint64_t r = 0; r < rows; ++r) {
+    if (near) near[r] = 0;
+    if (H == 0) { row_flagged[r] = 0; continue; }
+    float* ring = h->ring.data() + r * H;
+    uint32_t& head = h->head[r];
+    uint32_t& cnt = h->count[r];
+    auto push = [&](float v) { ring[head] = v; head = (uint32_t)((head + 1) % H); cnt = std::min<uint32_t>(cnt + 1, (uint32_t)H); };
+    if (rowcnt[r] == 0) { row_flagged[r] = 1; continue; }               // H1
+    const double cur = rowsum[r] / (double)rowcnt[r];                   // H2: meanOfUnflaggedSamples()
+    if (cnt < P.history_min_fill) { push((float)cur); row_flagged[r] = 0; continue; }   // H3
+    double m = 0.0;
+    for (uint32_t i = 0; i < cnt; ++i) m += (double)ring[i];            // H4: meanOfMeans()
+    m /= (double)cnt;
+    double ss = 0.0;
+    for (uint32_t i = 0; i < cnt; ++i) { const double d = (double)ring[i] - m; ss += d * d; }
+    const double sd = std::sqrt(ss / (double)cnt);                      // stddevOfMeans()
+    const double thr = m + sens * sd;                                   // H5
+    if (near && std::fabs(cur - thr) <= near_rel * std::fabs(thr)) near[r] = 1;
+    if (cur < thr) { push((float)cur); row_flagged[r] = 0; }            // H6
+    else {
+      push((float)thr); row_flagged[r] = 1;
+      uint32_t* fw = flags + r * words;
+      for (uint64_t w = 0; w < words; ++w) fw[w] = 0xFFFFFFFFu;
+      if (T & 31) fw[words - 1] = ((uint32_t)1 << (T & 31)) - 1;        // padding bits stay 0
+    }
+  }
+}
+
+void lofo_history_export(const lofo_history* h, float* ring, uint32_t* head, uint32_t* count) {
+  if (ring) std::memcpy(ring, h->ring.data(), h->ring.size() * sizeof(float));
+  if (head) std::memcpy(head, h->head.data(), h->head.size() * sizeof(uint32_t));
+  if (count) std::memcpy(count, h->count.data(), h->count.size() * sizeof(uint32_t));
+}
+
+}  // extern "C"

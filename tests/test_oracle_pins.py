@@ -1,0 +1,344 @@
+"""Pins for the oracle (oracle/lof_oracle.cpp) against what the paper and the mathematics fix.
+CPU only.  Every expected value is the paper's (cited), a closed form, a library routine, a
+hand-worked vector (tests/golden/) or brute force — never the CUDA path's output."""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_1701_08197_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _gold_factors():
+    rows = [l.split() for l in open(os.path.join(GOLD, "factor_table.txt")) if l.strip() and not l.startswith("#")]
+    return [(int(r[0]), float(r[1]), r[2] == "yes") for r in rows]
+
+
+HV = json.load(open(os.path.join(GOLD, "hand_vectors.json")))
+
+
+# ---------------------------------------------------------------- P1: factor table
+def test_factor_table_matches_paper(lofo):
+    gold = _gold_factors()
+    f = lofo.factor_table(len(gold))
+    for k, (I, val, printed) in enumerate(gold):
+        assert I == 1 << k
+        assert f[k] == val, (I, f[k], val)           # exact: 6 * (3/4)^k is a dyadic rational
+    assert f[0] == 6.0 and f[1] == 4.5               # the two values printed at PAPER.md:45
+
+
+def test_factor_formula_readings(lofo):
+    """Only the log2 reading of the garbled exponent gives 4.5 at I=2 (reading F1)."""
+    p, start = 1.5, 6.0
+    assert start * p ** math.log2(2) / 2 == 4.5
+    assert abs(start * p ** (2 * math.log(2)) / 2 - 4.5) > 0.5
+    assert abs(start * p ** (2 * math.log10(2)) / 2 - 4.5) > 0.5
+    f = lofo.factor_table(10, start_threshold=7.0, p=1.2)
+    for k in range(10):
+        assert f[k] == pytest.approx(7.0 * 1.2 ** k / 2 ** k, rel=1e-14)
+
+
+def test_threshold_table(lofo):
+    t = lofo.threshold_table(0.0, 1.0, 2)
+    assert list(t) == [6.0, 4.5]                     # "6 sigma", "4.5 sigma" PAPER.md:45
+    t = lofo.threshold_table(0.7, 2.0, 3, sensitivity=0.5)
+    assert list(t) == pytest.approx([0.7 + 6.0, 0.7 + 4.5, 0.7 + 3.375])
+
+
+# ---------------------------------------------------------------- V1-V3: 1-D hand vectors
+@pytest.mark.parametrize("name", ["V1a", "V1b", "V2", "V3"])
+@pytest.mark.parametrize("literal", [True, False])
+def test_hand_vectors_1d(lofo, name, literal):
+    v = HV[name]
+    m, _ = lofo.sumthreshold_1d(np.array(v["x"], np.float32), v["thr"], literal=literal)
+    assert list(m) == v["expect"], v["why"]
+
+
+def _run2d(lofo, X, thr, order):
+    X = np.array(X, np.float32)
+    Cn, T = X.shape
+
+    def freq(M):
+        M = M.copy()
+        for t in range(T):
+            M[:, t], _ = lofo.sumthreshold_1d(X[:, t], thr, mask=M[:, t], literal=True)
+        return M
+
+    def time(M):
+        M = M.copy()
+        for c in range(Cn):
+            M[c], _ = lofo.sumthreshold_1d(X[c], thr, mask=M[c], literal=True)
+        return M
+
+    Z = np.zeros((Cn, T), np.uint8)
+    if order == "ft":
+        return time(freq(Z))
+    if order == "tf":
+        return freq(time(Z))
+    return freq(Z) | time(Z)
+
+
+def test_hand_vector_v4_direction_order(lofo):
+    v = HV["V4"]
+    assert _run2d(lofo, v["X"], v["thr"], "ft").tolist() == v["expect_freq_then_time"]
+    assert _run2d(lofo, v["X"], v["thr"], "tf").tolist() == v["expect_time_then_freq"]
+    assert _run2d(lofo, v["X"], v["thr"], "or").tolist() == v["expect_independent_or"]
+
+
+def test_block_is_freq_then_time(lofo):
+    """lofo_flag_block = statistics -> thresholds -> frequency run -> time run on the shared mask
+    (PAPER.md:83 'We first flag in the frequency direction'), not the other compositions."""
+    w = W.config1()
+    prm = lofo.make_params(1, w.C, w.T, max_window=32)
+    out = lofo.flag_block(prm, w.power, want_mask_freq=True, literal=True)
+    st = out["stats"][0]
+    thr = lofo.threshold_table(float(st["median"]), st["stddev"], 6)
+    ft = _run2d(lofo, w.power[0], thr, "ft")
+    got = lofo.unpack_flags(out["flags"], w.T)[0]
+    assert np.array_equal(got, ft)
+    assert np.all(got >= out["mask_freq"][0])        # output is a superset of the frequency run
+    # a block on which the three compositions differ, so the check above has teeth
+    rng = np.random.default_rng(2)
+    X = rng.standard_exponential((8, 40)).astype(np.float32)
+    X[2:5, 10:14] += 5.0; X[6, 20:36] += 2.5; X[:, 30] += 3.0
+    stx = lofo.statistics(X)
+    thr = lofo.threshold_table(float(stx["median"]), stx["stddev"], 4)
+    a, b, c = (_run2d(lofo, X, thr, o) for o in ("ft", "tf", "or"))
+    prm = lofo.make_params(1, 8, 40, max_window=8)
+    got = lofo.unpack_flags(lofo.flag_block(prm, X)["flags"], 40)[0]
+    assert np.array_equal(got, a)
+    assert not np.array_equal(a, b) and not np.array_equal(a, c)
+
+
+# ---------------------------------------------------------------- P2: brute force vs fast sums
+def test_fast_equals_literal_random(lofo):
+    rng = np.random.default_rng(1)
+    for trial in range(60):
+        n = int(rng.integers(1, 65))
+        x = rng.standard_exponential(n).astype(np.float32) * rng.choice([1.0, 3.0])
+        pre = (rng.random(n) < rng.choice([0.0, 0.1, 0.5])).astype(np.uint8)
+        thr = lofo.threshold_table(0.7, 1.0 * rng.uniform(0.3, 1.2), 6)
+        a, _ = lofo.sumthreshold_1d(x, thr, mask=pre, literal=True)
+        b, _ = lofo.sumthreshold_1d(x, thr, mask=pre, literal=False)
+        assert np.array_equal(a, b), trial
+
+
+def test_literal_equals_python_bruteforce(lofo):
+    """The literal C++ loop against a from-scratch Python transcription of PAPER.md:37-47."""
+    rng = np.random.default_rng(2)
+    for trial in range(20):
+        n = int(rng.integers(1, 40))
+        x = (rng.standard_exponential(n) * 2).astype(np.float32)
+        pre = (rng.random(n) < 0.15).astype(np.uint8)
+        thr = [4.0, 3.0, 2.25, 1.7, 1.3]
+        M = pre.copy()
+        for k, T in enumerate(thr):
+            I = 1 << k
+            if I > n:
+                break
+            P = M.copy()
+            for t0 in range(n - I + 1):
+                S = sum(T if P[t0 + j] else float(x[t0 + j]) for j in range(I))
+                if S > I * T:
+                    M[t0:t0 + I] = 1
+        got, _ = lofo.sumthreshold_1d(x, thr, mask=pre, literal=True)
+        assert np.array_equal(got, M)
+
+
+def test_block_fast_equals_literal(lofo):
+    w = W.config2(n_stations=2)
+    prm = lofo.make_params(w.S, w.C, w.T, max_window=64)
+    a = lofo.flag_block(prm, w.power, literal=True)
+    b = lofo.flag_block(prm, w.power, literal=False)
+    assert np.array_equal(a["flags"], b["flags"])
+    assert np.array_equal(a["rowcnt"], b["rowcnt"])
+
+
+# ---------------------------------------------------------------- P3: I=1 == simple thresholder
+def test_window1_is_simple_thresholder(lofo):
+    w = W.config2(n_stations=1)
+    prm = lofo.make_params(w.S, w.C, w.T, max_window=1, directions=2)
+    out = lofo.flag_block(prm, w.power)
+    for s in range(w.S):
+        st = out["stats"][s]
+        expect = w.power[s].astype(np.float64) > float(st["median"]) + 6.0 * st["stddev"]
+        assert np.array_equal(lofo.unpack_flags(out["flags"][s], w.T).astype(bool), expect)
+
+
+# ---------------------------------------------------------------- P4: statistics vs library routines
+def test_statistics_vs_numpy(lofo):
+    rng = np.random.default_rng(3)
+    for n in (1, 2, 7, 4096, 49152):
+        x = (rng.standard_exponential(n) * 3 - 0.5).astype(np.float32)
+        st = lofo.statistics(x)
+        assert st["median"] == np.sort(x)[n // 2]                      # rank floor(N/2), bit-exact
+        xl = x.astype(np.longdouble)
+        assert st["mean"] == pytest.approx(float(xl.mean()), rel=1e-13)
+        assert st["stddev"] == pytest.approx(float(np.sqrt(((xl - xl.mean()) ** 2).mean())), rel=1e-12)
+    x[5] = np.inf
+    assert lofo.statistics(x)["n_nonfinite"] == 1
+
+
+# ---------------------------------------------------------------- P5: invariants
+def test_constant_block_no_flags(lofo):
+    for val in (0.0, 1.0, 0.1, 3.3333333, 2048.0):
+        x = np.full((2, 16, 300), val, np.float32)
+        prm = lofo.make_params(2, 16, 300, max_window=64)
+        for lit in (True, False):
+            out = lofo.flag_block(prm, x, literal=lit)
+            assert out["flags"].sum() == 0 and np.all(out["stats"]["stddev"] == 0.0)
+            assert np.all(out["rowcnt"] == 300)
+
+
+def test_spike_above_T1_always_flagged_and_padding_zero(lofo):
+    w = W.config2(n_stations=2, T=700)               # 700 is not a multiple of 32
+    prm = lofo.make_params(w.S, w.C, w.T, max_window=64)
+    out = lofo.flag_block(prm, w.power)
+    m = lofo.unpack_flags(out["flags"], w.T).astype(bool)
+    for s in range(w.S):
+        st = out["stats"][s]
+        assert np.all(m[s][w.power[s].astype(np.float64) > float(st["median"]) + 6.0 * st["stddev"]])
+    assert np.all(out["flags"][..., -1] >> np.uint32(700 % 32) == 0)
+    assert np.array_equal(out["stats"]["n_flagged"], m.reshape(w.S, -1).sum(1))
+    assert np.array_equal(out["rowcnt"], (~m).sum(2))
+    rs = np.where(m, 0.0, w.power.astype(np.float64)).sum(2)
+    assert np.allclose(out["rowsum"], rs, rtol=1e-12)
+
+
+def test_streams_independent(lofo):
+    w = W.config2(n_stations=2)
+    prm = lofo.make_params(w.S, w.C, w.T, max_window=64)
+    a = lofo.flag_block(prm, w.power)["flags"]
+    perm = np.array([2, 0, 3, 1])
+    b = lofo.flag_block(prm, w.power[perm])["flags"]
+    assert np.array_equal(a[perm], b)
+
+
+def test_i1_monotone_in_sensitivity(lofo):
+    """Monotonicity holds for the I=1 iteration only (hand vector V1 shows it fails per sample
+    for the full algorithm)."""
+    w = W.config1()
+    prev = None
+    for sens in (1.4, 1.0, 0.7, 0.4):
+        prm = lofo.make_params(1, w.C, w.T, max_window=1, sensitivity=sens)
+        m = lofo.unpack_flags(lofo.flag_block(prm, w.power)["flags"], w.T)
+        if prev is not None:
+            assert np.all(m >= prev)
+        prev = m
+
+
+def test_nonfinite_stream_fully_flagged(lofo):
+    w = W.config2(n_stations=1, T=100)
+    w.power[1, 3, 50] = np.nan
+    prm = lofo.make_params(w.S, w.C, w.T, max_window=64)
+    out = lofo.flag_block(prm, w.power)
+    m = lofo.unpack_flags(out["flags"], w.T)
+    assert m[1].all() and not m[0].all()
+    assert out["stats"]["n_nonfinite"][1] == 1 and out["stats"]["n_flagged"][1] == w.C * w.T
+
+
+# ---------------------------------------------------------------- P6: closed forms on pure noise
+def test_exponential_noise_closed_forms(lofo):
+    n = 1 << 21
+    x = np.random.default_rng(7).standard_exponential((1, 64, n // 64)).astype(np.float32)
+    prm = lofo.make_params(1, 64, n // 64, max_window=1, directions=2)
+    out = lofo.flag_block(prm, x)
+    st = out["stats"][0]
+    assert float(st["median"]) == pytest.approx(math.log(2), abs(4e-3))     # median of Exp(1)
+    assert st["mean"] == pytest.approx(1.0, abs=4e-3) and st["stddev"] == pytest.approx(1.0, abs=6e-3)
+    rate = out["stats"]["n_flagged"][0] / n
+    expect = 0.5 * math.exp(-6.0)                                            # P(x > ln2 + 6) = e^-6 / 2
+    assert rate == pytest.approx(expect, rel=0.15)
+
+
+# ---------------------------------------------------------------- P7: recall vs ground truth (config 1)
+def test_config1_recall(lofo):
+    w = W.config1()
+    prm = lofo.make_params(1, w.C, w.T, max_window=32)
+    out = lofo.flag_block(prm, w.power)
+    m = lofo.unpack_flags(out["flags"], w.T)[0].astype(bool)
+    cls = w.extra["cls"][0]
+    assert m[cls == 1].mean() == 1.0                  # narrowband channel: caught by time windows
+    assert m[cls == 2].mean() == 1.0                  # broadband spike: caught at I = 1
+    assert m[w.truth[0] == 0].mean() < 0.02           # few false positives
+    # the 8x8 burst at 10x is expected to be largely missed with plain stddev (reading S4): no gate
+
+
+# ---------------------------------------------------------------- margin mask
+def test_margin_mask(lofo):
+    x = np.array([0, 3.0, 6.0 * (1 + 5e-6), 0, 1], np.float32)
+    m, mg = lofo.sumthreshold_1d(x, [6.0], literal=True)
+    assert list(mg) == [0, 0, 1, 0, 0]
+    m, mg = lofo.sumthreshold_1d(x, [6.0, 4.5], literal=False)
+    assert mg[2] == 1 and mg[0] == 0
+
+
+# ---------------------------------------------------------------- V5, V6: history
+def _hist(lofo, H=3, sens=1.0, min_fill=2, T=40):
+    prm = lofo.make_params(1, 1, T, history_length=H, history_min_fill=min_fill, history_sensitivity=sens)
+    return lofo.History(prm), prm
+
+
+def _push(h, cur, T=40, cnt=None):
+    flags = np.zeros((1, 1, (T + 31) // 32), np.uint32)
+    cnt = T if cnt is None else cnt
+    rf, near = h.update(np.array([[cur * cnt]]), np.array([[cnt]], np.uint32), flags)
+    return int(rf[0, 0]), flags
+
+
+def test_history_hand_vector_v5(lofo):
+    v = HV["V5"]
+    for case in v["cases"]:
+        h, _ = _hist(lofo, H=4, sens=v["sensitivity"])
+        for r in v["ring"]:
+            assert _push(h, r)[0] in (0, 1)
+        h2, _ = _hist(lofo, H=4)                      # rebuild ring exactly [1,2,3] without flagging
+        h2.reset()
+        # fill via min_fill bypass: use a large min_fill so values are pushed unconditionally
+        prm = lofo.make_params(1, 1, 40, history_length=4, history_min_fill=3, history_sensitivity=1.0)
+        h3 = lofo.History(prm)
+        for r in v["ring"]:
+            assert _push(h3, r)[0] == 0
+        rf, flags = _push(h3, case["cur"])
+        assert rf == case["flagged"]
+        ring, head, count = h3.export()
+        assert count[0, 0] == 4 and ring[0, 0, 3] == np.float32(case["pushed"])
+        if rf:
+            assert flags[0, 0, 0] == 0xFFFFFFFF and flags[0, 0, 1] == 0xFF      # T = 40: padding stays 0
+        else:
+            assert flags.sum() == 0
+    assert v["thr"] == pytest.approx(2.0 + math.sqrt(2.0 / 3.0), rel=1e-15)
+
+
+def test_history_identical_values_flag(lofo):
+    """Ring of identical values v: thr = v, cur = v is NOT < thr -> flagged."""
+    prm = lofo.make_params(1, 1, 32, history_length=5, history_min_fill=2, history_sensitivity=1.0)
+    h = lofo.History(prm)
+    assert _push(h, 0.5, T=32)[0] == 0 and _push(h, 0.5, T=32)[0] == 0
+    assert _push(h, 0.5, T=32)[0] == 1
+    assert _push(h, 0.25, T=32)[0] == 0
+
+
+def test_history_eviction_and_empty_row(lofo):
+    prm = lofo.make_params(1, 1, 32, history_length=2, history_min_fill=5, history_sensitivity=1.0)
+    h = lofo.History(prm)
+    for v in (1.0, 2.0, 3.0):
+        _push(h, v, T=32)
+    ring, head, count = h.export()
+    assert list(ring[0, 0]) == [3.0, 2.0] and head[0, 0] == 1 and count[0, 0] == 2
+    rf, _ = _push(h, 0.0, T=32, cnt=0)                # H1: no unflagged sample -> flagged, nothing pushed
+    assert rf == 1 and np.array_equal(h.export()[0], ring)
+
+
+def test_history_buffer_sizing_arithmetic():
+    """64*248*256*4 B = 15.5 MByte per second; x300 = 4.5 GBytes;
+    2080*248*256*4 = 504 MByte per second; x300 = 148 GBytes."""
+    pre = 64 * 248 * 256 * 4
+    post = 2080 * 248 * 256 * 4
+    assert pre == 16252928 and round(pre / 2 ** 20, 1) == 15.5
+    assert round(pre * 300 / 2 ** 30, 1) == 4.5
+    assert round(post / 2 ** 20) == 504 and round(post * 300 / 2 ** 30) == 148
