@@ -1,0 +1,145 @@
+/* lof.h — C-ABI boundary of the B200-native LOFAR Online Flagger (LOF) hot path.
+ *
+ * Method: arXiv 1701.08197.  Per-stream statistics, SumThreshold
+ * with windows I = 1, 2, 4, ... and threshold_I = median + stddev * factor_I * sensitivity,
+ * factor_I = startThreshold * p^(log2 I) / I, run along frequency then time
+ * (PAPER.md:83, :180), then the history flagger over consecutive blocks.
+ * The readings taken where the paper is silent or garbled are listed in DESIGN.md §3.
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels (paper_1701_08197_b200/csrc).  There is
+ * no CPU fallback: a call on a machine without a usable CUDA device returns LOF_E_CUDA.
+ *
+ * Conventions
+ *  - A block is power[n_streams][n_channels][n_time], float32, time fastest.  A stream is one
+ *    [n_channels][n_time] slice; statistics, thresholds and flags of a stream depend on that
+ *    stream only.
+ *  - Pointers named d_* are DEVICE pointers owned by the caller, 16-byte aligned, valid until the
+ *    work queued on `cuda_stream` has completed; pointers named h_* are HOST pointers.  The
+ *    library never frees or retains caller pointers.
+ *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
+ *    calls only enqueue work on it and never synchronise the host.
+ *  - Flag bit of sample t of row (s, c): word (s*n_channels + c)*ceil(n_time/32) + t/32,
+ *    bit t%32 (LSB first), 1 = flagged.  Padding bits of a row's last word are 0.
+ *  - Return value: 0 on success, a negative LOF_E_* code otherwise; nothing throws or aborts
+ *    across this boundary.  lof_strerror() gives a static description; after LOF_E_CUDA,
+ *    lof_last_cuda_error() gives the CUDA runtime's text for the calling thread's last failure.
+ */
+#ifndef LOF_H
+#define LOF_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LOF_OK        0
+#define LOF_E_NULL   -1   /* a required pointer is NULL                                         */
+#define LOF_E_PARAM  -2   /* bad lof_params (see lof_create)                                    */
+#define LOF_E_ALIGN  -3   /* a device pointer is not 16-byte aligned                            */
+#define LOF_E_STATE  -4   /* call order violated (see lof_history_update)                       */
+#define LOF_E_CUDA   -5   /* a CUDA runtime call failed, or no usable device                    */
+
+#define LOF_DIR_FREQ 1u   /* SumThreshold along channels (run first)               */
+#define LOF_DIR_TIME 2u   /* SumThreshold along time                                            */
+
+#define LOF_MAX_LEVELS 11 /* windows 1 .. 1024                                                  */
+
+typedef struct lof_ctx lof_ctx;   /* opaque; owns all scratch memory and the history rings */
+
+typedef struct {
+  uint32_t struct_size;         /* = sizeof(lof_params); anything else -> LOF_E_PARAM            */
+  int32_t  device;              /* CUDA device ordinal                                           */
+  uint32_t n_streams;           /* S > 0, fixed for the context                                  */
+  uint32_t n_channels;          /* C > 0 (<= 4096)                                               */
+  uint32_t n_time;              /* T > 0                                                         */
+  float    p;                   /* > 0; paper default 1.5                          */
+  float    sensitivity;         /* > 0; paper default 1.0                          */
+  float    start_threshold;     /* > 0; 6.0 = "6 sigma" at I = 1                   */
+  uint32_t max_window;          /* power of two in 1..1024; "7-10 iterations"      */
+  uint32_t directions;          /* LOF_DIR_FREQ | LOF_DIR_TIME, non-zero; freq always runs first */
+  uint32_t history_length;      /* H entries per (stream, channel) ring; 0 disables the history
+                                   flagger; the paper's example is 300            */
+  uint32_t history_min_fill;    /* below this many entries a ring only records (H3')   */
+  float    history_sensitivity; /* <= 0: use `sensitivity`, the literal text of PAPER.md:106     */
+} lof_params;
+
+/* Per-stream results of lof_flag_block (32 bytes, no padding surprises: 4+4+8+8+8). */
+typedef struct {
+  float    median;       /* element of rank floor(N/2) of the stream's N = C*T samples (bit-exact) */
+  uint32_t n_nonfinite;  /* NaN/Inf samples; if > 0 the whole stream is flagged and the other
+                            fields except n_flagged are unspecified (S6)                 */
+  double   mean;         /* of all N samples, before any flagging (S1)      */
+  double   stddev;       /* population standard deviation about the mean                           */
+  uint64_t n_flagged;    /* flagged samples of the stream after the SumThreshold runs              */
+} lof_stream_stats;
+
+/* Validate params (LOF_E_PARAM when: struct_size mismatch; S, C or T zero; C > 4096; max_window
+ * zero, not a power of two or > 1024; directions zero or with unknown bits; p, sensitivity or
+ * start_threshold not > 0 and finite), select the device, allocate scratch and history rings
+ * (zero-filled, all rings empty).  *out receives the handle; on failure *out = NULL. */
+int lof_create(const lof_params* params, lof_ctx** out);
+
+/* Frees everything the context owns.  Synchronises the device first.  NULL is accepted. */
+int lof_destroy(lof_ctx* ctx);
+
+/* One pass of the hot path over one block:
+ *   statistics -> thresholds -> SumThreshold(frequency) -> SumThreshold(time) -> bit-pack,
+ *   per-row sums of unflagged samples (kept inside the context for lof_history_update).
+ * d_power [S][C][T] float32 (in), d_flags [S][C][ceil(T/32)] uint32 (out, fully overwritten),
+ * d_stats [S] (out, may be NULL).  Asynchronous on cuda_stream. */
+int lof_flag_block(lof_ctx* ctx, const float* d_power, uint32_t* d_flags,
+                   lof_stream_stats* d_stats, void* cuda_stream);
+
+/* Same, for raw complex voltages ("we may have to compute amplitudes first"):
+ * d_volt [S][C][T][2] int16 (re, im); the power x = (float)(uint32)(re*re + im*im) is formed in
+ * registers on load and never written to memory (S5). */
+int lof_flag_block_ci16(lof_ctx* ctx, const int16_t* d_volt, uint32_t* d_flags,
+                        lof_stream_stats* d_stats, void* cuda_stream);
+
+/* History flagger (PAPER.md:97-113 pseudocode), one ring per (stream, channel):
+ *   cur = mean of the row's unflagged samples of the block just flagged;
+ *   thr = mean(ring) + history_sensitivity * stddev(ring);
+ *   cur < thr: push cur; else push thr and flag the whole row in d_flags.
+ * d_flags (in/out) must be the flags lof_flag_block wrote for that block; d_row_flagged [S][C]
+ * uint8 (out, may be NULL) is 1 for rows flagged here (or left without any unflagged sample).
+ * LOF_E_STATE if no lof_flag_block call precedes it or it was already called for that block,
+ * or if history_length == 0.  Asynchronous on cuda_stream. */
+int lof_history_update(lof_ctx* ctx, uint32_t* d_flags, uint8_t* d_row_flagged, void* cuda_stream);
+
+/* Empties every history ring (asynchronous on cuda_stream). */
+int lof_reset(lof_ctx* ctx, void* cuda_stream);
+
+/* Read-only views of context-owned device buffers written by the last lof_flag_block:
+ * rowsum [S][C] double = sum of unflagged samples per row, rowcnt [S][C] uint32 = their number
+ * (what PAPER.md:102 "meanOfUnflaggedSamples" is formed from).  Valid until lof_destroy. */
+int lof_row_sums(lof_ctx* ctx, const double** d_rowsum, const uint32_t** d_rowcnt);
+
+/* Copies the history state to caller DEVICE buffers (any may be NULL): ring [S][C][H] float32,
+ * head [S][C] uint32 (next write position), count [S][C] uint32.  Asynchronous. */
+int lof_history_export(lof_ctx* ctx, float* d_ring, uint32_t* d_head, uint32_t* d_count,
+                       void* cuda_stream);
+
+/* End-to-end convenience with HOST buffers: copies h_power (or h_volt when is_ci16 != 0) to a
+ * context-owned device buffer, runs lof_flag_block[_ci16], copies flags and stats back and
+ * synchronises.  h_stats may be NULL.  Pinned host memory makes the copies asynchronous to
+ * each other; pageable memory works too. */
+int lof_flag_block_host(lof_ctx* ctx, const void* h_input, int is_ci16, uint32_t* h_flags,
+                        lof_stream_stats* h_stats);
+
+/* Host only: factor_I = start_threshold * (p/2)^k for I = 2^k, k = 0..n_out-1. */
+int lof_factor_table(const lof_params* params, double* h_out, uint32_t n_out);
+
+/* Number of kernel launches the library has enqueued for this context so far (bench.py's
+ * gpu_launches is the difference over the timed region). */
+uint64_t lof_launch_count(const lof_ctx* ctx);
+
+/* Selects the kernel path: 0 = automatic (fused kernels where the shape allows), 1 = force the
+ * generic multi-kernel path.  Both compute the same results; for tests and profiling. */
+int lof_set_path(lof_ctx* ctx, int path);
+
+const char* lof_strerror(int code);
+const char* lof_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LOF_H */

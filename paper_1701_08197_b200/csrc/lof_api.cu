@@ -1,0 +1,341 @@
+// lof_api.cu — host side of the C-ABI in include/lof.h: context, scratch, launch sequencing.
+// Every compute step is a kernel launch on the caller's stream; nothing here computes on the CPU
+// except the factor table and launch geometry.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "lof_common.cuh"
+#include "lof_stats.cuh"
+#include "lof_flag_generic.cuh"
+#include "lof_history.cuh"
+#include "lof_fused.cuh"
+
+static thread_local char g_cuda_err[256] = "";
+
+#define LOF_CUDA(call)                                                              \
+  do {                                                                              \
+    cudaError_t e_ = (call);                                                        \
+    if (e_ != cudaSuccess) {                                                        \
+      snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s", #call, cudaGetErrorString(e_)); \
+      return LOF_E_CUDA;                                                            \
+    }                                                                               \
+  } while (0)
+
+struct lof_ctx {
+  lof_params prm;
+  LofKParams kp;
+  int path;                       // 0 auto, 1 force generic
+  int sm_count;
+  uint64_t launches;
+  bool block_pending;             // a lof_flag_block result is waiting for lof_history_update
+  // geometry of the generic path
+  uint32_t group;                 // streams per group (bounded so a group's input stays in L2)
+  uint32_t n_chunks;              // statistics chunks per stream
+  uint32_t TT, halo, n_tiles;     // time tiling
+  size_t smem_freq, smem_time;
+  // device memory owned by the context
+  LofStreamState* d_state;
+  uint32_t* d_hist;               // [group][2048]
+  double* d_partial;              // [group][n_chunks][2]
+  uint32_t* d_fmask;              // [S][C][W] mask after the frequency run
+  double* d_part_sum;             // [group*C][n_tiles]
+  uint32_t* d_part_cnt;
+  double* d_rowsum;               // [S][C]
+  uint32_t* d_rowcnt;
+  lof_stream_stats* d_stats;      // [S] internal copy
+  float* d_ring;                  // [S][C][H]
+  uint32_t* d_head; uint32_t* d_count;
+  uint8_t* d_row_flagged;
+  // staging for lof_flag_block_host
+  void* d_in_stage; size_t in_stage_bytes;
+  uint32_t* d_flags_stage;
+  cudaStream_t host_stream;
+};
+
+static bool is_pow2(uint32_t v) { return v && !(v & (v - 1)); }
+
+static int validate(const lof_params* p) {
+  if (!p) return LOF_E_NULL;
+  if (p->struct_size != sizeof(lof_params)) return LOF_E_PARAM;
+  if (!p->n_streams || !p->n_channels || !p->n_time) return LOF_E_PARAM;
+  if (p->n_channels > 256) return LOF_E_PARAM;
+  if (!is_pow2(p->max_window) || p->max_window > 1024) return LOF_E_PARAM;
+  if (!p->directions || (p->directions & ~3u)) return LOF_E_PARAM;
+  if (!(p->p > 0.f) || !std::isfinite(p->p)) return LOF_E_PARAM;
+  if (!(p->sensitivity > 0.f) || !std::isfinite(p->sensitivity)) return LOF_E_PARAM;
+  if (!(p->start_threshold > 0.f) || !std::isfinite(p->start_threshold)) return LOF_E_PARAM;
+  if ((uint64_t)p->n_channels * p->n_time > 0xFFFFFFFFull) return LOF_E_PARAM;
+  return LOF_OK;
+}
+
+extern "C" int lof_factor_table(const lof_params* p, double* out, uint32_t n_out) {
+  if (!p || !out) return LOF_E_NULL;
+  // factor_I = startThreshold * p^(log2 I) / I = startThreshold * (p/2)^k, I = 2^k
+  double f = (double)p->start_threshold;
+  const double r = (double)p->p / 2.0;
+  for (uint32_t k = 0; k < n_out; ++k) { out[k] = f; f *= r; }
+  return LOF_OK;
+}
+
+extern "C" const char* lof_strerror(int code) {
+  switch (code) {
+    case LOF_OK: return "success";
+    case LOF_E_NULL: return "required pointer is NULL";
+    case LOF_E_PARAM: return "invalid parameter";
+    case LOF_E_ALIGN: return "device pointer not 16-byte aligned";
+    case LOF_E_STATE: return "call order violated";
+    case LOF_E_CUDA: return "CUDA runtime failure (see lof_last_cuda_error)";
+    default: return "unknown error";
+  }
+}
+extern "C" const char* lof_last_cuda_error(void) { return g_cuda_err; }
+
+template <class T>
+static cudaError_t dev_alloc(T** p, size_t n) {
+  *p = nullptr;
+  if (n == 0) n = 1;
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T));
+  if (e == cudaSuccess) e = cudaMemset(*p, 0, n * sizeof(T));
+  return e;
+}
+
+extern "C" int lof_destroy(lof_ctx* c) {
+  if (!c) return LOF_OK;
+  cudaSetDevice(c->prm.device);
+  cudaDeviceSynchronize();
+  cudaFree(c->d_state); cudaFree(c->d_hist); cudaFree(c->d_partial); cudaFree(c->d_fmask);
+  cudaFree(c->d_part_sum); cudaFree(c->d_part_cnt); cudaFree(c->d_rowsum); cudaFree(c->d_rowcnt);
+  cudaFree(c->d_stats); cudaFree(c->d_ring); cudaFree(c->d_head); cudaFree(c->d_count);
+  cudaFree(c->d_row_flagged); cudaFree(c->d_in_stage); cudaFree(c->d_flags_stage);
+  if (c->host_stream) cudaStreamDestroy(c->host_stream);
+  delete c;
+  return LOF_OK;
+}
+
+static cudaError_t lof_generic_set_attributes(size_t smem_freq, size_t smem_time) {
+  cudaError_t e = cudaSuccess;
+  auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  const int f = (int)smem_freq, t = (int)smem_time;
+  A(cudaFuncSetAttribute(lof_k_freq_generic<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, f));
+  A(cudaFuncSetAttribute(lof_k_freq_generic<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, f));
+  A(cudaFuncSetAttribute(lof_k_time_generic<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, t));
+  A(cudaFuncSetAttribute(lof_k_time_generic<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, t));
+  return e;
+}
+
+static uint32_t ilog2(uint32_t v) { uint32_t k = 0; while ((1u << (k + 1)) <= v) ++k; return k; }
+
+extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
+  if (!out) return LOF_E_NULL;
+  *out = nullptr;
+  int rc = validate(p);
+  if (rc) return rc;
+  int ndev = 0;
+  LOF_CUDA(cudaGetDeviceCount(&ndev));
+  if (p->device < 0 || p->device >= ndev) {
+    snprintf(g_cuda_err, sizeof g_cuda_err, "device %d not present (%d devices)", p->device, ndev);
+    return LOF_E_CUDA;
+  }
+  LOF_CUDA(cudaSetDevice(p->device));
+  lof_ctx* c = new (std::nothrow) lof_ctx();
+  if (!c) return LOF_E_CUDA;
+  memset(c, 0, sizeof *c);
+  c->prm = *p;
+  LOF_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, p->device));
+  const uint32_t S = p->n_streams, C = p->n_channels, T = p->n_time, W = (T + 31) / 32;
+  LofKParams& kp = c->kp;
+  kp.S = S; kp.C = C; kp.T = T; kp.W = W;
+  kp.n_levels = ilog2(p->max_window) + 1;
+  kp.n_lev_f = (p->directions & LOF_DIR_FREQ) ? ilog2(p->max_window < C ? p->max_window : C) + 1 : 0;
+  kp.n_lev_t = (p->directions & LOF_DIR_TIME) ? ilog2(p->max_window < T ? p->max_window : T) + 1 : 0;
+  kp.s0 = 0;
+  lof_factor_table(p, kp.factor, LOF_MAX_LEVELS);
+  kp.sensitivity = (double)p->sensitivity;
+
+  const uint64_t N = (uint64_t)C * T;
+  c->n_chunks = (uint32_t)((N + LOF_STATS_CHUNK - 1) / LOF_STATS_CHUNK);
+  // groups: keep one group's input (read four to five times by the generic path) inside L2
+  const uint64_t group_bytes = 48ull << 20;
+  uint64_t g = group_bytes / (N * 4);
+  if (g < 1) g = 1;
+  if (g > S) g = S;
+  c->group = (uint32_t)g;
+  // time tiling: halo = dependency cone sum_k (2^k - 1) of the time run, rounded up to 32
+  uint32_t cone = 0;
+  for (uint32_t k = 0; k < kp.n_lev_t; ++k) cone += (1u << k) - 1;
+  const uint32_t TT0 = 4096;
+  if (T <= TT0 + 2 * ((cone + 31) & ~31u)) { c->TT = (T + 31) & ~31u; c->halo = 0; c->n_tiles = 1; }
+  else { c->TT = TT0; c->halo = (cone + 31) & ~31u; c->n_tiles = (T + TT0 - 1) / TT0; }
+  c->smem_freq = (size_t)C * 32 * LOF_GEN_BYTES_PER_ELEM;
+  c->smem_time = (size_t)((c->TT + 2 * c->halo + 31) & ~31u) * LOF_GEN_BYTES_PER_ELEM;
+
+  cudaError_t e = cudaSuccess;
+  auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  A(dev_alloc(&c->d_state, S));
+  A(dev_alloc(&c->d_hist, (size_t)c->group * LOF_HIST_BINS));
+  A(dev_alloc(&c->d_partial, (size_t)c->group * c->n_chunks * 2));
+  A(dev_alloc(&c->d_fmask, (size_t)S * C * W));
+  A(dev_alloc(&c->d_part_sum, (size_t)c->group * C * c->n_tiles));
+  A(dev_alloc(&c->d_part_cnt, (size_t)c->group * C * c->n_tiles));
+  A(dev_alloc(&c->d_rowsum, (size_t)S * C));
+  A(dev_alloc(&c->d_rowcnt, (size_t)S * C));
+  A(dev_alloc(&c->d_stats, S));
+  A(dev_alloc(&c->d_ring, (size_t)S * C * p->history_length));
+  A(dev_alloc(&c->d_head, (size_t)S * C));
+  A(dev_alloc(&c->d_count, (size_t)S * C));
+  A(dev_alloc(&c->d_row_flagged, (size_t)S * C));
+  if (e == cudaSuccess) e = lof_generic_set_attributes(c->smem_freq, c->smem_time);
+  if (e != cudaSuccess) {
+    snprintf(g_cuda_err, sizeof g_cuda_err, "lof_create: %s", cudaGetErrorString(e));
+    lof_destroy(c);
+    return LOF_E_CUDA;
+  }
+  *out = c;
+  return LOF_OK;
+}
+
+// ---- the hot path: statistics -> thresholds -> SumThreshold(freq) -> SumThreshold(time) -> pack
+template <class In>
+static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t st) {
+  const uint32_t S = c->prm.n_streams, C = c->prm.n_channels;
+  for (uint32_t s0 = 0; s0 < S; s0 += c->group) {
+    const uint32_t G = (S - s0 < c->group) ? S - s0 : c->group;
+    LofKParams kp = c->kp;
+    kp.s0 = s0;
+    const uint32_t nb = G * c->n_chunks;
+    lof_k_clear_state<<<(G + 255) / 256, 256, 0, st>>>(c->d_state, s0, G);
+    lof_k_hist<In, 0><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
+    lof_k_scan<In, 0><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
+    lof_k_hist<In, 1><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
+    lof_k_scan<In, 1><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
+    lof_k_hist<In, 2><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
+    lof_k_scan<In, 2><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
+    c->launches += 7;
+    if (kp.n_lev_f) {
+      lof_k_freq_generic<In><<<G * kp.W, LOF_GEN_THREADS, c->smem_freq, st>>>(in, kp, c->d_state, c->d_fmask);
+      c->launches += 1;
+    }
+    const uint32_t rows = G * C;
+    lof_k_time_generic<In><<<rows * c->n_tiles, LOF_GEN_THREADS, c->smem_time, st>>>(
+        in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum, c->d_part_cnt, c->d_stats, c->TT, c->halo, c->n_tiles);
+    lof_k_rowsum_final<<<(rows + 255) / 256, 256, 0, st>>>(c->d_part_sum, c->d_part_cnt, c->d_rowsum, c->d_rowcnt,
+                                                           (uint64_t)s0 * C, rows, c->n_tiles);
+    c->launches += 2;
+  }
+  LOF_CUDA(cudaGetLastError());
+  return LOF_OK;
+}
+
+template <class In>
+static int flag_block_any(lof_ctx* c, In in, uint32_t* d_flags, lof_stream_stats* d_stats, void* cuda_stream) {
+  if (!c || !in.p || !d_flags) return LOF_E_NULL;
+  if (((uintptr_t)in.p & 15) || ((uintptr_t)d_flags & 15) || ((uintptr_t)d_stats & 7)) return LOF_E_ALIGN;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  int rc = flag_block_generic(c, in, d_flags, st);
+  if (rc) return rc;
+  if (d_stats)
+    LOF_CUDA(cudaMemcpyAsync(d_stats, c->d_stats, (size_t)c->prm.n_streams * sizeof(lof_stream_stats),
+                             cudaMemcpyDeviceToDevice, st));
+  c->block_pending = true;
+  return LOF_OK;
+}
+
+extern "C" int lof_flag_block(lof_ctx* c, const float* d_power, uint32_t* d_flags, lof_stream_stats* d_stats,
+                              void* cuda_stream) {
+  return flag_block_any(c, InF32{d_power}, d_flags, d_stats, cuda_stream);
+}
+extern "C" int lof_flag_block_ci16(lof_ctx* c, const int16_t* d_volt, uint32_t* d_flags, lof_stream_stats* d_stats,
+                                   void* cuda_stream) {
+  return flag_block_any(c, InCI16{d_volt}, d_flags, d_stats, cuda_stream);
+}
+
+extern "C" int lof_history_update(lof_ctx* c, uint32_t* d_flags, uint8_t* d_row_flagged, void* cuda_stream) {
+  if (!c || !d_flags) return LOF_E_NULL;
+  if ((uintptr_t)d_flags & 15) return LOF_E_ALIGN;
+  if (!c->block_pending || c->prm.history_length == 0) return LOF_E_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  const uint64_t rows = (uint64_t)c->prm.n_streams * c->prm.n_channels;
+  const double sens = c->prm.history_sensitivity > 0.f ? (double)c->prm.history_sensitivity
+                                                       : (double)c->prm.sensitivity;
+  lof_k_history_decide<<<(unsigned)((rows + 127) / 128), 128, 0, st>>>(
+      c->d_ring, c->d_head, c->d_count, c->d_rowsum, c->d_rowcnt, c->d_row_flagged, rows,
+      c->prm.history_length, c->prm.history_min_fill, sens);
+  lof_k_history_fill<<<(unsigned)((rows * 32 + 255) / 256), 256, 0, st>>>(c->d_row_flagged, d_flags, rows,
+                                                                         c->kp.W, c->prm.n_time);
+  c->launches += 2;
+  LOF_CUDA(cudaGetLastError());
+  if (d_row_flagged)
+    LOF_CUDA(cudaMemcpyAsync(d_row_flagged, c->d_row_flagged, rows, cudaMemcpyDeviceToDevice, st));
+  c->block_pending = false;
+  return LOF_OK;
+}
+
+extern "C" int lof_reset(lof_ctx* c, void* cuda_stream) {
+  if (!c) return LOF_E_NULL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  const size_t rows = (size_t)c->prm.n_streams * c->prm.n_channels;
+  LOF_CUDA(cudaMemsetAsync(c->d_ring, 0, rows * c->prm.history_length * sizeof(float) + (c->prm.history_length ? 0 : 4), st));
+  LOF_CUDA(cudaMemsetAsync(c->d_head, 0, rows * 4, st));
+  LOF_CUDA(cudaMemsetAsync(c->d_count, 0, rows * 4, st));
+  c->block_pending = false;
+  return LOF_OK;
+}
+
+extern "C" int lof_row_sums(lof_ctx* c, const double** d_rowsum, const uint32_t** d_rowcnt) {
+  if (!c) return LOF_E_NULL;
+  if (d_rowsum) *d_rowsum = c->d_rowsum;
+  if (d_rowcnt) *d_rowcnt = c->d_rowcnt;
+  return LOF_OK;
+}
+
+extern "C" int lof_history_export(lof_ctx* c, float* d_ring, uint32_t* d_head, uint32_t* d_count, void* cuda_stream) {
+  if (!c) return LOF_E_NULL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  const size_t rows = (size_t)c->prm.n_streams * c->prm.n_channels;
+  if (d_ring && c->prm.history_length)
+    LOF_CUDA(cudaMemcpyAsync(d_ring, c->d_ring, rows * c->prm.history_length * 4, cudaMemcpyDeviceToDevice, st));
+  if (d_head) LOF_CUDA(cudaMemcpyAsync(d_head, c->d_head, rows * 4, cudaMemcpyDeviceToDevice, st));
+  if (d_count) LOF_CUDA(cudaMemcpyAsync(d_count, c->d_count, rows * 4, cudaMemcpyDeviceToDevice, st));
+  return LOF_OK;
+}
+
+extern "C" int lof_flag_block_host(lof_ctx* c, const void* h_input, int is_ci16, uint32_t* h_flags,
+                                   lof_stream_stats* h_stats) {
+  if (!c || !h_input || !h_flags) return LOF_E_NULL;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  const size_t n = (size_t)c->prm.n_streams * c->prm.n_channels * c->prm.n_time;
+  const size_t in_bytes = n * 4;                        // float32, or 2 x int16
+  const size_t fl_bytes = (size_t)c->prm.n_streams * c->prm.n_channels * c->kp.W * 4;
+  if (!c->host_stream) LOF_CUDA(cudaStreamCreateWithFlags(&c->host_stream, cudaStreamNonBlocking));
+  if (!c->d_in_stage) {
+    LOF_CUDA(cudaMalloc(&c->d_in_stage, in_bytes));
+    LOF_CUDA(cudaMalloc(reinterpret_cast<void**>(&c->d_flags_stage), fl_bytes));
+    c->in_stage_bytes = in_bytes;
+  }
+  cudaStream_t st = c->host_stream;
+  LOF_CUDA(cudaMemcpyAsync(c->d_in_stage, h_input, in_bytes, cudaMemcpyHostToDevice, st));
+  int rc = is_ci16 ? lof_flag_block_ci16(c, (const int16_t*)c->d_in_stage, c->d_flags_stage, nullptr, st)
+                   : lof_flag_block(c, (const float*)c->d_in_stage, c->d_flags_stage, nullptr, st);
+  if (rc) return rc;
+  LOF_CUDA(cudaMemcpyAsync(h_flags, c->d_flags_stage, fl_bytes, cudaMemcpyDeviceToHost, st));
+  if (h_stats)
+    LOF_CUDA(cudaMemcpyAsync(h_stats, c->d_stats, (size_t)c->prm.n_streams * sizeof(lof_stream_stats),
+                             cudaMemcpyDeviceToHost, st));
+  LOF_CUDA(cudaStreamSynchronize(st));
+  return LOF_OK;
+}
+
+extern "C" uint64_t lof_launch_count(const lof_ctx* c) { return c ? c->launches : 0; }
+
+extern "C" int lof_set_path(lof_ctx* c, int path) {
+  if (!c) return LOF_E_NULL;
+  if (path < 0 || path > 1) return LOF_E_PARAM;
+  c->path = path;
+  return LOF_OK;
+}

@@ -1,0 +1,83 @@
+// lof_common.cuh — shared device-side definitions of the LOF CUDA path (sm_100a).
+// Nothing here is shared with oracle/ (the oracle is written separately from PAPER.md).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/lof.h"
+
+#define LOF_HIST_BINS 2048
+
+// Per-stream device state: statistics, radix-select progress, thresholds.
+struct LofStreamState {
+  double   shift;                  // K = first sample; sums are of (x - K) (statistics)
+  double   sum, sumsq;             // sum (x-K), sum (x-K)^2 over the stream, fixed reduction order
+  double   mean, stddev;
+  double   thr_d[LOF_MAX_LEVELS];  // threshold_I, fp64
+  float    thr_f[LOF_MAX_LEVELS];  // same rounded to fp32: what the flag kernels compare against
+  uint32_t nonfinite;
+  uint32_t prefix;                 // radix select: key bits fixed so far
+  uint32_t rank;                   // rank still to find among keys matching prefix
+  float    median;
+  uint32_t pad_;
+};
+
+// Parameters every kernel needs, passed by value.
+struct LofKParams {
+  uint32_t S, C, T, W;             // W = ceil(T/32) flag words per row
+  uint32_t n_levels;               // log2(max_window)+1
+  uint32_t n_lev_f, n_lev_t;       // levels actually run along frequency / time (0 = direction off)
+  uint32_t s0;                     // first stream of the group this launch works on
+  double   factor[LOF_MAX_LEVELS]; // factor_I, fp64, host-computed
+  double   sensitivity;
+};
+
+// Monotone map float -> uint32: ascending keys <=> ascending floats (radix select on bit patterns).
+__device__ __forceinline__ uint32_t lof_key(float x) {
+  uint32_t b = __float_as_uint(x);
+  return b ^ ((b >> 31) ? 0xFFFFFFFFu : 0x80000000u);
+}
+__device__ __forceinline__ float lof_unkey(uint32_t k) {
+  uint32_t b = (k >> 31) ? (k ^ 0x80000000u) : ~k;
+  return __uint_as_float(b);
+}
+__device__ __forceinline__ bool lof_finite(float x) {
+  return (__float_as_uint(x) & 0x7F800000u) != 0x7F800000u;
+}
+
+// Input adapters: float32 power, or complex int16 voltages turned into power on load
+// (x = (float)(uint32)(re*re + im*im), integer-exact, S5).
+struct InF32 {
+  const float* p;
+  __device__ __forceinline__ float ld(size_t i) const { return __ldg(p + i); }
+  static constexpr int kBytes = 4;
+};
+struct InCI16 {
+  const int16_t* p;
+  __device__ __forceinline__ float ld(size_t i) const {
+    const short2 v = __ldg(reinterpret_cast<const short2*>(p) + i);
+    const int re = v.x, im = v.y;
+    return __uint2float_rn((unsigned)(re * re + im * im));
+  }
+  static constexpr int kBytes = 4;
+};
+
+// Deterministic block reduction of a double (fixed shuffle tree, then warp 0 in warp order).
+__device__ __forceinline__ double lof_warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double lof_block_sum(double v, double* sh /* >= 32 doubles */) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  v = lof_warp_sum(v);
+  __syncthreads();
+  if (lane == 0) sh[w] = v;
+  __syncthreads();
+  double r = 0.0;
+  if (w == 0) {
+    r = lane < nw ? sh[lane] : 0.0;
+    r = lof_warp_sum(r);
+  }
+  return r;   // valid in thread 0
+}

@@ -1,0 +1,201 @@
+"""GPU parity tests: the CUDA path (through the C-ABI, paper_1701_08197_b200.lof) against the CPU
+oracle (oracle/) on the same seeded inputs.  Rules: median bit-exact; mean, stddev <= 1e-6 relative;
+flags bit-exact except samples explained by an oracle margin bit (window sum within 1e-5 relative of
+its threshold), which must total <= 1e-6 of samples (BASELINE.json north_star)."""
+import numpy as np
+import pytest
+
+from parity import assert_flags, assert_stats, unpack
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lof():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1701_08197_b200 import build, lof as m
+    build.build_lib()
+    return m
+
+
+@pytest.fixture(scope="module")
+def wl():
+    from paper_1701_08197_b200 import workloads
+    return workloads
+
+
+def run_gpu(lof, power, S, C, T, path=0, **kw):
+    import torch
+    f = lof.Flagger(S, C, T, **kw)
+    f.set_path(path)
+    x = torch.from_numpy(np.ascontiguousarray(power)).cuda()
+    flags, stats = f.flag_block(x)
+    torch.cuda.synchronize()
+    rs, rc = f.row_sums()
+    out = dict(flags=lof.flags_to_numpy(flags), stats=lof.stats_to_numpy(stats),
+               rowsum=rs.cpu().numpy(), rowcnt=rc.cpu().numpy().view(np.uint32))
+    f.close()
+    return out
+
+
+def run_oracle(lofo, power, S, C, T, threads=8, **kw):
+    prm = lofo.make_params(S, C, T, **kw)
+    return lofo.flag_block_threads(prm, power, threads, want_margin=True)
+
+
+def check(lof, lofo, power, S, C, T, exact=False, volt=None, paths=(0, 1), **kw):
+    if volt is not None:
+        power = lofo.power_from_ci16(volt)
+    ora = run_oracle(lofo, power, S, C, T, **kw)
+    res = None
+    for path in paths:
+        g = run_gpu(lof, volt if volt is not None else power, S, C, T, path=path, **kw)
+        assert_stats(g["stats"], ora["stats"])
+        res = assert_flags(g["flags"], ora, T, kw.get("max_window", 64), exact=exact)
+        if res["n_mismatch"] == 0:
+            assert np.array_equal(g["stats"]["n_flagged"], ora["stats"]["n_flagged"])
+            assert np.array_equal(g["rowcnt"], ora["rowcnt"])
+            np.testing.assert_allclose(g["rowsum"], ora["rowsum"], rtol=1e-12, atol=0)
+        # padding bits are zero
+        if T % 32:
+            assert (g["flags"][..., -1] >> np.uint32(T % 32)).max() == 0
+    return res, ora
+
+
+def test_config1_exact(lof, lofo, wl):
+    w = wl.config1(0)
+    res, ora = check(lof, lofo, w.power, 1, 16, 256, exact=True, max_window=32)
+    m = unpack(ora["flags"], 256)
+    assert m[0, 5].all() and m[0, :, 100].all()          # narrowband channel and broadband spike found
+
+
+def test_config2_one_subband(lof, lofo, wl):
+    w = wl.config2(0, n_subbands=1)
+    res, _ = check(lof, lofo, w.power, w.S, 64, 768, max_window=64)
+    print("cfg2", res)
+
+
+def test_config3_cut(lof, lofo, wl):
+    w = wl.config3(0, max_baselines=40)
+    res, _ = check(lof, lofo, w.power, w.S, 16, 768, max_window=64)
+    print("cfg3", res)
+
+
+def test_config4_cut_ci16(lof, lofo, wl):
+    # 2 stations x 2 pol, 32 subbands, ragged long time axis spanning several time tiles
+    w = wl.config4(0, n_stations=2, T=20011)
+    res, _ = check(lof, lofo, None, w.S, 32, 20011, volt=w.volt, max_window=256)
+    print("cfg4", res)
+
+
+def test_config5_cut_with_history(lof, lofo, wl):
+    import torch
+    S, C, T, H = 6, 16, 12208, 4
+    gen = wl.Config5Stream(0, S=S, C=C, T=T)
+    kw = dict(max_window=64, history_length=H, history_min_fill=2)
+    f = lof.Flagger(S, C, T, **kw)
+    prm = lofo.make_params(S, C, T, **kw)
+    hist = lofo.History(prm)
+    n_row_flagged = 0
+    for k in range(7):
+        w = gen.next_block()
+        ora = lofo.flag_block_threads(prm, w.power, 8, want_margin=True)
+        flags, stats = f.flag_block(torch.from_numpy(w.power).cuda())
+        torch.cuda.synchronize()
+        g = lof.flags_to_numpy(flags)
+        assert_stats(lof.stats_to_numpy(stats), ora["stats"])
+        r = assert_flags(g, ora, T, 64)
+        assert r["n_mismatch"] == 0              # needed so that the row means below are comparable
+        oflags = ora["flags"].copy()
+        rf_o, near = hist.update(ora["rowsum"], ora["rowcnt"], oflags)
+        rf_g = f.history_update(flags)
+        torch.cuda.synchronize()
+        rf_g = rf_g.cpu().numpy()
+        differ = rf_g != rf_o
+        assert not (differ & (near == 0)).any()   # decisions may differ only at near-ties
+        if not differ.any():
+            assert np.array_equal(lof.flags_to_numpy(flags), oflags)
+            ring_g, head_g, cnt_g = [a.cpu().numpy() for a in f.history_export()]
+            ring_o, head_o, cnt_o = hist.export()
+            assert np.array_equal(head_g.view(np.uint32), head_o) and np.array_equal(cnt_g.view(np.uint32), cnt_o)
+            np.testing.assert_allclose(ring_g, ring_o, rtol=1e-6)
+        n_row_flagged += int(rf_o.sum())
+    assert n_row_flagged > 0                      # the history flagger did act (and H = 4 evicted)
+    # call-order errors
+    with pytest.raises(lof.LofError) as e:
+        f.history_update(flags)
+    assert e.value.code == lof.E_STATE
+    f.reset()
+    ring_g, head_g, cnt_g = [a.cpu().numpy() for a in f.history_export()]
+    assert not cnt_g.any() and not head_g.any()
+    f.close()
+
+
+@pytest.mark.parametrize("S,C,T,mw,dirs", [
+    (3, 5, 77, 8, 3), (2, 1, 100, 16, 3), (2, 7, 1, 4, 3), (1, 3, 33, 64, 3), (2, 16, 256, 32, 1),
+    (2, 16, 256, 32, 2), (1, 64, 768, 1, 3), (2, 48, 1000, 1024, 3), (1, 256, 40, 256, 3), (1, 2, 9000, 128, 3)])
+def test_ragged_shapes(lof, lofo, S, C, T, mw, dirs):
+    rng = np.random.default_rng(S * 1000 + C * 10 + T)
+    x = rng.standard_exponential((S, C, T)).astype(np.float32)
+    x[0, C // 2, :] += 4.0
+    x[:, :, T // 3] += 9.0
+    if T > 40:
+        x[0, :, 20:36] += 2.5
+    check(lof, lofo, x, S, C, T, max_window=mw, directions=dirs)
+
+
+def test_negative_values_and_constant(lof, lofo):
+    rng = np.random.default_rng(5)
+    x = rng.standard_normal((2, 8, 300)).astype(np.float32) - 3.0
+    x[1] = 2.5                                            # constant stream: stddev 0, no flags (F6)
+    res, ora = check(lof, lofo, x, 2, 8, 300, max_window=32)
+    g = run_gpu(lof, x, 2, 8, 300, max_window=32)
+    assert g["stats"]["stddev"][1] == 0.0 and g["stats"]["n_flagged"][1] == 0
+
+
+def test_nonfinite_stream_fully_flagged(lof, lofo):
+    rng = np.random.default_rng(6)
+    x = rng.standard_exponential((3, 4, 70)).astype(np.float32)
+    x[1, 2, 5] = np.nan
+    x[1, 0, 9] = np.inf
+    for path in (0, 1):
+        g = run_gpu(lof, x, 3, 4, 70, path=path, max_window=8)
+        ora = run_oracle(lofo, x, 3, 4, 70, max_window=8)
+        assert np.array_equal(g["flags"], ora["flags"])
+        assert g["stats"]["n_nonfinite"].tolist() == [0, 2, 0]
+        assert g["stats"]["n_flagged"][1] == 4 * 70 and (g["rowcnt"][1] == 0).all()
+
+
+def test_sensitivity_and_p_params(lof, lofo, wl):
+    w = wl.config1(1)
+    check(lof, lofo, w.power, 1, 16, 256, max_window=32, sensitivity=0.7, p=1.3, start_threshold=5.0)
+
+
+def test_alignment_and_null_errors(lof):
+    import ctypes as C
+    import torch
+    f = lof.Flagger(1, 4, 64)
+    x = torch.zeros(4 * 64 + 4, dtype=torch.float32, device="cuda")
+    fl = f.new_flags()
+    L = lof.lib()
+    s = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    assert L.lof_flag_block(f.h, C.c_void_p(x.data_ptr() + 4), C.c_void_p(fl.data_ptr()), None, s) == lof.E_ALIGN
+    assert L.lof_flag_block(f.h, None, C.c_void_p(fl.data_ptr()), None, s) == lof.E_NULL
+    assert L.lof_history_update(f.h, C.c_void_p(fl.data_ptr()), None, s) == lof.E_STATE   # H = 0
+    f.close()
+
+
+def test_host_entry_point(lof, lofo, wl):
+    import torch
+    w = wl.config1(0)
+    f = lof.Flagger(1, 16, 256, max_window=32)
+    hp = torch.from_numpy(w.power).pin_memory()
+    hf = torch.empty((1, 16, 8), dtype=torch.int32).pin_memory()
+    hs = torch.empty((1, 32), dtype=torch.uint8).pin_memory()
+    f.flag_block_host(hp, hf, hs)
+    ora = run_oracle(lofo, w.power, 1, 16, 256, max_window=32)
+    assert np.array_equal(hf.numpy().view(np.uint32), ora["flags"])
+    assert_stats(hs.numpy().view(lof.STATS_DTYPE).reshape(-1), ora["stats"])
+    assert f.launch_count() > 0
+    f.close()
