@@ -49,7 +49,7 @@ typedef struct {
   uint32_t struct_size;         /* = sizeof(lof_params); anything else -> LOF_E_PARAM            */
   int32_t  device;              /* CUDA device ordinal                                           */
   uint32_t n_streams;           /* S > 0, fixed for the context                                  */
-  uint32_t n_channels;          /* C > 0 (<= 4096)                                               */
+  uint32_t n_channels;          /* C > 0 (<= 256)                                                */
   uint32_t n_time;              /* T > 0                                                         */
   float    p;                   /* > 0; paper default 1.5                          */
   float    sensitivity;         /* > 0; paper default 1.0                          */
@@ -72,7 +72,7 @@ typedef struct {
   uint64_t n_flagged;    /* flagged samples of the stream after the SumThreshold runs              */
 } lof_stream_stats;
 
-/* Validate params (LOF_E_PARAM when: struct_size mismatch; S, C or T zero; C > 4096; max_window
+/* Validate params (LOF_E_PARAM when: struct_size mismatch; S, C or T zero; C > 256; max_window
  * zero, not a power of two or > 1024; directions zero or with unknown bits; p, sensitivity or
  * start_threshold not > 0 and finite), select the device, allocate scratch and history rings
  * (zero-filled, all rings empty).  *out receives the handle; on failure *out = NULL. */
@@ -108,10 +108,11 @@ int lof_history_update(lof_ctx* ctx, uint32_t* d_flags, uint8_t* d_row_flagged, 
 /* Empties every history ring (asynchronous on cuda_stream). */
 int lof_reset(lof_ctx* ctx, void* cuda_stream);
 
-/* Read-only views of context-owned device buffers written by the last lof_flag_block:
- * rowsum [S][C] double = sum of unflagged samples per row, rowcnt [S][C] uint32 = their number
- * (what PAPER.md:102 "meanOfUnflaggedSamples" is formed from).  Valid until lof_destroy. */
-int lof_row_sums(lof_ctx* ctx, const double** d_rowsum, const uint32_t** d_rowcnt);
+/* Copies to caller DEVICE buffers (either may be NULL) what the last lof_flag_block left in the
+ * context for the history flagger: rowsum [S][C] double = sum of unflagged samples per row,
+ * rowcnt [S][C] uint32 = their number (what PAPER.md:102 "meanOfUnflaggedSamples" is formed
+ * from).  Asynchronous on cuda_stream. */
+int lof_row_sums(lof_ctx* ctx, double* d_rowsum, uint32_t* d_rowcnt, void* cuda_stream);
 
 /* Copies the history state to caller DEVICE buffers (any may be NULL): ring [S][C][H] float32,
  * head [S][C] uint32 (next write position), count [S][C] uint32.  Asynchronous. */

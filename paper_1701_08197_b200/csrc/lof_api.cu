@@ -286,10 +286,13 @@ extern "C" int lof_reset(lof_ctx* c, void* cuda_stream) {
   return LOF_OK;
 }
 
-extern "C" int lof_row_sums(lof_ctx* c, const double** d_rowsum, const uint32_t** d_rowcnt) {
+extern "C" int lof_row_sums(lof_ctx* c, double* d_rowsum, uint32_t* d_rowcnt, void* cuda_stream) {
   if (!c) return LOF_E_NULL;
-  if (d_rowsum) *d_rowsum = c->d_rowsum;
-  if (d_rowcnt) *d_rowcnt = c->d_rowcnt;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  const size_t rows = (size_t)c->prm.n_streams * c->prm.n_channels;
+  if (d_rowsum) LOF_CUDA(cudaMemcpyAsync(d_rowsum, c->d_rowsum, rows * 8, cudaMemcpyDeviceToDevice, st));
+  if (d_rowcnt) LOF_CUDA(cudaMemcpyAsync(d_rowcnt, c->d_rowcnt, rows * 4, cudaMemcpyDeviceToDevice, st));
   return LOF_OK;
 }
 

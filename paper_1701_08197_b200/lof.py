@@ -147,19 +147,13 @@ class Flagger:
     def reset(self, stream=None):
         _check(lib().lof_reset(self.h, _stream(stream)))
 
-    def row_sums(self):
-        """Copies of the context's rowsum [S][C] float64 and rowcnt [S][C] (as int32 bit patterns)."""
+    def row_sums(self, stream=None):
+        """rowsum [S][C] float64 and rowcnt [S][C] (uint32 bit patterns in an int32 tensor)."""
         t = self.torch
-        ps, pc = C.c_void_p(), C.c_void_p()
-        _check(lib().lof_row_sums(self.h, C.byref(ps), C.byref(pc)))
-        n = self.S * self.Cn
-        rs = t.empty(n, dtype=t.float64, device=self.dev)
-        rc = t.empty(n, dtype=t.int32, device=self.dev)
-        t.cuda.current_stream().synchronize()
-        cudart = t.cuda.cudart()
-        cudart.cudaMemcpy(rs.data_ptr(), ps.value, n * 8, 3)
-        cudart.cudaMemcpy(rc.data_ptr(), pc.value, n * 4, 3)
-        return rs.view(self.S, self.Cn), rc.view(self.S, self.Cn)
+        rs = t.empty((self.S, self.Cn), dtype=t.float64, device=self.dev)
+        rc = t.empty((self.S, self.Cn), dtype=t.int32, device=self.dev)
+        _check(lib().lof_row_sums(self.h, _ptr(rs), _ptr(rc), _stream(stream)))
+        return rs, rc
 
     def history_export(self, stream=None):
         t = self.torch
