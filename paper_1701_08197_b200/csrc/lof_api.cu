@@ -228,14 +228,54 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
   return LOF_OK;
 }
 
+// ---- fused path: streams that fit one SM's shared memory (lof_fused.cuh)
+template <int C, int L>
+static cudaError_t fused_launch(lof_ctx* c, const float* d_power, uint32_t* d_flags, cudaStream_t st) {
+  using Cfg = LofFusedCfg<C, L>;
+  static bool attr_done[64] = {};
+  cudaError_t e = cudaSuccess;
+  if (!attr_done[c->prm.device & 63]) {
+    e = cudaFuncSetAttribute(lof_k_fused<C, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes);
+    if (e != cudaSuccess) return e;
+    attr_done[c->prm.device & 63] = true;
+  }
+  int per_sm = 1;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lof_k_fused<C, L>, Cfg::NT, Cfg::smem_bytes);
+  if (e != cudaSuccess) return e;
+  if (per_sm < 1) per_sm = 1;
+  uint32_t grid = (uint32_t)(c->sm_count * per_sm);
+  if (grid > c->prm.n_streams) grid = c->prm.n_streams;
+  lof_k_fused<C, L><<<grid, Cfg::NT, Cfg::smem_bytes, st>>>(d_power, d_flags, c->d_stats, c->d_rowsum, c->d_rowcnt, c->kp);
+  c->launches += 1;
+  return cudaGetLastError();
+}
+
+// returns 1 if the shape has a fused instantiation and it was launched, 0 if not, <0 on error
+static int flag_block_fused(lof_ctx* c, const float* d_power, uint32_t* d_flags, cudaStream_t st) {
+  const uint32_t C = c->prm.n_channels, T = c->prm.n_time;
+  cudaError_t e;
+  if (C == 64 && T == 768) e = fused_launch<64, 24>(c, d_power, d_flags, st);
+  else if (C == 16 && T == 768) e = fused_launch<16, 24>(c, d_power, d_flags, st);
+  else if (C == 32 && T == 768) e = fused_launch<32, 24>(c, d_power, d_flags, st);
+  else if (C == 16 && T == 256) e = fused_launch<16, 8>(c, d_power, d_flags, st);
+  else return 0;
+  if (e != cudaSuccess) {
+    snprintf(g_cuda_err, sizeof g_cuda_err, "fused launch: %s", cudaGetErrorString(e));
+    return LOF_E_CUDA;
+  }
+  return 1;
+}
+static int flag_block_fused(lof_ctx*, const int16_t*, uint32_t*, cudaStream_t) { return 0; }
+
 template <class In>
 static int flag_block_any(lof_ctx* c, In in, uint32_t* d_flags, lof_stream_stats* d_stats, void* cuda_stream) {
   if (!c || !in.p || !d_flags) return LOF_E_NULL;
   if (((uintptr_t)in.p & 15) || ((uintptr_t)d_flags & 15) || ((uintptr_t)d_stats & 7)) return LOF_E_ALIGN;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   LOF_CUDA(cudaSetDevice(c->prm.device));
-  int rc = flag_block_generic(c, in, d_flags, st);
-  if (rc) return rc;
+  int rc = c->path == 0 ? flag_block_fused(c, in.p, d_flags, st) : 0;
+  if (rc < 0) return rc;
+  if (rc == 0) { rc = flag_block_generic(c, in, d_flags, st); if (rc) return rc; }
   if (d_stats)
     LOF_CUDA(cudaMemcpyAsync(d_stats, c->d_stats, (size_t)c->prm.n_streams * sizeof(lof_stream_stats),
                              cudaMemcpyDeviceToDevice, st));

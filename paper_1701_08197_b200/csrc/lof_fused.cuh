@@ -1,3 +1,545 @@
-// lof_fused.cuh — shape-specialised fused kernels (filled in below the generic path).
+// lof_fused.cuh — the fused LOF kernel for streams that fit one SM's shared memory
+// (BASELINE.json configs 1-3: 16x256, 64x768, 16x768 float32 = 16 / 192 / 48 KB per stream).
+//
+// One CTA owns one stream at a time (persistent over streams) and does the whole hot path with a
+// single HBM read of the stream and a single write of its flag words:
+//   load stream -> shared memory                                    (4 B/sample from HBM)
+//   S: statistics: shifted fp32 group sums folded into fp64;
+//      exact median by a 1024-bin value histogram around the estimated centre, then an exact
+//      rank count among the few samples of the median's bin (radix select as the fallback)
+//   F: SumThreshold along frequency: a thread per time column, the
+//      column's C window sums in registers, doubled in place level by level
+//   T: SumThreshold along time, starting from F's mask: a warp per channel row, each lane holding
+//      L = T/32 consecutive samples in registers, neighbours' partial sums by warp shuffle
+//   bit-pack + row sums of unflagged samples          (1/8 B/sample to HBM)
+// The window test is the paper's "sum with flagged samples replaced by threshold_I > I*threshold_I"
+// written as  u > e * threshold_I  with u = sum of the unflagged samples of the window and
+// e = their number, both obtained by doubling: X_2I[t] = X_I[t] + X_I[t+I].
+// Flags are frozen during an iteration (F8): u and e are rebuilt from level 0 whenever
+// an iteration set a new flag.
 #pragma once
 #include "lof_common.cuh"
+
+#define LOF_F_NBINS 1024
+#define LOF_F_CAP 1024
+#define LOF_F_MAGIC 12582912.0f   // 1.5 * 2^23: adding it leaves round-to-nearest(x) in the low mantissa bits
+
+template <int C, int L>
+struct LofFusedCfg {
+  static constexpr int T = 32 * L, N = C * T, W = L;
+  static constexpr int NT = 256;                         // threads per CTA
+  static constexpr int MINB = (C >= 64) ? 1 : 2;
+  static constexpr size_t smem_bytes =
+      (size_t)N * 4 + (size_t)C * W * 4 + 2048 * 4 + LOF_F_CAP * 4 + 64 * 8 + 64 * 4;
+};
+
+struct LofFusedSmem {
+  float* xs; uint32_t* fm; uint32_t* hist; float* cand; double* red; float* thr; uint32_t* ctl;
+  template <int C, int L>
+  __device__ static LofFusedSmem make(unsigned char* base) {
+    LofFusedSmem s;
+    constexpr int N = C * 32 * L;
+    s.xs = reinterpret_cast<float*>(base);
+    s.fm = reinterpret_cast<uint32_t*>(s.xs + N);
+    s.hist = s.fm + C * L;
+    s.cand = reinterpret_cast<float*>(s.hist + 2048);
+    s.red = reinterpret_cast<double*>(s.cand + LOF_F_CAP);
+    s.thr = reinterpret_cast<float*>(s.red + 64);
+    s.ctl = reinterpret_cast<uint32_t*>(s.thr + 16);
+    return s;
+  }
+};
+// ctl slots
+enum { CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS, CT_NFLAG, CT_BAD, CT_SELP, CT_SELACC, CT_PREFIX, CT_RANK, CT_FOUND };
+
+// Find the bin holding `rank` in hist[NB] (NB a multiple of 256, blockDim >= 256).
+// Results in ctl[CT_BIN] (bin) and ctl[CT_BEFORE] (number of entries in lower bins).
+template <int NB>
+__device__ void lof_find_bin(const uint32_t* hist, uint32_t rank, uint32_t* part /*256*/, uint32_t* ctl) {
+  constexpr int PER = NB / 256;
+  const int tid = threadIdx.x, lane = tid & 31;
+  uint32_t loc[PER], tot = 0;
+  if (tid < 256) {
+#pragma unroll
+    for (int j = 0; j < PER; ++j) { loc[j] = hist[tid * PER + j]; tot += loc[j]; }
+    part[tid] = tot;
+  }
+  __syncthreads();
+  if (tid < 32) {
+    uint32_t p[8], s = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { p[j] = part[lane * 8 + j]; s += p[j]; }
+    uint32_t inc = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+    const uint32_t exc = inc - s;
+    const bool mine = (rank >= exc && rank < inc) || (lane == 31 && rank >= inc);
+    if (mine) {
+      uint32_t acc = exc; int j = 0;
+      for (; j < 7; ++j) { if (acc + p[j] > rank) break; acc += p[j]; }
+      ctl[CT_SELP] = lane * 8 + j; ctl[CT_SELACC] = acc;
+    }
+  }
+  __syncthreads();
+  if (tid == (int)ctl[CT_SELP]) {
+    uint32_t acc = ctl[CT_SELACC]; int j = 0;
+    for (; j < PER - 1; ++j) { if (acc + loc[j] > rank) break; acc += loc[j]; }
+    ctl[CT_BIN] = tid * PER + j; ctl[CT_BEFORE] = acc;
+  }
+  __syncthreads();
+}
+
+// Exact rank-`rank` element of xs[0..N) by a 3-pass radix select (11+11+10 bits of the key) with a
+// shared-memory histogram: the fallback when the value histogram cannot isolate the median.
+template <int NT>
+__device__ float lof_radix_select_smem(const float* xs, int N, uint32_t rank, uint32_t* hist, uint32_t* part,
+                                       uint32_t* ctl) {
+  uint32_t prefix = 0;
+  for (int pass = 0; pass < 3; ++pass) {
+    for (int b = threadIdx.x; b < 2048; b += NT) hist[b] = 0;
+    __syncthreads();
+    for (int i = threadIdx.x; i < N; i += NT) {
+      const uint32_t key = lof_key(xs[i]);
+      if (pass == 0) atomicAdd(&hist[key >> 21], 1u);
+      else if (pass == 1) { if ((key >> 21) == prefix) atomicAdd(&hist[(key >> 10) & 2047u], 1u); }
+      else { if ((key >> 10) == prefix) atomicAdd(&hist[key & 1023u], 1u); }
+    }
+    __syncthreads();
+    lof_find_bin<2048>(hist, rank, part, ctl);
+    const uint32_t bin = ctl[CT_BIN];
+    rank -= ctl[CT_BEFORE];
+    prefix = pass == 0 ? bin : (pass == 1 ? ((prefix << 11) | bin) : ((prefix << 10) | bin));
+    __syncthreads();
+  }
+  return lof_unkey(prefix);
+}
+
+// Block reduction of two doubles at once (fixed order); result valid in every thread.
+template <int NT>
+__device__ __forceinline__ void lof_block_sum2(double& a, double& b, double* red /*64*/) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  constexpr int NW = NT / 32;
+  a = lof_warp_sum(a); b = lof_warp_sum(b);
+  __syncthreads();
+  if (lane == 0) { red[w] = a; red[32 + w] = b; }
+  __syncthreads();
+  double ra = 0.0, rb = 0.0;
+#pragma unroll
+  for (int i = 0; i < NW; ++i) { ra += red[i]; rb += red[32 + i]; }
+  a = ra; b = rb;
+  __syncthreads();
+}
+
+// Statistics of the stream in xs[0..N): mean, stddev (population), exact median of
+// rank floor(N/2), thresholds.  Writes sm.thr[], the stats record, and returns the number of
+// non-finite samples (then everything else is unspecified, S6).
+template <int C, int L>
+__device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParams& prm, lof_stream_stats* out) {
+  using Cfg = LofFusedCfg<C, L>;
+  constexpr int N = Cfg::N, NT = Cfg::NT;
+  const int tid = threadIdx.x;
+  uint32_t* part = reinterpret_cast<uint32_t*>(sm.cand);
+  // --- S1: centre K and spread from a strided sample (one sample per thread): makes the shifted sums
+  // well conditioned and places the value histogram.  Any K gives the same exact results.
+  double sa, sq;
+  {
+    const int idx = (int)(((long long)tid * N) / NT) + (tid * 7) % (N / NT > 0 ? N / NT : 1);
+    const float v = sm.xs[idx < N ? idx : N - 1];
+    sa = (double)v; sq = (double)v * (double)v;
+    lof_block_sum2<NT>(sa, sq, sm.red);
+  }
+  float K = (float)(sa / NT);
+  float sd = sqrtf(fmaxf((float)(sq / NT) - K * K, 0.f));
+  if (!lof_finite(K) || !lof_finite(sd)) { K = 0.f; sd = 1.f; }
+  float h = 1.25f * sd;
+  if (!(h > 0.f)) h = fmaxf(fabsf(K) * 1e-6f, 1e-30f);
+  const float scale = 1022.0f / (2.0f * h);
+  const float off = fmaf(-(K - h), scale, 1.0f);        // x = K-h -> 1, x = K+h -> 1023
+  for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
+  if (tid == 0) { sm.ctl[CT_NCAND] = 0; sm.ctl[CT_BAD] = 0; sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_FOUND] = 0; }
+  __syncthreads();
+  // --- S2: one pass: sums of d = x-K and d^2 in fp32 over groups of 8, folded into fp64; histogram of
+  // round(clamp((x-lo)*scale)) (a monotone map of x, so bins are value-ordered).
+  double da = 0.0, dq = 0.0;
+  const float4* x4 = reinterpret_cast<const float4*>(sm.xs);
+  for (int i = tid; i < N / 4; i += 2 * NT) {
+    float ga = 0.f, gq = 0.f;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      const int ii = i + r * NT;
+      if (ii < N / 4) {
+        const float4 v = x4[ii];
+        const float xv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const float d = xv[q] - K;
+          ga += d; gq = fmaf(d, d, gq);
+          float yb = fmaf(xv[q], scale, off);
+          yb = fminf(fmaxf(yb, 0.f), 1023.4f);
+          const uint32_t bin = __float_as_uint(yb + LOF_F_MAGIC) & 1023u;
+          atomicAdd(&sm.hist[bin], 1u);
+        }
+      }
+    }
+    da += (double)ga; dq += (double)gq;
+  }
+  lof_block_sum2<NT>(da, dq, sm.red);
+  uint32_t n_bad = 0;
+  if (!isfinite(da) || !isfinite(dq)) {
+    // rare: a non-finite sample, or d^2 overflowed fp32: count exactly and redo the sums in fp64
+    uint32_t bad = 0; double a2 = 0.0, q2 = 0.0;
+    for (int i = tid; i < N; i += NT) {
+      const float x = sm.xs[i];
+      bad += lof_finite(x) ? 0u : 1u;
+      const double d = (double)x - (double)K; a2 += d; q2 = fma(d, d, q2);
+    }
+    if (bad) atomicAdd(&sm.ctl[CT_BAD], bad);
+    lof_block_sum2<NT>(a2, q2, sm.red);
+    da = a2; dq = q2;
+    n_bad = sm.ctl[CT_BAD];
+  }
+  const double n = (double)N;
+  double var = (dq - da * da / n) / n;
+  if (!(var > 0.0)) var = 0.0;
+  const double mean = (double)K + da / n, stddev = sqrt(var);
+  // --- S3..S5: median
+  const uint32_t rank = N / 2;                          // DESIGN.md S3: rank floor(N/2), 0-based
+  float median = 0.f;
+  if (n_bad == 0) {
+    lof_find_bin<LOF_F_NBINS>(sm.hist, rank, part, sm.ctl);
+    const uint32_t bin = sm.ctl[CT_BIN], before = sm.ctl[CT_BEFORE];
+    const uint32_t n_b = sm.hist[bin];
+    __syncthreads();
+    bool ok = bin > 0 && bin < 1023 && n_b <= LOF_F_CAP;
+    if (ok) {
+      // S4: gather the samples of the median's bin
+      for (int i = tid; i < N / 4; i += NT) {
+        const float4 v = x4[i];
+        const float xv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          float yb = fmaf(xv[q], scale, off);
+          yb = fminf(fmaxf(yb, 0.f), 1023.4f);
+          if ((__float_as_uint(yb + LOF_F_MAGIC) & 1023u) == bin) {
+            const uint32_t slot = atomicAdd(&sm.ctl[CT_NCAND], 1u);
+            if (slot < LOF_F_CAP) sm.cand[slot] = xv[q];
+          }
+        }
+      }
+      __syncthreads();
+      // S5: the candidate with exactly (rank - before) candidates ordered before it
+      const uint32_t want = rank - before, nc = sm.ctl[CT_NCAND];
+      for (uint32_t i = tid; i < nc; i += NT) {
+        const float v = sm.cand[i];
+        uint32_t less = 0;
+        for (uint32_t j = 0; j < nc; ++j) {
+          const float w = sm.cand[j];
+          less += (w < v || (w == v && j < i)) ? 1u : 0u;
+        }
+        if (less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
+      }
+      __syncthreads();
+      ok = sm.ctl[CT_FOUND] != 0;
+      median = __uint_as_float(sm.ctl[CT_MEDBITS]);
+    }
+    if (!ok) median = lof_radix_select_smem<NT>(sm.xs, N, rank, sm.hist, part, sm.ctl);
+  }
+  if (tid == 0) {
+    for (uint32_t k = 0; k < prm.n_levels; ++k)
+      sm.thr[k] = (float)((double)median + stddev * prm.factor[k] * prm.sensitivity);
+    lof_stream_stats o;
+    o.median = median; o.n_nonfinite = n_bad; o.mean = mean; o.stddev = stddev;
+    o.n_flagged = n_bad ? (uint64_t)N : 0;
+    *out = o;
+  }
+  __syncthreads();
+  return n_bad;
+}
+
+// ---- F: SumThreshold along frequency.  One thread per time column; u[c], e[c] in registers.
+template <int C>
+__device__ __forceinline__ void lof_col_rebuild(const float* col, int T, uint64_t fb, float (&u)[C], float (&e)[C],
+                                                int k_upto) {
+#pragma unroll
+  for (int c = 0; c < C; ++c) {
+    const bool f = (fb >> c) & 1ull;
+    u[c] = f ? 0.f : col[c * T];
+    e[c] = f ? 0.f : 1.f;
+  }
+#pragma unroll
+  for (int j = 1; (1 << j) <= C; ++j) {
+    if (j <= k_upto) {
+      const int d = 1 << (j - 1);
+#pragma unroll
+      for (int c = 0; c + (1 << j) <= C; ++c) { u[c] += u[c + d]; e[c] += e[c + d]; }
+    }
+  }
+}
+
+template <int C, int L>
+__device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
+  using Cfg = LofFusedCfg<C, L>;
+  constexpr int T = Cfg::T, NT = Cfg::NT, W = Cfg::W;
+  const int lane = threadIdx.x & 31;
+  constexpr int ROUNDS = (T + NT - 1) / NT;
+  for (int r = 0; r < ROUNDS; ++r) {
+    const int col = r * NT + threadIdx.x;               // T and NT are multiples of 32: warps stay whole
+    if (col >= T) break;
+    const float* cp = sm.xs + col;
+    float u[C], e[C];
+    uint64_t fb = 0;
+    {
+      float m0 = -INFINITY, m1 = -INFINITY;
+#pragma unroll
+      for (int c = 0; c < C; c += 2) {
+        u[c] = cp[c * T]; u[c + 1] = cp[(c + 1) * T];
+        m0 = fmaxf(m0, u[c]); m1 = fmaxf(m1, u[c + 1]);
+        e[c] = 1.f; e[c + 1] = 1.f;
+      }
+      const float T0 = sm.thr[0];
+      if (fmaxf(m0, m1) > T0) {                          // level 0: I = 1, the simple thresholder
+#pragma unroll
+        for (int c = 0; c < C; ++c)
+          if (u[c] > T0) { fb |= 1ull << c; u[c] = 0.f; e[c] = 0.f; }
+      }
+    }
+#pragma unroll
+    for (int k = 1; (1 << k) <= C; ++k) {
+      if (k < (int)n_lev_f) {
+        const int d = 1 << (k - 1), I = 1 << k;
+        const float negT = -sm.thr[k];
+        float t0 = -INFINITY, t1 = -INFINITY;
+#pragma unroll
+        for (int c = 0; c + I <= C; ++c) {
+          u[c] += u[c + d]; e[c] += e[c + d];
+          const float v = fmaf(e[c], negT, u[c]);       // u - e*T > 0  <=>  window flagged
+          if (c & 1) t1 = fmaxf(t1, v); else t0 = fmaxf(t0, v);
+        }
+        if (fmaxf(t0, t1) > 0.f) {
+          uint64_t trig = 0;
+#pragma unroll
+          for (int c = 0; c + I <= C; ++c)
+            if (fmaf(e[c], negT, u[c]) > 0.f) trig |= 1ull << c;
+          uint64_t dil = trig;
+#pragma unroll
+          for (int s = 1; s < I; s <<= 1) dil |= dil << s;
+          const uint64_t nf = fb | dil;
+          if (nf != fb) {
+            fb = nf;
+            if ((1 << (k + 1)) <= C && k + 1 < (int)n_lev_f) lof_col_rebuild<C>(cp, T, fb, u, e, k);
+          }
+        }
+      }
+    }
+    // this warp's 32 columns -> one mask word per channel
+    const int w = col >> 5;
+    uint32_t mine0 = 0, mine1 = 0;
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+      const uint32_t word = __ballot_sync(0xffffffffu, (fb >> c) & 1ull);
+      if ((c & 31) == lane) { if (c < 32) mine0 = word; else mine1 = word; }
+    }
+    if (lane < C) sm.fm[lane * W + w] = mine0;
+    if (C > 32 && lane + 32 < C) sm.fm[(lane + 32) * W + w] = mine1;
+  }
+}
+
+// ---- T: SumThreshold along time.  One warp per channel row; lane l holds samples [l*L, l*L+L).
+// One doubling step of distance D (window 2D): partners beyond the lane's own L samples come from the
+// following lanes by shuffle; a partner outside the row is -inf, so such windows never fire.
+template <int L, int D>
+__device__ __forceinline__ void lof_row_step(float (&u)[L], float (&e)[L], int lane) {
+  constexpr int NP = D < L ? D : L;
+  float pu[NP], pe[NP];
+#pragma unroll
+  for (int jj = 0; jj < NP; ++jj) {
+    const int j = L - NP + jj, src = (j + D) % L, off = (j + D) / L;
+    pu[jj] = __shfl_down_sync(0xffffffffu, u[src], off);
+    pe[jj] = __shfl_down_sync(0xffffffffu, e[src], off);
+    if (lane + off > 31) pu[jj] = -INFINITY;
+  }
+#pragma unroll
+  for (int j = 0; j < L; ++j) {
+    if (j + D < L) { u[j] += u[j + D]; e[j] += e[j + D]; }
+    else { u[j] += pu[j - (L - NP)]; e[j] += pe[j - (L - NP)]; }
+  }
+}
+
+template <int L>
+__device__ __forceinline__ void lof_row_rebuild(const float (&x)[L], uint32_t fb, float (&u)[L], float (&e)[L],
+                                                int lane, int k_upto) {
+#pragma unroll
+  for (int j = 0; j < L; ++j) {
+    const bool f = (fb >> j) & 1u;
+    u[j] = f ? 0.f : x[j];
+    e[j] = f ? 0.f : 1.f;
+  }
+  if (k_upto >= 1) lof_row_step<L, 1>(u, e, lane);
+  if (k_upto >= 2) lof_row_step<L, 2>(u, e, lane);
+  if (k_upto >= 3) lof_row_step<L, 4>(u, e, lane);
+  if (k_upto >= 4) lof_row_step<L, 8>(u, e, lane);
+  if (k_upto >= 5) lof_row_step<L, 16>(u, e, lane);
+  if (k_upto >= 6) lof_row_step<L, 32>(u, e, lane);
+  if (k_upto >= 7) lof_row_step<L, 64>(u, e, lane);
+  if (k_upto >= 8) lof_row_step<L, 128>(u, e, lane);
+  if (k_upto >= 9) lof_row_step<L, 256>(u, e, lane);
+}
+
+// One iteration I = 2^K (K >= 1) on a row: doubling step, test, and - if any window fired - flag
+// dilation across the warp and a rebuild of u, e under the new flags.  Returns nothing; fb updated.
+template <int L, int K>
+__device__ __forceinline__ void lof_row_level(const float (&x)[L], uint32_t& fb, float (&u)[L], float (&e)[L],
+                                              int lane, float thr, bool more_levels) {
+  constexpr int I = 1 << K;
+  lof_row_step<L, (I >> 1)>(u, e, lane);
+  const float negT = -thr;
+  float t0 = -INFINITY, t1 = -INFINITY;
+#pragma unroll
+  for (int j = 0; j < L; ++j) {
+    const float v = fmaf(e[j], negT, u[j]);
+    if (j & 1) t1 = fmaxf(t1, v); else t0 = fmaxf(t0, v);
+  }
+  if (__any_sync(0xffffffffu, fmaxf(t0, t1) > 0.f)) {
+    uint32_t trig = 0;
+#pragma unroll
+    for (int j = 0; j < L; ++j) trig |= (fmaf(e[j], negT, u[j]) > 0.f) ? (1u << j) : 0u;
+    // own windows, inside the lane's L bits
+    uint32_t own = trig;
+#pragma unroll
+    for (int s = 1; s < I && s < 32; s <<= 1) own |= own << s;
+    // windows started in earlier lanes: sample p is covered iff p < (last start before this lane) + I
+    int hi = trig ? (lane * L + 31 - __clz(trig)) : -(1 << 20);
+    int pm = hi;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pm, o); if (lane >= o) pm = max(pm, v); }
+    int prev = __shfl_up_sync(0xffffffffu, pm, 1);
+    if (lane == 0) prev = -(1 << 20);
+    int cnt = prev + I - lane * L;
+    cnt = cnt < 0 ? 0 : (cnt > L ? L : cnt);
+    const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
+    const uint32_t pre = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
+    const uint32_t nf = (fb | own | pre) & maskL;
+    const bool changed = nf != fb;
+    fb = nf;
+    if (more_levels && __any_sync(0xffffffffu, changed)) lof_row_rebuild<L>(x, fb, u, e, lane, K);
+  }
+}
+
+template <int C, int L>
+__device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, uint32_t s, bool have_f,
+                               uint32_t* __restrict__ flags, double* __restrict__ rowsum,
+                               uint32_t* __restrict__ rowcnt) {
+  using Cfg = LofFusedCfg<C, L>;
+  constexpr int T = Cfg::T, NT = Cfg::NT, W = Cfg::W, NW = NT / 32;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t nlt = prm.n_lev_t;
+  const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
+  uint32_t n_flag_acc = 0;
+  for (int c = warp; c < C; c += NW) {
+    float x[L], u[L], e[L];
+    const float4* rp = reinterpret_cast<const float4*>(sm.xs + c * T + lane * L);
+#pragma unroll
+    for (int q = 0; q < L / 4; ++q) {
+      const float4 v = rp[q];
+      x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
+    }
+    uint32_t fb = 0;
+    if (have_f) {                                       // start from the frequency run's mask (F10)
+      const int b0 = lane * L, q = b0 >> 5, r = b0 & 31;
+      const uint32_t lo = sm.fm[c * W + q], hi = (q + 1 < W) ? sm.fm[c * W + q + 1] : 0u;
+      fb = __funnelshift_r(lo, hi, r) & maskL;
+    }
+    if (nlt > 0) {
+      // level 0 (I = 1): x > threshold_1 on samples not yet flagged
+      const float T0 = sm.thr[0];
+#pragma unroll
+      for (int j = 0; j < L; ++j) {
+        const bool f = ((fb >> j) & 1u) || (x[j] > T0);
+        fb |= f ? (1u << j) : 0u;
+        u[j] = f ? 0.f : x[j];
+        e[j] = f ? 0.f : 1.f;
+      }
+      const bool all_flagged = __all_sync(0xffffffffu, fb == maskL);
+      if (!all_flagged) {
+        if (nlt > 1) lof_row_level<L, 1>(x, fb, u, e, lane, sm.thr[1], nlt > 2);
+        if (nlt > 2) lof_row_level<L, 2>(x, fb, u, e, lane, sm.thr[2], nlt > 3);
+        if (nlt > 3) lof_row_level<L, 3>(x, fb, u, e, lane, sm.thr[3], nlt > 4);
+        if (nlt > 4) lof_row_level<L, 4>(x, fb, u, e, lane, sm.thr[4], nlt > 5);
+        if (nlt > 5) lof_row_level<L, 5>(x, fb, u, e, lane, sm.thr[5], nlt > 6);
+        if (nlt > 6) lof_row_level<L, 6>(x, fb, u, e, lane, sm.thr[6], nlt > 7);
+        if (nlt > 7) lof_row_level<L, 7>(x, fb, u, e, lane, sm.thr[7], nlt > 8);
+        if (nlt > 8) lof_row_level<L, 8>(x, fb, u, e, lane, sm.thr[8], nlt > 9);
+        if (nlt > 9) lof_row_level<L, 9>(x, fb, u, e, lane, sm.thr[9], false);
+      }
+    }
+    // bit-pack: word w of the row = bits [32w, 32w+32) gathered from the lanes' L-bit masks
+    {
+      const int q0 = (32 * lane) / L, r0 = 32 * lane - L * q0;
+      uint32_t word = 0;
+      constexpr int NI = (31 + L) / L + 1;
+#pragma unroll
+      for (int i = 0; i < NI; ++i) {
+        const int src = q0 + i;
+        uint32_t v = __shfl_sync(0xffffffffu, fb, src & 31);
+        if (src > 31) v = 0;
+        const int sh = i * L - r0;
+        if (sh < 32) word |= sh >= 0 ? (v << sh) : (v >> (-sh));
+      }
+      if (lane < W) flags[((size_t)s * C + c) * W + lane] = word;
+    }
+    // row sum of unflagged samples, fp32 within the lane, fp64 across lanes
+    float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
+#pragma unroll
+    for (int j = 0; j < L; j += 4) {
+      p0 += ((fb >> j) & 1u) ? 0.f : x[j];
+      p1 += ((fb >> (j + 1)) & 1u) ? 0.f : x[j + 1];
+      p2 += ((fb >> (j + 2)) & 1u) ? 0.f : x[j + 2];
+      p3 += ((fb >> (j + 3)) & 1u) ? 0.f : x[j + 3];
+    }
+    double rs = (double)((p0 + p1) + (p2 + p3));
+    rs = lof_warp_sum(rs);
+    uint32_t nf = __popc(fb);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) nf += __shfl_down_sync(0xffffffffu, nf, o);
+    if (lane == 0) {
+      rowsum[(size_t)s * C + c] = rs;
+      rowcnt[(size_t)s * C + c] = T - nf;
+      n_flag_acc += nf;
+    }
+  }
+  if (lane == 0 && n_flag_acc) atomicAdd(&sm.ctl[CT_NFLAG], n_flag_acc);
+}
+
+// The kernel: persistent CTAs, one stream at a time.
+template <int C, int L>
+__global__ void __launch_bounds__(LofFusedCfg<C, L>::NT, LofFusedCfg<C, L>::MINB)
+lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_stream_stats* __restrict__ stats,
+            double* __restrict__ rowsum, uint32_t* __restrict__ rowcnt, LofKParams prm) {
+  using Cfg = LofFusedCfg<C, L>;
+  constexpr int N = Cfg::N, NT = Cfg::NT, W = Cfg::W;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const LofFusedSmem sm = LofFusedSmem::make<C, L>(smem_raw);
+  for (uint32_t s = blockIdx.x; s < prm.S; s += gridDim.x) {
+    // load the stream (one read of HBM)
+    const float4* g4 = reinterpret_cast<const float4*>(power + (size_t)s * N);
+    float4* s4 = reinterpret_cast<float4*>(sm.xs);
+#pragma unroll 4
+    for (int i = threadIdx.x; i < N / 4; i += NT) s4[i] = __ldg(g4 + i);
+    __syncthreads();
+    const uint32_t n_bad = lof_fused_statistics<C, L>(sm, prm, stats + s);
+    if (n_bad) {
+      // DESIGN.md S6: the whole stream is flagged
+      for (int i = threadIdx.x; i < C * W; i += NT) flags[(size_t)s * C * W + i] = 0xFFFFFFFFu;
+      for (int i = threadIdx.x; i < C; i += NT) { rowsum[(size_t)s * C + i] = 0.0; rowcnt[(size_t)s * C + i] = 0; }
+      __syncthreads();
+      continue;
+    }
+    const bool have_f = prm.n_lev_f > 0;
+    if (have_f) lof_fused_freq<C, L>(sm, prm.n_lev_f);
+    __syncthreads();
+    lof_fused_time<C, L>(sm, prm, s, have_f, flags, rowsum, rowcnt);
+    __syncthreads();
+    if (threadIdx.x == 0) stats[s].n_flagged = sm.ctl[CT_NFLAG];
+    __syncthreads();
+  }
+}

@@ -56,7 +56,9 @@ def check(lof, lofo, power, S, C, T, exact=False, volt=None, paths=(0, 1), **kw)
         if res["n_mismatch"] == 0:
             assert np.array_equal(g["stats"]["n_flagged"], ora["stats"]["n_flagged"])
             assert np.array_equal(g["rowcnt"], ora["rowcnt"])
-            np.testing.assert_allclose(g["rowsum"], ora["rowsum"], rtol=1e-12, atol=0)
+            # row sums feed float32 history entries: the fused kernel adds each lane's samples
+            # in fp32 before the fp64 reduction, so 1e-6 relative is the bar
+            np.testing.assert_allclose(g["rowsum"], ora["rowsum"], rtol=1e-6, atol=0)
         # padding bits are zero
         if T % 32:
             assert (g["flags"][..., -1] >> np.uint32(T % 32)).max() == 0
