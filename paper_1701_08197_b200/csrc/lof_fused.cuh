@@ -20,7 +20,7 @@
 #pragma once
 #include "lof_common.cuh"
 
-#define LOF_F_NBINS 1024
+#define LOF_F_NBINS 2048
 #define LOF_F_CAP 1024
 #define LOF_F_MAGIC 12582912.0f   // 1.5 * 2^23: adding it leaves round-to-nearest(x) in the low mantissa bits
 
@@ -30,11 +30,11 @@ struct LofFusedCfg {
   static constexpr int NT = 256;                         // threads per CTA
   static constexpr int MINB = (C >= 64) ? 1 : 2;
   static constexpr size_t smem_bytes =
-      (size_t)N * 4 + (size_t)C * W * 4 + 2048 * 4 + LOF_F_CAP * 4 + 64 * 8 + 64 * 4;
+      (size_t)N * 4 + (size_t)C * W * 4 + 2048 * 4 + LOF_F_CAP * 4 + 64 * 8 + 64 * 4 + 256 * 4;
 };
 
 struct LofFusedSmem {
-  float* xs; uint32_t* fm; uint32_t* hist; float* cand; double* red; float* thr; uint32_t* ctl;
+  float* xs; uint32_t* fm; uint32_t* hist; float* cand; double* red; float* thr; uint32_t* ctl; uint32_t* part;
   template <int C, int L>
   __device__ static LofFusedSmem make(unsigned char* base) {
     LofFusedSmem s;
@@ -46,6 +46,7 @@ struct LofFusedSmem {
     s.red = reinterpret_cast<double*>(s.cand + LOF_F_CAP);
     s.thr = reinterpret_cast<float*>(s.red + 64);
     s.ctl = reinterpret_cast<uint32_t*>(s.thr + 16);
+    s.part = s.ctl + 48;
     return s;
   }
 };
@@ -138,7 +139,7 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
   using Cfg = LofFusedCfg<C, L>;
   constexpr int N = Cfg::N, NT = Cfg::NT;
   const int tid = threadIdx.x;
-  uint32_t* part = reinterpret_cast<uint32_t*>(sm.cand);
+  uint32_t* part = sm.part;
   // --- S1: centre K and spread from a strided sample (one sample per thread): makes the shifted sums
   // well conditioned and places the value histogram.  Any K gives the same exact results.
   double sa, sq;
@@ -153,8 +154,8 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
   if (!lof_finite(K) || !lof_finite(sd)) { K = 0.f; sd = 1.f; }
   float h = 1.25f * sd;
   if (!(h > 0.f)) h = fmaxf(fabsf(K) * 1e-6f, 1e-30f);
-  const float scale = 1022.0f / (2.0f * h);
-  const float off = fmaf(-(K - h), scale, 1.0f);        // x = K-h -> 1, x = K+h -> 1023
+  const float scale = 2046.0f / (2.0f * h);
+  const float off = fmaf(-(K - h), scale, 1.0f);        // x = K-h -> 1, x = K+h -> 2047
   for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
   if (tid == 0) { sm.ctl[CT_NCAND] = 0; sm.ctl[CT_BAD] = 0; sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_FOUND] = 0; }
   __syncthreads();
@@ -175,8 +176,8 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
           const float d = xv[q] - K;
           ga += d; gq = fmaf(d, d, gq);
           float yb = fmaf(xv[q], scale, off);
-          yb = fminf(fmaxf(yb, 0.f), 1023.4f);
-          const uint32_t bin = __float_as_uint(yb + LOF_F_MAGIC) & 1023u;
+          yb = fminf(fmaxf(yb, 0.f), 2047.4f);
+          const uint32_t bin = __float_as_uint(yb + LOF_F_MAGIC) & 2047u;
           atomicAdd(&sm.hist[bin], 1u);
         }
       }
@@ -210,7 +211,7 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
     const uint32_t bin = sm.ctl[CT_BIN], before = sm.ctl[CT_BEFORE];
     const uint32_t n_b = sm.hist[bin];
     __syncthreads();
-    bool ok = bin > 0 && bin < 1023 && n_b <= LOF_F_CAP;
+    bool ok = bin > 0 && bin < 2047 && n_b <= LOF_F_CAP;
     if (ok) {
       // S4: gather the samples of the median's bin
       for (int i = tid; i < N / 4; i += NT) {
@@ -219,8 +220,8 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           float yb = fmaf(xv[q], scale, off);
-          yb = fminf(fmaxf(yb, 0.f), 1023.4f);
-          if ((__float_as_uint(yb + LOF_F_MAGIC) & 1023u) == bin) {
+          yb = fminf(fmaxf(yb, 0.f), 2047.4f);
+          if ((__float_as_uint(yb + LOF_F_MAGIC) & 2047u) == bin) {
             const uint32_t slot = atomicAdd(&sm.ctl[CT_NCAND], 1u);
             if (slot < LOF_F_CAP) sm.cand[slot] = xv[q];
           }
@@ -229,16 +230,22 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
       __syncthreads();
       // S5: the candidate with exactly (rank - before) candidates ordered before it
       const uint32_t want = rank - before, nc = sm.ctl[CT_NCAND];
-      for (uint32_t i = tid; i < nc; i += NT) {
-        const float v = sm.cand[i];
-        uint32_t less = 0;
-        for (uint32_t j = 0; j < nc; ++j) {
-          const float w = sm.cand[j];
-          less += (w < v || (w == v && j < i)) ? 1u : 0u;
+      if (nc <= 64) {
+        for (uint32_t i = tid; i < nc; i += NT) {
+          const float v = sm.cand[i];
+          uint32_t less = 0;
+          for (uint32_t j = 0; j < nc; ++j) {
+            const float w = sm.cand[j];
+            less += (w < v || (w == v && j < i)) ? 1u : 0u;
+          }
+          if (less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
         }
-        if (less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
+        __syncthreads();
+      } else {
+        const float m = lof_radix_select_smem<NT>(sm.cand, (int)nc, want, sm.hist, part, sm.ctl);
+        if (tid == 0) { sm.ctl[CT_MEDBITS] = __float_as_uint(m); sm.ctl[CT_FOUND] = 1; }
+        __syncthreads();
       }
-      __syncthreads();
       ok = sm.ctl[CT_FOUND] != 0;
       median = __uint_as_float(sm.ctl[CT_MEDBITS]);
     }
@@ -256,6 +263,23 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
   return n_bad;
 }
 
+__host__ __device__ constexpr int lof_ilog2c(int v) { return v <= 1 ? 0 : 1 + lof_ilog2c(v / 2); }
+
+// Shared-memory layout of a row: float4 chunk g is stored at g ^ ((g >> 3) & 1): adjacent float4 pairs swapped in
+// every odd group of 32 floats.  Column access (32 consecutive t) stays conflict-free, and the time pass's
+// per-lane runs of L consecutive floats (lane stride 96 B for L = 24) become conflict-free LDS.128 as well.
+__device__ __forceinline__ int lof_swz_chunk(int g) { return g ^ ((g >> 3) & 1); }
+__device__ __forceinline__ int lof_swz_elem(int t) { return t ^ (((t >> 5) & 1) << 2); }
+
+// 16-byte asynchronous global -> shared copy (LDGSTS); completion via lof_cp_async_wait_all().
+__device__ __forceinline__ void lof_cp_async16(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void lof_cp_async_wait_all() {
+  asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
+
 // ---- F: SumThreshold along frequency.  One thread per time column; u[c], e[c] in registers.
 template <int C>
 __device__ __forceinline__ void lof_col_rebuild(const float* col, int T, uint64_t fb, float (&u)[C], float (&e)[C],
@@ -267,7 +291,7 @@ __device__ __forceinline__ void lof_col_rebuild(const float* col, int T, uint64_
     e[c] = f ? 0.f : 1.f;
   }
 #pragma unroll
-  for (int j = 1; (1 << j) <= C; ++j) {
+  for (int j = 1; j <= lof_ilog2c(C); ++j) {
     if (j <= k_upto) {
       const int d = 1 << (j - 1);
 #pragma unroll
@@ -285,7 +309,7 @@ __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
   for (int r = 0; r < ROUNDS; ++r) {
     const int col = r * NT + threadIdx.x;               // T and NT are multiples of 32: warps stay whole
     if (col >= T) break;
-    const float* cp = sm.xs + col;
+    const float* cp = sm.xs + lof_swz_elem(col);
     float u[C], e[C];
     uint64_t fb = 0;
     {
@@ -304,7 +328,7 @@ __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
       }
     }
 #pragma unroll
-    for (int k = 1; (1 << k) <= C; ++k) {
+    for (int k = 1; k <= lof_ilog2c(C); ++k) {
       if (k < (int)n_lev_f) {
         const int d = 1 << (k - 1), I = 1 << k;
         const float negT = -sm.thr[k];
@@ -428,7 +452,7 @@ __device__ __forceinline__ void lof_row_level(const float (&x)[L], uint32_t& fb,
 template <int C, int L>
 __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, uint32_t s, bool have_f,
                                uint32_t* __restrict__ flags, double* __restrict__ rowsum,
-                               uint32_t* __restrict__ rowcnt) {
+                               uint32_t* __restrict__ rowcnt, const float* __restrict__ next_stream) {
   using Cfg = LofFusedCfg<C, L>;
   constexpr int T = Cfg::T, NT = Cfg::NT, W = Cfg::W, NW = NT / 32;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -437,10 +461,10 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
   uint32_t n_flag_acc = 0;
   for (int c = warp; c < C; c += NW) {
     float x[L], u[L], e[L];
-    const float4* rp = reinterpret_cast<const float4*>(sm.xs + c * T + lane * L);
+    const float4* rp = reinterpret_cast<const float4*>(sm.xs + c * T);
 #pragma unroll
     for (int q = 0; q < L / 4; ++q) {
-      const float4 v = rp[q];
+      const float4 v = rp[lof_swz_chunk(lane * (L / 4) + q)];
       x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
     }
     uint32_t fb = 0;
@@ -458,6 +482,13 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
         fb |= f ? (1u << j) : 0u;
         u[j] = f ? 0.f : x[j];
         e[j] = f ? 0.f : 1.f;
+      }
+      // the row now lives in registers: its shared-memory slot can take the next stream's row already
+      if (next_stream) {
+        float4* dst = reinterpret_cast<float4*>(sm.xs + c * T);
+        const float4* src = reinterpret_cast<const float4*>(next_stream + c * T);
+#pragma unroll
+        for (int q = 0; q < L / 4; ++q) lof_cp_async16(dst + lof_swz_chunk(q * 32 + lane), src + q * 32 + lane);
       }
       const bool all_flagged = __all_sync(0xffffffffu, fb == maskL);
       if (!all_flagged) {
@@ -519,13 +550,16 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
   constexpr int N = Cfg::N, NT = Cfg::NT, W = Cfg::W;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const LofFusedSmem sm = LofFusedSmem::make<C, L>(smem_raw);
+  bool loaded = false;
   for (uint32_t s = blockIdx.x; s < prm.S; s += gridDim.x) {
-    // load the stream (one read of HBM)
-    const float4* g4 = reinterpret_cast<const float4*>(power + (size_t)s * N);
-    float4* s4 = reinterpret_cast<float4*>(sm.xs);
-#pragma unroll 4
-    for (int i = threadIdx.x; i < N / 4; i += NT) s4[i] = __ldg(g4 + i);
+    if (!loaded) {                                      // first stream of this CTA (or after a skipped one)
+      const float4* g4 = reinterpret_cast<const float4*>(power + (size_t)s * N);
+      float4* s4 = reinterpret_cast<float4*>(sm.xs);
+      for (int i = threadIdx.x; i < N / 4; i += NT) lof_cp_async16(s4 + lof_swz_chunk(i), g4 + i);
+    }
+    lof_cp_async_wait_all();
     __syncthreads();
+    loaded = false;
     const uint32_t n_bad = lof_fused_statistics<C, L>(sm, prm, stats + s);
     if (n_bad) {
       // DESIGN.md S6: the whole stream is flagged
@@ -537,9 +571,14 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
     const bool have_f = prm.n_lev_f > 0;
     if (have_f) lof_fused_freq<C, L>(sm, prm.n_lev_f);
     __syncthreads();
-    lof_fused_time<C, L>(sm, prm, s, have_f, flags, rowsum, rowcnt);
+    const uint32_t s_next = s + gridDim.x;
+    // the time pass prefetches the next stream row by row (only when it runs level 0, i.e. n_lev_t > 0)
+    const bool prefetch = s_next < prm.S && prm.n_lev_t > 0;
+    lof_fused_time<C, L>(sm, prm, s, have_f, flags, rowsum, rowcnt, prefetch ? power + (size_t)s_next * N : nullptr);
+    loaded = prefetch;
     __syncthreads();
     if (threadIdx.x == 0) stats[s].n_flagged = sm.ctl[CT_NFLAG];
     __syncthreads();
   }
+  lof_cp_async_wait_all();
 }
