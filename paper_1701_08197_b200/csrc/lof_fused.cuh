@@ -27,7 +27,10 @@
 template <int C, int L>
 struct LofFusedCfg {
   static constexpr int T = 32 * L, N = C * T, W = L;
-  static constexpr int NT = 256;                         // threads per CTA
+#ifndef LOF_FUSED_NT
+#define LOF_FUSED_NT 256
+#endif
+  static constexpr int NT = LOF_FUSED_NT;                // threads per CTA
   static constexpr int MINB = (C >= 64) ? 1 : 2;
   static constexpr size_t smem_bytes =
       (size_t)N * 4 + (size_t)C * W * 4 + 2048 * 4 + LOF_F_CAP * 4 + 64 * 8 + 64 * 4 + 256 * 4;
@@ -51,7 +54,7 @@ struct LofFusedSmem {
   }
 };
 // ctl slots
-enum { CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS, CT_NFLAG, CT_BAD, CT_SELP, CT_SELACC, CT_PREFIX, CT_RANK, CT_FOUND };
+enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS, CT_NFLAG, CT_BAD, CT_SELP, CT_SELACC, CT_PREFIX, CT_RANK, CT_FOUND };
 
 // Find the bin holding `rank` in hist[NB] (NB a multiple of 256, blockDim >= 256).
 // Results in ctl[CT_BIN] (bin) and ctl[CT_BEFORE] (number of entries in lower bins).
@@ -157,7 +160,7 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
   const float scale = 2046.0f / (2.0f * h);
   const float off = fmaf(-(K - h), scale, 1.0f);        // x = K-h -> 1, x = K+h -> 2047
   for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
-  if (tid == 0) { sm.ctl[CT_NCAND] = 0; sm.ctl[CT_BAD] = 0; sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_FOUND] = 0; }
+  if (tid == 0) { sm.ctl[CT_NCAND] = 0; sm.ctl[CT_BAD] = 0; sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_FOUND] = 0; sm.ctl[CT_ROW] = 0; sm.ctl[CT_COLGRP] = 0; }
   __syncthreads();
   // --- S2: one pass: sums of d = x-K and d^2 in fp32 over groups of 8, folded into fp64; histogram of
   // round(clamp((x-lo)*scale)) (a monotone map of x, so bins are value-ordered).
@@ -281,38 +284,68 @@ __device__ __forceinline__ void lof_cp_async_wait_all() {
 }
 
 // ---- F: SumThreshold along frequency.  One thread per time column; u[c], e[c] in registers.
-template <int C>
-__device__ __forceinline__ void lof_col_rebuild(const float* col, int T, uint64_t fb, float (&u)[C], float (&e)[C],
-                                                int k_upto) {
+// Levels run in order; u, e are doubled in place (ascending c, so u[c + d] is still the previous level).
+// When an iteration sets a new flag anywhere in the warp, the warp restarts from level 0 under the new
+// mask and re-doubles up to that level without testing (k_next), then carries on: every step and every
+// test exists once in the code, which keeps the kernel inside the instruction cache.
+template <int C, int K>
+__device__ __forceinline__ void lof_col_step(float (&u)[C], float (&e)[C]) {
+  constexpr int d = 1 << (K - 1), I = 1 << K;
 #pragma unroll
-  for (int c = 0; c < C; ++c) {
-    const bool f = (fb >> c) & 1ull;
-    u[c] = f ? 0.f : col[c * T];
-    e[c] = f ? 0.f : 1.f;
-  }
+  for (int c = 0; c + I <= C; ++c) { u[c] += u[c + d]; e[c] += e[c + d]; }
+}
+
+template <int C, int K>
+__device__ __forceinline__ bool lof_col_eval(const float (&u)[C], const float (&e)[C], float thr, uint64_t& fb) {
+  constexpr int I = 1 << K;
+  const float negT = -thr;
+  float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
-  for (int j = 1; j <= lof_ilog2c(C); ++j) {
-    if (j <= k_upto) {
-      const int d = 1 << (j - 1);
+  for (int c = 0; c + I <= C; ++c) tm[c & 3] = fmaxf(tm[c & 3], fmaf(e[c], negT, u[c]));   // u - e*T > 0 <=> flagged
+  const bool fired = fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f;
+  bool changed = false;
+  if (__any_sync(0xffffffffu, fired)) {
+    if (fired) {
+      uint64_t trig = 0;
 #pragma unroll
-      for (int c = 0; c + (1 << j) <= C; ++c) { u[c] += u[c + d]; e[c] += e[c + d]; }
+      for (int c = 0; c + I <= C; ++c)
+        if (fmaf(e[c], negT, u[c]) > 0.f) trig |= 1ull << c;
+      uint64_t dil = trig;
+#pragma unroll
+      for (int s = 1; s < I; s <<= 1) dil |= dil << s;
+      const uint64_t nf = fb | dil;
+      changed = nf != fb;
+      fb = nf;
     }
+    changed = __any_sync(0xffffffffu, changed);
   }
+  return changed;
 }
 
 template <int C, int L>
 __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
   using Cfg = LofFusedCfg<C, L>;
-  constexpr int T = Cfg::T, NT = Cfg::NT, W = Cfg::W;
+  constexpr int T = Cfg::T, NT = Cfg::NT, W = Cfg::W, KMAX = lof_ilog2c(C);
   const int lane = threadIdx.x & 31;
-  constexpr int ROUNDS = (T + NT - 1) / NT;
-  for (int r = 0; r < ROUNDS; ++r) {
-    const int col = r * NT + threadIdx.x;               // T and NT are multiples of 32: warps stay whole
-    if (col >= T) break;
+  const int nlf = (int)n_lev_f;
+  (void)NT;
+#pragma unroll 1
+  for (;;) {
+    // groups of 32 columns are handed out dynamically (restarts make their cost uneven)
+    int g = 0;
+    if (lane == 0) g = (int)atomicAdd(&sm.ctl[CT_COLGRP], 1u);
+    g = __shfl_sync(0xffffffffu, g, 0);
+    if (g >= T / 32) break;
+    const int col = g * 32 + lane;
     const float* cp = sm.xs + lof_swz_elem(col);
     float u[C], e[C];
     uint64_t fb = 0;
-    {
+    const float T0 = sm.thr[0];
+    int k_next = 1;
+    bool again = true;
+#pragma unroll 1
+    while (again) {
+      // level 0 under the current mask: I = 1 is the simple thresholder x > threshold_1
       float m0 = -INFINITY, m1 = -INFINITY;
 #pragma unroll
       for (int c = 0; c < C; c += 2) {
@@ -320,48 +353,31 @@ __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
         m0 = fmaxf(m0, u[c]); m1 = fmaxf(m1, u[c + 1]);
         e[c] = 1.f; e[c + 1] = 1.f;
       }
-      const float T0 = sm.thr[0];
-      if (fmaxf(m0, m1) > T0) {                          // level 0: I = 1, the simple thresholder
+      if (fb != 0 || fmaxf(m0, m1) > T0) {
 #pragma unroll
         for (int c = 0; c < C; ++c)
-          if (u[c] > T0) { fb |= 1ull << c; u[c] = 0.f; e[c] = 0.f; }
+          if (((fb >> c) & 1ull) || u[c] > T0) { fb |= 1ull << c; u[c] = 0.f; e[c] = 0.f; }
       }
-    }
-#pragma unroll
-    for (int k = 1; k <= lof_ilog2c(C); ++k) {
-      if (k < (int)n_lev_f) {
-        const int d = 1 << (k - 1), I = 1 << k;
-        const float negT = -sm.thr[k];
-        float t0 = -INFINITY, t1 = -INFINITY;
-#pragma unroll
-        for (int c = 0; c + I <= C; ++c) {
-          u[c] += u[c + d]; e[c] += e[c + d];
-          const float v = fmaf(e[c], negT, u[c]);       // u - e*T > 0  <=>  window flagged
-          if (c & 1) t1 = fmaxf(t1, v); else t0 = fmaxf(t0, v);
-        }
-        if (fmaxf(t0, t1) > 0.f) {
-          uint64_t trig = 0;
-#pragma unroll
-          for (int c = 0; c + I <= C; ++c)
-            if (fmaf(e[c], negT, u[c]) > 0.f) trig |= 1ull << c;
-          uint64_t dil = trig;
-#pragma unroll
-          for (int s = 1; s < I; s <<= 1) dil |= dil << s;
-          const uint64_t nf = fb | dil;
-          if (nf != fb) {
-            fb = nf;
-            if ((1 << (k + 1)) <= C && k + 1 < (int)n_lev_f) lof_col_rebuild<C>(cp, T, fb, u, e, k);
-          }
-        }
+      again = false;
+#define LOF_COL_LEVEL(K)                                                               \
+      if (K <= KMAX && K < nlf && !again) {                                            \
+        lof_col_step<C, (K <= KMAX ? K : 1)>(u, e);                                    \
+        if (K >= k_next && lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e, sm.thr[K], fb) && \
+            K + 1 <= KMAX && K + 1 < nlf) { again = true; k_next = K + 1; }            \
       }
+      LOF_COL_LEVEL(1) LOF_COL_LEVEL(2) LOF_COL_LEVEL(3) LOF_COL_LEVEL(4)
+      LOF_COL_LEVEL(5) LOF_COL_LEVEL(6) LOF_COL_LEVEL(7) LOF_COL_LEVEL(8)
+#undef LOF_COL_LEVEL
     }
     // this warp's 32 columns -> one mask word per channel
     const int w = col >> 5;
     uint32_t mine0 = 0, mine1 = 0;
+    if (__any_sync(0xffffffffu, fb != 0)) {
 #pragma unroll
-    for (int c = 0; c < C; ++c) {
-      const uint32_t word = __ballot_sync(0xffffffffu, (fb >> c) & 1ull);
-      if ((c & 31) == lane) { if (c < 32) mine0 = word; else mine1 = word; }
+      for (int c = 0; c < C; ++c) {
+        const uint32_t word = __ballot_sync(0xffffffffu, (fb >> c) & 1ull);
+        if ((c & 31) == lane) { if (c < 32) mine0 = word; else mine1 = word; }
+      }
     }
     if (lane < C) sm.fm[lane * W + w] = mine0;
     if (C > 32 && lane + 32 < C) sm.fm[(lane + 32) * W + w] = mine1;
@@ -389,64 +405,39 @@ __device__ __forceinline__ void lof_row_step(float (&u)[L], float (&e)[L], int l
   }
 }
 
-template <int L>
-__device__ __forceinline__ void lof_row_rebuild(const float (&x)[L], uint32_t fb, float (&u)[L], float (&e)[L],
-                                                int lane, int k_upto) {
-#pragma unroll
-  for (int j = 0; j < L; ++j) {
-    const bool f = (fb >> j) & 1u;
-    u[j] = f ? 0.f : x[j];
-    e[j] = f ? 0.f : 1.f;
-  }
-  if (k_upto >= 1) lof_row_step<L, 1>(u, e, lane);
-  if (k_upto >= 2) lof_row_step<L, 2>(u, e, lane);
-  if (k_upto >= 3) lof_row_step<L, 4>(u, e, lane);
-  if (k_upto >= 4) lof_row_step<L, 8>(u, e, lane);
-  if (k_upto >= 5) lof_row_step<L, 16>(u, e, lane);
-  if (k_upto >= 6) lof_row_step<L, 32>(u, e, lane);
-  if (k_upto >= 7) lof_row_step<L, 64>(u, e, lane);
-  if (k_upto >= 8) lof_row_step<L, 128>(u, e, lane);
-  if (k_upto >= 9) lof_row_step<L, 256>(u, e, lane);
-}
-
-// One iteration I = 2^K (K >= 1) on a row: doubling step, test, and - if any window fired - flag
-// dilation across the warp and a rebuild of u, e under the new flags.  Returns nothing; fb updated.
+// Test of iteration I = 2^K on a row after its doubling step: fire windows with u > e*T, dilate the fired
+// starts over I samples across lanes, OR into fb.  Returns (warp-uniform) whether any flag is new.
 template <int L, int K>
-__device__ __forceinline__ void lof_row_level(const float (&x)[L], uint32_t& fb, float (&u)[L], float (&e)[L],
-                                              int lane, float thr, bool more_levels) {
+__device__ __forceinline__ bool lof_row_eval(const float (&u)[L], const float (&e)[L], int lane, float thr,
+                                             uint32_t& fb) {
   constexpr int I = 1 << K;
-  lof_row_step<L, (I >> 1)>(u, e, lane);
   const float negT = -thr;
-  float t0 = -INFINITY, t1 = -INFINITY;
+  float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
-  for (int j = 0; j < L; ++j) {
-    const float v = fmaf(e[j], negT, u[j]);
-    if (j & 1) t1 = fmaxf(t1, v); else t0 = fmaxf(t0, v);
-  }
-  if (__any_sync(0xffffffffu, fmaxf(t0, t1) > 0.f)) {
-    uint32_t trig = 0;
+  for (int j = 0; j < L; ++j) tm[j & 3] = fmaxf(tm[j & 3], fmaf(e[j], negT, u[j]));
+  if (!__any_sync(0xffffffffu, fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f)) return false;
+  uint32_t trig = 0;
 #pragma unroll
-    for (int j = 0; j < L; ++j) trig |= (fmaf(e[j], negT, u[j]) > 0.f) ? (1u << j) : 0u;
-    // own windows, inside the lane's L bits
-    uint32_t own = trig;
+  for (int j = 0; j < L; ++j) trig |= (fmaf(e[j], negT, u[j]) > 0.f) ? (1u << j) : 0u;
+  // own windows, inside the lane's L bits
+  uint32_t own = trig;
 #pragma unroll
-    for (int s = 1; s < I && s < 32; s <<= 1) own |= own << s;
-    // windows started in earlier lanes: sample p is covered iff p < (last start before this lane) + I
-    int hi = trig ? (lane * L + 31 - __clz(trig)) : -(1 << 20);
-    int pm = hi;
+  for (int s = 1; s < I && s < 32; s <<= 1) own |= own << s;
+  // windows started in earlier lanes: sample p is covered iff p < (last start before this lane) + I
+  const int hi = trig ? (lane * L + 31 - __clz(trig)) : -(1 << 20);
+  int pm = hi;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pm, o); if (lane >= o) pm = max(pm, v); }
-    int prev = __shfl_up_sync(0xffffffffu, pm, 1);
-    if (lane == 0) prev = -(1 << 20);
-    int cnt = prev + I - lane * L;
-    cnt = cnt < 0 ? 0 : (cnt > L ? L : cnt);
-    const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
-    const uint32_t pre = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
-    const uint32_t nf = (fb | own | pre) & maskL;
-    const bool changed = nf != fb;
-    fb = nf;
-    if (more_levels && __any_sync(0xffffffffu, changed)) lof_row_rebuild<L>(x, fb, u, e, lane, K);
-  }
+  for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pm, o); if (lane >= o) pm = max(pm, v); }
+  int prev = __shfl_up_sync(0xffffffffu, pm, 1);
+  if (lane == 0) prev = -(1 << 20);
+  int cnt = prev + I - lane * L;
+  cnt = cnt < 0 ? 0 : (cnt > L ? L : cnt);
+  const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
+  const uint32_t pre = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
+  const uint32_t nf = (fb | own | pre) & maskL;
+  const bool changed = nf != fb;
+  fb = nf;
+  return __any_sync(0xffffffffu, changed);
 }
 
 template <int C, int L>
@@ -459,7 +450,14 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
   const uint32_t nlt = prm.n_lev_t;
   const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
   uint32_t n_flag_acc = 0;
-  for (int c = warp; c < C; c += NW) {
+  (void)warp; (void)NW;
+#pragma unroll 1
+  for (;;) {
+    // rows are handed out dynamically: their cost varies with the number of restarts
+    int c = 0;
+    if (lane == 0) c = (int)atomicAdd(&sm.ctl[CT_ROW], 1u);
+    c = __shfl_sync(0xffffffffu, c, 0);
+    if (c >= C) break;
     float x[L], u[L], e[L];
     const float4* rp = reinterpret_cast<const float4*>(sm.xs + c * T);
 #pragma unroll
@@ -474,34 +472,45 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
       fb = __funnelshift_r(lo, hi, r) & maskL;
     }
     if (nlt > 0) {
-      // level 0 (I = 1): x > threshold_1 on samples not yet flagged
       const float T0 = sm.thr[0];
+      int k_next = 1;
+      bool again = true;
+#pragma unroll 1
+      while (again) {
+        // level 0 (I = 1) under the current mask: x > threshold_1 on samples not yet flagged
 #pragma unroll
-      for (int j = 0; j < L; ++j) {
-        const bool f = ((fb >> j) & 1u) || (x[j] > T0);
-        fb |= f ? (1u << j) : 0u;
-        u[j] = f ? 0.f : x[j];
-        e[j] = f ? 0.f : 1.f;
-      }
-      // the row now lives in registers: its shared-memory slot can take the next stream's row already
-      if (next_stream) {
-        float4* dst = reinterpret_cast<float4*>(sm.xs + c * T);
-        const float4* src = reinterpret_cast<const float4*>(next_stream + c * T);
+        for (int j = 0; j < L; ++j) {
+          const bool f = ((fb >> j) & 1u) || (x[j] > T0);
+          fb |= f ? (1u << j) : 0u;
+          u[j] = f ? 0.f : x[j];
+          e[j] = f ? 0.f : 1.f;
+        }
+        again = false;
+        // the row lives in registers now (level 0 consumed every x[j]): its shared-memory slot can
+        // already take the next stream's row
+        if (next_stream && k_next == 1) {
+          float4* dst = reinterpret_cast<float4*>(sm.xs + c * T);
+          const float4* src = reinterpret_cast<const float4*>(next_stream + c * T);
 #pragma unroll
-        for (int q = 0; q < L / 4; ++q) lof_cp_async16(dst + lof_swz_chunk(q * 32 + lane), src + q * 32 + lane);
+          for (int q = 0; q < L / 4; ++q) lof_cp_async16(dst + lof_swz_chunk(q * 32 + lane), src + q * 32 + lane);
+        }
+        if (__all_sync(0xffffffffu, fb == maskL)) break;   // nothing left to test in this row
+#define LOF_ROW_LEVEL(K)                                                                   \
+        if (K < (int)nlt && !again) {                                                      \
+          lof_row_step<L, (1 << (K - 1))>(u, e, lane);                                     \
+          if (K >= k_next && lof_row_eval<L, K>(u, e, lane, sm.thr[K], fb) && K + 1 < (int)nlt) { \
+            again = true; k_next = K + 1;                                                  \
+          }                                                                                \
+        }
+        LOF_ROW_LEVEL(1) LOF_ROW_LEVEL(2) LOF_ROW_LEVEL(3) LOF_ROW_LEVEL(4) LOF_ROW_LEVEL(5)
+        LOF_ROW_LEVEL(6) LOF_ROW_LEVEL(7) LOF_ROW_LEVEL(8) LOF_ROW_LEVEL(9)
+#undef LOF_ROW_LEVEL
       }
-      const bool all_flagged = __all_sync(0xffffffffu, fb == maskL);
-      if (!all_flagged) {
-        if (nlt > 1) lof_row_level<L, 1>(x, fb, u, e, lane, sm.thr[1], nlt > 2);
-        if (nlt > 2) lof_row_level<L, 2>(x, fb, u, e, lane, sm.thr[2], nlt > 3);
-        if (nlt > 3) lof_row_level<L, 3>(x, fb, u, e, lane, sm.thr[3], nlt > 4);
-        if (nlt > 4) lof_row_level<L, 4>(x, fb, u, e, lane, sm.thr[4], nlt > 5);
-        if (nlt > 5) lof_row_level<L, 5>(x, fb, u, e, lane, sm.thr[5], nlt > 6);
-        if (nlt > 6) lof_row_level<L, 6>(x, fb, u, e, lane, sm.thr[6], nlt > 7);
-        if (nlt > 7) lof_row_level<L, 7>(x, fb, u, e, lane, sm.thr[7], nlt > 8);
-        if (nlt > 8) lof_row_level<L, 8>(x, fb, u, e, lane, sm.thr[8], nlt > 9);
-        if (nlt > 9) lof_row_level<L, 9>(x, fb, u, e, lane, sm.thr[9], false);
-      }
+    } else if (next_stream) {
+      float4* dst = reinterpret_cast<float4*>(sm.xs + c * T);
+      const float4* src = reinterpret_cast<const float4*>(next_stream + c * T);
+#pragma unroll
+      for (int q = 0; q < L / 4; ++q) lof_cp_async16(dst + lof_swz_chunk(q * 32 + lane), src + q * 32 + lane);
     }
     // bit-pack: word w of the row = bits [32w, 32w+32) gathered from the lanes' L-bit masks
     {
@@ -551,6 +560,7 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const LofFusedSmem sm = LofFusedSmem::make<C, L>(smem_raw);
   bool loaded = false;
+#pragma unroll 1
   for (uint32_t s = blockIdx.x; s < prm.S; s += gridDim.x) {
     if (!loaded) {                                      // first stream of this CTA (or after a skipped one)
       const float4* g4 = reinterpret_cast<const float4*>(power + (size_t)s * N);
@@ -572,8 +582,8 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
     if (have_f) lof_fused_freq<C, L>(sm, prm.n_lev_f);
     __syncthreads();
     const uint32_t s_next = s + gridDim.x;
-    // the time pass prefetches the next stream row by row (only when it runs level 0, i.e. n_lev_t > 0)
-    const bool prefetch = s_next < prm.S && prm.n_lev_t > 0;
+    // the time pass prefetches the next stream row by row, as each row moves into registers
+    const bool prefetch = s_next < prm.S;
     lof_fused_time<C, L>(sm, prm, s, have_f, flags, rowsum, rowcnt, prefetch ? power + (size_t)s_next * N : nullptr);
     loaded = prefetch;
     __syncthreads();

@@ -9,7 +9,7 @@ import os
 import numpy as np
 
 _DIR = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_DIR, "liblof.so")
+LIB_PATH = os.environ.get("LOF_LIB_PATH") or os.path.join(_DIR, "liblof.so")   # override: kernel experiments
 
 DIR_FREQ, DIR_TIME = 1, 2
 MAX_LEVELS = 11
