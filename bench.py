@@ -194,11 +194,9 @@ def run_gpu(args):
     sampler.stop_flag = True
     sampler.join()
     per = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps))
-    t = torch.tensor([total_ms], device="cuda")
-    if dist:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
-    value = world * n_samples * args.steps / (total_ms * 1e-3) / 1e9
+    from paper_1701_08197_b200 import sharding
+    total_ms = sharding.max_over_ranks(total_ms, device="cuda")
+    value = sharding.aggregate_rate(n_samples, args.steps, total_ms, world) / 1e9
 
     # end to end through the C-ABI host entry point: pinned host input -> flags + stats on the host
     hp = torch.from_numpy(power).pin_memory()
@@ -213,10 +211,8 @@ def run_gpu(args):
     for _ in range(e2e_steps):
         f.flag_block_host(hp, hf, hs)
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], device="cuda")
-    if dist:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_val = world * n_samples * e2e_steps / float(te.item()) / 1e9
+    e2e_s = sharding.max_over_ranks(e2e_s, device="cuda")
+    e2e_val = sharding.aggregate_rate(n_samples, e2e_steps, e2e_s * 1e3, world) / 1e9
 
     if rank != 0:
         return

@@ -201,3 +201,28 @@ def test_host_entry_point(lof, lofo, wl):
     assert_stats(hs.numpy().view(lof.STATS_DTYPE).reshape(-1), ora["stats"])
     assert f.launch_count() > 0
     f.close()
+
+
+def test_bench_configuration_sampled_streams(lof, lofo, wl):
+    """The launch configuration bench.py times (config 2 batched over subbands, S a multiple of 96 far above
+    the number of SMs, persistent CTAs looping over streams with prefetch): every stream of a sample is
+    compared with the oracle, which computes streams one by one."""
+    import torch
+    w = wl.config2(0, n_subbands=16, want_truth=False)             # 1536 streams = 10.4 per SM
+    S, C, T = w.power.shape
+    f = lof.Flagger(S, C, T, max_window=64)
+    flags, stats = f.flag_block(torch.from_numpy(w.power).cuda())
+    torch.cuda.synchronize()
+    g = lof.flags_to_numpy(flags)
+    st = lof.stats_to_numpy(stats)
+    pick = np.unique(np.concatenate([np.arange(0, 8), np.arange(S - 8, S),
+                                     np.random.default_rng(3).integers(0, S, 240)]))
+    prm = lofo.make_params(len(pick), C, T, max_window=64)
+    ora = lofo.flag_block_threads(prm, w.power[pick], 8, want_margin=True)
+    assert_stats(st[pick], ora["stats"])
+    r = assert_flags(g[pick], ora, T, 64)
+    assert np.array_equal(st["n_flagged"][pick], ora["stats"]["n_flagged"]) or r["n_mismatch"] > 0
+    # properties that hold at any size: n_flagged equals the popcount of the words; padding-free rows
+    pop = np.unpackbits(g.view(np.uint8), axis=-1).reshape(S, -1).sum(axis=1)
+    assert np.array_equal(pop.astype(np.uint64), st["n_flagged"])
+    f.close()
