@@ -34,6 +34,17 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def measured_traffic(config):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, or None."""
+    import csv
+    p = os.path.join(ROOT, "profiles", "r01_fused_traffic.csv")
+    if os.path.exists(p):
+        for r in csv.DictReader(open(p)):
+            if r["config"] == config:
+                return float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]), r["kernel"]
+    return None, None
+
+
 def make_workload(name, seed=0):
     """Returns (power float32 [S][C][T] numpy, dict of Flagger kwargs, description, block seconds)."""
     from paper_1701_08197_b200 import workloads as wl
@@ -219,6 +230,8 @@ def run_gpu(args):
     peak, peak_src = measured_peaks()
     ms_step = total_ms / args.steps
     achieved = n_samples * ALGO_BYTES_PER_SAMPLE / (ms_step * 1e-3) / 1e9
+    traffic, kname = measured_traffic(args.config)
+    one_kernel = launches == args.steps * (2 if has_hist else 1) - (args.steps if has_hist else 0) or launches == args.steps
     cpu_val, cores, sample = oracle_rate(power, kw)
     line = {
         "metric": "Gsamples/s flagged", "value": value, "unit": "Gsamples/s", "n_gpus": world,
@@ -233,8 +246,10 @@ def run_gpu(args):
         "e2e": {"value": e2e_val, "unit": "Gsamples/s", "h2d_bytes_per_step": n_samples * 4,
                 "d2h_bytes_per_step": S * C * f.W * 4 + S * 32, "steps": e2e_steps},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src, "frac_of_8TBs": achieved / 8000.0,
-                     "kernel": "whole step (all kernels of lof_flag_block)",
+                     "traffic": traffic, "peak_source": peak_src, "frac_of_8TBs": achieved / 8000.0,
+                     "kernel": (kname or "lof_k_fused") + " (one launch per step)" if one_kernel
+                     else "whole step (all kernels of lof_flag_block, generic path)",
+                     "algorithmic_bytes_per_launch": n_samples * ALGO_BYTES_PER_SAMPLE,
                      "algorithmic_bytes_per_sample": ALGO_BYTES_PER_SAMPLE},
         "cpu_baseline": {"value": cpu_val / 1e9, "unit": "Gsamples/s", "cores": cores, "kind": "oracle", "sample": sample},
     }
