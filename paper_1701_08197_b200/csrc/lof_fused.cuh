@@ -18,6 +18,8 @@
 // Flags are frozen during an iteration (F8): u and e are rebuilt from level 0 whenever
 // an iteration set a new flag.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "lof_common.cuh"
 
 #define LOF_F_NBINS 2048
@@ -27,10 +29,13 @@
 template <int C, int L>
 struct LofFusedCfg {
   static constexpr int T = 32 * L, N = C * T, W = L;
-#ifndef LOF_FUSED_NT
-#define LOF_FUSED_NT 256
+  // threads per CTA: the 64-channel column (64 sums + 32 packed counts in registers) allows 12 warps at
+  // 168 registers; 24 column groups and 64 rows then split evenly enough over 12 warps
+#ifdef LOF_FUSED_NT
+  static constexpr int NT = LOF_FUSED_NT;
+#else
+  static constexpr int NT = (C >= 64) ? 384 : 256;
 #endif
-  static constexpr int NT = LOF_FUSED_NT;                // threads per CTA
   static constexpr int MINB = (C >= 64) ? 1 : 2;
   static constexpr size_t smem_bytes =
       (size_t)N * 4 + (size_t)C * W * 4 + 2048 * 4 + LOF_F_CAP * 4 + 64 * 8 + 64 * 4 + 256 * 4;
@@ -233,7 +238,7 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
       __syncthreads();
       // S5: the candidate with exactly (rank - before) candidates ordered before it
       const uint32_t want = rank - before, nc = sm.ctl[CT_NCAND];
-      if (nc <= 64) {
+      if (nc <= 256) {
         for (uint32_t i = tid; i < nc; i += NT) {
           const float v = sm.cand[i];
           uint32_t less = 0;
@@ -288,28 +293,65 @@ __device__ __forceinline__ void lof_cp_async_wait_all() {
 // When an iteration sets a new flag anywhere in the warp, the warp restarts from level 0 under the new
 // mask and re-doubles up to that level without testing (k_next), then carries on: every step and every
 // test exists once in the code, which keeps the kernel inside the instruction cache.
-template <int C, int K>
-__device__ __forceinline__ void lof_col_step(float (&u)[C], float (&e)[C]) {
-  constexpr int d = 1 << (K - 1), I = 1 << K;
-#pragma unroll
-  for (int c = 0; c + I <= C; ++c) { u[c] += u[c + d]; e[c] += e[c + d]; }
+// e (number of unflagged samples of a window, an integer <= 1024) is kept as packed halves, two window
+// positions per register: exact, half the registers of fp32 (the 64-channel column then fits 128 registers
+// per thread, i.e. 16 warps per SM), and one HADD2 doubles two positions.
+#define LOF_H2_ONES 0x3C003C00u
+__device__ __forceinline__ __half2 lof_h2_bits(uint32_t b) { return *reinterpret_cast<__half2*>(&b); }
+__device__ __forceinline__ uint32_t lof_bits_h2(__half2 h) { return *reinterpret_cast<uint32_t*>(&h); }
+// (a.hi, b.lo): the pair starting one position later
+__device__ __forceinline__ __half2 lof_h2_shift1(__half2 a, __half2 b) {
+  return lof_h2_bits(__byte_perm(lof_bits_h2(a), lof_bits_h2(b), 0x5432));
+}
+// e of two consecutive positions from their flag bits (bit 0 = first): 1.0 where unflagged, 0.0 where flagged
+__device__ __forceinline__ __half2 lof_h2_unflagged(uint32_t two_flag_bits) {
+  const uint32_t keep = ((two_flag_bits & 1u) ? 0u : 0x0000FFFFu) | ((two_flag_bits & 2u) ? 0u : 0xFFFF0000u);
+  return lof_h2_bits(LOF_H2_ONES & keep);
 }
 
 template <int C, int K>
-__device__ __forceinline__ bool lof_col_eval(const float (&u)[C], const float (&e)[C], float thr, uint64_t& fb) {
+__device__ __forceinline__ void lof_col_step(float (&u)[C], __half2 (&e2)[C / 2]) {
+  constexpr int d = 1 << (K - 1), I = 1 << K;
+#pragma unroll
+  for (int c = 0; c + I <= C; ++c) u[c] += u[c + d];
+  if constexpr (K == 1) {
+#pragma unroll
+    for (int m = 0; m < C / 2; ++m)
+      e2[m] = __hadd2(e2[m], lof_h2_shift1(e2[m], e2[m + 1 < C / 2 ? m + 1 : m]));
+  } else {
+#pragma unroll
+    for (int m = 0; 2 * m + I <= C; ++m) e2[m] = __hadd2(e2[m], e2[m + d / 2]);
+  }
+}
+
+// v[c] = u[c] - e[c]*T for the two positions of pair m
+#define LOF_COL_V(m, v0, v1)                                   \
+  const float2 ef_ = __half22float2(e2[m]);                    \
+  const float v0 = fmaf(ef_.x, negT, u[2 * (m)]);              \
+  const float v1 = fmaf(ef_.y, negT, u[2 * (m) + 1]);
+
+template <int C, int K>
+__device__ __forceinline__ bool lof_col_eval(const float (&u)[C], const __half2 (&e2)[C / 2], float thr, uint64_t& fb) {
   constexpr int I = 1 << K;
   const float negT = -thr;
   float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
-  for (int c = 0; c + I <= C; ++c) tm[c & 3] = fmaxf(tm[c & 3], fmaf(e[c], negT, u[c]));   // u - e*T > 0 <=> flagged
+  for (int m = 0; 2 * m + I <= C; ++m) {
+    LOF_COL_V(m, v0, v1)
+    tm[(2 * m) & 3] = fmaxf(tm[(2 * m) & 3], v0);                          // u - e*T > 0 <=> window flagged
+    if (2 * m + 1 + I <= C) tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], v1);
+  }
   const bool fired = fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f;
   bool changed = false;
   if (__any_sync(0xffffffffu, fired)) {
     if (fired) {
       uint64_t trig = 0;
 #pragma unroll
-      for (int c = 0; c + I <= C; ++c)
-        if (fmaf(e[c], negT, u[c]) > 0.f) trig |= 1ull << c;
+      for (int m = 0; 2 * m + I <= C; ++m) {
+        LOF_COL_V(m, v0, v1)
+        if (v0 > 0.f) trig |= 1ull << (2 * m);
+        if (2 * m + 1 + I <= C && v1 > 0.f) trig |= 1ull << (2 * m + 1);
+      }
       uint64_t dil = trig;
 #pragma unroll
       for (int s = 1; s < I; s <<= 1) dil |= dil << s;
@@ -338,7 +380,8 @@ __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
     if (g >= T / 32) break;
     const int col = g * 32 + lane;
     const float* cp = sm.xs + lof_swz_elem(col);
-    float u[C], e[C];
+    float u[C];
+    __half2 e2[C / 2];
     uint64_t fb = 0;
     const float T0 = sm.thr[0];
     int k_next = 1;
@@ -351,18 +394,20 @@ __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
       for (int c = 0; c < C; c += 2) {
         u[c] = cp[c * T]; u[c + 1] = cp[(c + 1) * T];
         m0 = fmaxf(m0, u[c]); m1 = fmaxf(m1, u[c + 1]);
-        e[c] = 1.f; e[c + 1] = 1.f;
+        e2[c / 2] = lof_h2_bits(LOF_H2_ONES);
       }
       if (fb != 0 || fmaxf(m0, m1) > T0) {
 #pragma unroll
         for (int c = 0; c < C; ++c)
-          if (((fb >> c) & 1ull) || u[c] > T0) { fb |= 1ull << c; u[c] = 0.f; e[c] = 0.f; }
+          if (((fb >> c) & 1ull) || u[c] > T0) { fb |= 1ull << c; u[c] = 0.f; }
+#pragma unroll
+        for (int m = 0; m < C / 2; ++m) e2[m] = lof_h2_unflagged((uint32_t)(fb >> (2 * m)) & 3u);
       }
       again = false;
 #define LOF_COL_LEVEL(K)                                                               \
       if (K <= KMAX && K < nlf && !again) {                                            \
-        lof_col_step<C, (K <= KMAX ? K : 1)>(u, e);                                    \
-        if (K >= k_next && lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e, sm.thr[K], fb) && \
+        lof_col_step<C, (K <= KMAX ? K : 1)>(u, e2);                                   \
+        if (K >= k_next && lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e2, sm.thr[K], fb) && \
             K + 1 <= KMAX && K + 1 < nlf) { again = true; k_next = K + 1; }            \
       }
       LOF_COL_LEVEL(1) LOF_COL_LEVEL(2) LOF_COL_LEVEL(3) LOF_COL_LEVEL(4)
@@ -388,37 +433,57 @@ __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
 // One doubling step of distance D (window 2D): partners beyond the lane's own L samples come from the
 // following lanes by shuffle; a partner outside the row is -inf, so such windows never fire.
 template <int L, int D>
-__device__ __forceinline__ void lof_row_step(float (&u)[L], float (&e)[L], int lane) {
-  constexpr int NP = D < L ? D : L;
-  float pu[NP], pe[NP];
+__device__ __forceinline__ void lof_row_step(float (&u)[L], __half2 (&e2)[L / 2], int lane) {
+  if constexpr (D == 1) {
+    float pu = __shfl_down_sync(0xffffffffu, u[0], 1);
+    const uint32_t pe = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[0]), 1);
+    if (lane == 31) pu = -INFINITY;
 #pragma unroll
-  for (int jj = 0; jj < NP; ++jj) {
-    const int j = L - NP + jj, src = (j + D) % L, off = (j + D) / L;
-    pu[jj] = __shfl_down_sync(0xffffffffu, u[src], off);
-    pe[jj] = __shfl_down_sync(0xffffffffu, e[src], off);
-    if (lane + off > 31) pu[jj] = -INFINITY;
-  }
+    for (int j = 0; j < L; ++j) u[j] += (j + 1 < L) ? u[j + 1] : pu;
 #pragma unroll
-  for (int j = 0; j < L; ++j) {
-    if (j + D < L) { u[j] += u[j + D]; e[j] += e[j + D]; }
-    else { u[j] += pu[j - (L - NP)]; e[j] += pe[j - (L - NP)]; }
+    for (int m = 0; m < L / 2; ++m)
+      e2[m] = __hadd2(e2[m], lof_h2_shift1(e2[m], (m + 1 < L / 2) ? e2[m + 1] : lof_h2_bits(pe)));
+  } else {
+    constexpr int NP = D < L ? D : L;                   // elements whose partner lives in a following lane
+    float pu[NP];
+    uint32_t pe[NP / 2];
+#pragma unroll
+    for (int jj = 0; jj < NP; ++jj) {
+      const int j = L - NP + jj, src = (j + D) % L, off = (j + D) / L;
+      pu[jj] = __shfl_down_sync(0xffffffffu, u[src], off);
+      if (lane + off > 31) pu[jj] = -INFINITY;
+      if ((jj & 1) == 0) pe[jj / 2] = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[src / 2]), off);
+    }
+#pragma unroll
+    for (int j = 0; j < L; ++j) u[j] += (j + D < L) ? u[j + D] : pu[j - (L - NP)];
+#pragma unroll
+    for (int m = 0; m < L / 2; ++m)
+      e2[m] = __hadd2(e2[m], (2 * m + D < L) ? e2[m + D / 2] : lof_h2_bits(pe[(2 * m - (L - NP)) / 2]));
   }
 }
 
 // Test of iteration I = 2^K on a row after its doubling step: fire windows with u > e*T, dilate the fired
 // starts over I samples across lanes, OR into fb.  Returns (warp-uniform) whether any flag is new.
 template <int L, int K>
-__device__ __forceinline__ bool lof_row_eval(const float (&u)[L], const float (&e)[L], int lane, float thr,
+__device__ __forceinline__ bool lof_row_eval(const float (&u)[L], const __half2 (&e2)[L / 2], int lane, float thr,
                                              uint32_t& fb) {
   constexpr int I = 1 << K;
   const float negT = -thr;
   float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
-  for (int j = 0; j < L; ++j) tm[j & 3] = fmaxf(tm[j & 3], fmaf(e[j], negT, u[j]));
+  for (int m = 0; m < L / 2; ++m) {
+    const float2 ef = __half22float2(e2[m]);
+    tm[(2 * m) & 3] = fmaxf(tm[(2 * m) & 3], fmaf(ef.x, negT, u[2 * m]));
+    tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], fmaf(ef.y, negT, u[2 * m + 1]));
+  }
   if (!__any_sync(0xffffffffu, fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f)) return false;
   uint32_t trig = 0;
 #pragma unroll
-  for (int j = 0; j < L; ++j) trig |= (fmaf(e[j], negT, u[j]) > 0.f) ? (1u << j) : 0u;
+  for (int m = 0; m < L / 2; ++m) {
+    const float2 ef = __half22float2(e2[m]);
+    trig |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
+    trig |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
+  }
   // own windows, inside the lane's L bits
   uint32_t own = trig;
 #pragma unroll
@@ -458,7 +523,8 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
     if (lane == 0) c = (int)atomicAdd(&sm.ctl[CT_ROW], 1u);
     c = __shfl_sync(0xffffffffu, c, 0);
     if (c >= C) break;
-    float x[L], u[L], e[L];
+    float x[L], u[L];
+    __half2 e2[L / 2];
     const float4* rp = reinterpret_cast<const float4*>(sm.xs + c * T);
 #pragma unroll
     for (int q = 0; q < L / 4; ++q) {
@@ -483,8 +549,9 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
           const bool f = ((fb >> j) & 1u) || (x[j] > T0);
           fb |= f ? (1u << j) : 0u;
           u[j] = f ? 0.f : x[j];
-          e[j] = f ? 0.f : 1.f;
         }
+#pragma unroll
+        for (int m = 0; m < L / 2; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
         again = false;
         // the row lives in registers now (level 0 consumed every x[j]): its shared-memory slot can
         // already take the next stream's row
@@ -497,8 +564,8 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
         if (__all_sync(0xffffffffu, fb == maskL)) break;   // nothing left to test in this row
 #define LOF_ROW_LEVEL(K)                                                                   \
         if (K < (int)nlt && !again) {                                                      \
-          lof_row_step<L, (1 << (K - 1))>(u, e, lane);                                     \
-          if (K >= k_next && lof_row_eval<L, K>(u, e, lane, sm.thr[K], fb) && K + 1 < (int)nlt) { \
+          lof_row_step<L, (1 << (K - 1))>(u, e2, lane);                                     \
+          if (K >= k_next && lof_row_eval<L, K>(u, e2, lane, sm.thr[K], fb) && K + 1 < (int)nlt) { \
             again = true; k_next = K + 1;                                                  \
           }                                                                                \
         }
