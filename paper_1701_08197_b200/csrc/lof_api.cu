@@ -11,6 +11,7 @@
 #include "lof_flag_generic.cuh"
 #include "lof_history.cuh"
 #include "lof_fused.cuh"
+#include "lof_longrow.cuh"
 
 static thread_local char g_cuda_err[256] = "";
 
@@ -34,6 +35,8 @@ struct lof_ctx {
   uint32_t group;                 // streams per group (bounded so a group's input stays in L2)
   uint32_t n_chunks;              // statistics chunks per stream
   uint32_t TT, halo, n_tiles;     // time tiling
+  bool lr_freq, lr_time;          // register-resident long-row kernels usable (lof_longrow.cuh)
+  uint32_t seg_out, seg_halo, n_seg;
   size_t smem_freq, smem_time;
   // device memory owned by the context
   LofStreamState* d_state;
@@ -168,6 +171,13 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   const uint32_t TT0 = 4096;
   if (T <= TT0 + 2 * ((cone + 31) & ~31u)) { c->TT = (T + 31) & ~31u; c->halo = 0; c->n_tiles = 1; }
   else { c->TT = TT0; c->halo = (cone + 31) & ~31u; c->n_tiles = (T + TT0 - 1) / TT0; }
+  // register-resident long-row kernels: columns of 16/32/64 channels; row segments of 1024 samples whose
+  // halo (the cone, rounded up to 32) leaves at least half of the segment as output
+  c->lr_freq = (C == 16 || C == 32 || C == 64);
+  c->seg_halo = (cone + 31) & ~31u;
+  c->lr_time = c->seg_halo <= 256;
+  c->seg_out = c->lr_time ? LOF_LR_TILE - 2 * c->seg_halo : LOF_LR_TILE;
+  c->n_seg = (T + c->seg_out - 1) / c->seg_out;
   c->smem_freq = (size_t)C * 32 * LOF_GEN_BYTES_PER_ELEM;
   c->smem_time = (size_t)((c->TT + 2 * c->halo + 31) & ~31u) * LOF_GEN_BYTES_PER_ELEM;
 
@@ -177,8 +187,9 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   A(dev_alloc(&c->d_hist, (size_t)c->group * LOF_HIST_BINS));
   A(dev_alloc(&c->d_partial, (size_t)c->group * c->n_chunks * 2));
   A(dev_alloc(&c->d_fmask, (size_t)S * C * W));
-  A(dev_alloc(&c->d_part_sum, (size_t)c->group * C * c->n_tiles));
-  A(dev_alloc(&c->d_part_cnt, (size_t)c->group * C * c->n_tiles));
+  const size_t n_part = c->n_tiles > c->n_seg ? c->n_tiles : c->n_seg;
+  A(dev_alloc(&c->d_part_sum, (size_t)c->group * C * n_part));
+  A(dev_alloc(&c->d_part_cnt, (size_t)c->group * C * n_part));
   A(dev_alloc(&c->d_rowsum, (size_t)S * C));
   A(dev_alloc(&c->d_rowcnt, (size_t)S * C));
   A(dev_alloc(&c->d_stats, S));
@@ -213,15 +224,33 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
     lof_k_hist<In, 2><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
     lof_k_scan<In, 2><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
     c->launches += 7;
+    const bool fast = c->path == 0;                     // path 1 forces the shared-memory generic kernels
     if (kp.n_lev_f) {
-      lof_k_freq_generic<In><<<G * kp.W, LOF_GEN_THREADS, c->smem_freq, st>>>(in, kp, c->d_state, c->d_fmask);
+      const uint32_t nb_f = (uint32_t)(((uint64_t)G * kp.W + LOF_LR_WARPS - 1) / LOF_LR_WARPS);
+      if (fast && c->lr_freq && C == 16)
+        lof_k_freq_reg<16, In><<<nb_f, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, G);
+      else if (fast && c->lr_freq && C == 32)
+        lof_k_freq_reg<32, In><<<nb_f, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, G);
+      else if (fast && c->lr_freq && C == 64)
+        lof_k_freq_reg<64, In><<<nb_f, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, G);
+      else
+        lof_k_freq_generic<In><<<G * kp.W, LOF_GEN_THREADS, c->smem_freq, st>>>(in, kp, c->d_state, c->d_fmask);
       c->launches += 1;
     }
     const uint32_t rows = G * C;
-    lof_k_time_generic<In><<<rows * c->n_tiles, LOF_GEN_THREADS, c->smem_time, st>>>(
-        in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum, c->d_part_cnt, c->d_stats, c->TT, c->halo, c->n_tiles);
+    uint32_t n_part;
+    if (fast && c->lr_time) {
+      n_part = c->n_seg;
+      const uint32_t nb_t = (uint32_t)(((uint64_t)rows * n_part + LOF_LR_WARPS - 1) / LOF_LR_WARPS);
+      lof_k_time_seg<In><<<nb_t, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum,
+                                                        c->d_part_cnt, c->d_stats, c->seg_out, c->seg_halo, n_part, rows);
+    } else {
+      n_part = c->n_tiles;
+      lof_k_time_generic<In><<<rows * c->n_tiles, LOF_GEN_THREADS, c->smem_time, st>>>(
+          in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum, c->d_part_cnt, c->d_stats, c->TT, c->halo, c->n_tiles);
+    }
     lof_k_rowsum_final<<<(rows + 255) / 256, 256, 0, st>>>(c->d_part_sum, c->d_part_cnt, c->d_rowsum, c->d_rowcnt,
-                                                           (uint64_t)s0 * C, rows, c->n_tiles);
+                                                           (uint64_t)s0 * C, rows, n_part);
     c->launches += 2;
   }
   LOF_CUDA(cudaGetLastError());

@@ -364,13 +364,66 @@ __device__ __forceinline__ bool lof_col_eval(const float (&u)[C], const __half2 
   return changed;
 }
 
+// The frequency run of one column: ld(c) returns the sample of channel c (called again on a restart).
+// Returns the column's flag mask (bit c).  Every lane of the warp must call it (warp-uniform restarts).
+template <int C, class Ld>
+__device__ __forceinline__ uint64_t lof_col_flag(Ld ld, const float* thr, int nlf) {
+  constexpr int KMAX = lof_ilog2c(C);
+  float u[C];
+  __half2 e2[C / 2];
+  uint64_t fb = 0;
+  const float T0 = thr[0];
+  int k_next = 1;
+  bool again = true;
+#pragma unroll 1
+  while (again) {
+    // level 0 under the current mask: I = 1 is the simple thresholder x > threshold_1
+    float m0 = -INFINITY, m1 = -INFINITY;
+#pragma unroll
+    for (int c = 0; c < C; c += 2) {
+      u[c] = ld(c); u[c + 1] = ld(c + 1);
+      m0 = fmaxf(m0, u[c]); m1 = fmaxf(m1, u[c + 1]);
+      e2[c / 2] = lof_h2_bits(LOF_H2_ONES);
+    }
+    if (fb != 0 || fmaxf(m0, m1) > T0) {
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+        if (((fb >> c) & 1ull) || u[c] > T0) { fb |= 1ull << c; u[c] = 0.f; }
+#pragma unroll
+      for (int m = 0; m < C / 2; ++m) e2[m] = lof_h2_unflagged((uint32_t)(fb >> (2 * m)) & 3u);
+    }
+    again = false;
+#define LOF_COL_LEVEL(K)                                                             \
+    if (K <= KMAX && K < nlf && !again) {                                            \
+      lof_col_step<C, (K <= KMAX ? K : 1)>(u, e2);                                   \
+      if (K >= k_next && lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e2, thr[K], fb) &&  \
+          K + 1 <= KMAX && K + 1 < nlf) { again = true; k_next = K + 1; }            \
+    }
+    LOF_COL_LEVEL(1) LOF_COL_LEVEL(2) LOF_COL_LEVEL(3) LOF_COL_LEVEL(4)
+    LOF_COL_LEVEL(5) LOF_COL_LEVEL(6) LOF_COL_LEVEL(7) LOF_COL_LEVEL(8)
+#undef LOF_COL_LEVEL
+  }
+  return fb;
+}
+
+// A warp's 32 column masks -> one word per channel (lane c & 31 ends up holding channel c's word).
+template <int C>
+__device__ __forceinline__ void lof_col_words(uint64_t fb, int lane, uint32_t& mine0, uint32_t& mine1) {
+  mine0 = 0; mine1 = 0;
+  if (__any_sync(0xffffffffu, fb != 0)) {
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+      const uint32_t word = __ballot_sync(0xffffffffu, (fb >> c) & 1ull);
+      if ((c & 31) == lane) { if (c < 32) mine0 = word; else mine1 = word; }
+    }
+  }
+}
+
 template <int C, int L>
 __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
   using Cfg = LofFusedCfg<C, L>;
-  constexpr int T = Cfg::T, NT = Cfg::NT, W = Cfg::W, KMAX = lof_ilog2c(C);
+  constexpr int T = Cfg::T, W = Cfg::W;
   const int lane = threadIdx.x & 31;
-  const int nlf = (int)n_lev_f;
-  (void)NT;
 #pragma unroll 1
   for (;;) {
     // groups of 32 columns are handed out dynamically (restarts make their cost uneven)
@@ -380,50 +433,11 @@ __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
     if (g >= T / 32) break;
     const int col = g * 32 + lane;
     const float* cp = sm.xs + lof_swz_elem(col);
-    float u[C];
-    __half2 e2[C / 2];
-    uint64_t fb = 0;
-    const float T0 = sm.thr[0];
-    int k_next = 1;
-    bool again = true;
-#pragma unroll 1
-    while (again) {
-      // level 0 under the current mask: I = 1 is the simple thresholder x > threshold_1
-      float m0 = -INFINITY, m1 = -INFINITY;
-#pragma unroll
-      for (int c = 0; c < C; c += 2) {
-        u[c] = cp[c * T]; u[c + 1] = cp[(c + 1) * T];
-        m0 = fmaxf(m0, u[c]); m1 = fmaxf(m1, u[c + 1]);
-        e2[c / 2] = lof_h2_bits(LOF_H2_ONES);
-      }
-      if (fb != 0 || fmaxf(m0, m1) > T0) {
-#pragma unroll
-        for (int c = 0; c < C; ++c)
-          if (((fb >> c) & 1ull) || u[c] > T0) { fb |= 1ull << c; u[c] = 0.f; }
-#pragma unroll
-        for (int m = 0; m < C / 2; ++m) e2[m] = lof_h2_unflagged((uint32_t)(fb >> (2 * m)) & 3u);
-      }
-      again = false;
-#define LOF_COL_LEVEL(K)                                                               \
-      if (K <= KMAX && K < nlf && !again) {                                            \
-        lof_col_step<C, (K <= KMAX ? K : 1)>(u, e2);                                   \
-        if (K >= k_next && lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e2, sm.thr[K], fb) && \
-            K + 1 <= KMAX && K + 1 < nlf) { again = true; k_next = K + 1; }            \
-      }
-      LOF_COL_LEVEL(1) LOF_COL_LEVEL(2) LOF_COL_LEVEL(3) LOF_COL_LEVEL(4)
-      LOF_COL_LEVEL(5) LOF_COL_LEVEL(6) LOF_COL_LEVEL(7) LOF_COL_LEVEL(8)
-#undef LOF_COL_LEVEL
-    }
+    const uint64_t fb = lof_col_flag<C>([cp](int c) { return cp[c * T]; }, sm.thr, (int)n_lev_f);
     // this warp's 32 columns -> one mask word per channel
     const int w = col >> 5;
-    uint32_t mine0 = 0, mine1 = 0;
-    if (__any_sync(0xffffffffu, fb != 0)) {
-#pragma unroll
-      for (int c = 0; c < C; ++c) {
-        const uint32_t word = __ballot_sync(0xffffffffu, (fb >> c) & 1ull);
-        if ((c & 31) == lane) { if (c < 32) mine0 = word; else mine1 = word; }
-      }
-    }
+    uint32_t mine0, mine1;
+    lof_col_words<C>(fb, lane, mine0, mine1);
     if (lane < C) sm.fm[lane * W + w] = mine0;
     if (C > 32 && lane + 32 < C) sm.fm[(lane + 32) * W + w] = mine1;
   }
@@ -505,6 +519,45 @@ __device__ __forceinline__ bool lof_row_eval(const float (&u)[L], const __half2 
   return __any_sync(0xffffffffu, changed);
 }
 
+// The time run of one row segment held by a warp (lane l: samples [l*L, l*L+L) in x[]): level 0, then the
+// doubling levels with restarts.  fb enters as the mask so far and leaves as the final mask.  `after_level0`
+// is called once, right after the first level 0 has consumed every x[j].  Warp-uniform control flow.
+template <int L, class Hook>
+__device__ __forceinline__ void lof_row_flag(const float (&x)[L], uint32_t& fb, const float* thr, int nlt, int lane,
+                                             Hook after_level0) {
+  const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
+  float u[L];
+  __half2 e2[L / 2];
+  const float T0 = thr[0];
+  int k_next = 1;
+  bool again = true;
+#pragma unroll 1
+  while (again) {
+    // level 0 (I = 1) under the current mask: x > threshold_1 on samples not yet flagged
+#pragma unroll
+    for (int j = 0; j < L; ++j) {
+      const bool f = ((fb >> j) & 1u) || (x[j] > T0);
+      fb |= f ? (1u << j) : 0u;
+      u[j] = f ? 0.f : x[j];
+    }
+#pragma unroll
+    for (int m = 0; m < L / 2; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
+    again = false;
+    if (k_next == 1) after_level0();
+    if (__all_sync(0xffffffffu, fb == maskL)) break;     // nothing left to test in this row
+#define LOF_ROW_LEVEL(K)                                                                 \
+    if (K < nlt && !again) {                                                             \
+      lof_row_step<L, (1 << (K - 1))>(u, e2, lane);                                      \
+      if (K >= k_next && lof_row_eval<L, K>(u, e2, lane, thr[K], fb) && K + 1 < nlt) {   \
+        again = true; k_next = K + 1;                                                    \
+      }                                                                                  \
+    }
+    LOF_ROW_LEVEL(1) LOF_ROW_LEVEL(2) LOF_ROW_LEVEL(3) LOF_ROW_LEVEL(4) LOF_ROW_LEVEL(5)
+    LOF_ROW_LEVEL(6) LOF_ROW_LEVEL(7) LOF_ROW_LEVEL(8) LOF_ROW_LEVEL(9)
+#undef LOF_ROW_LEVEL
+  }
+}
+
 template <int C, int L>
 __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, uint32_t s, bool have_f,
                                uint32_t* __restrict__ flags, double* __restrict__ rowsum,
@@ -523,8 +576,7 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
     if (lane == 0) c = (int)atomicAdd(&sm.ctl[CT_ROW], 1u);
     c = __shfl_sync(0xffffffffu, c, 0);
     if (c >= C) break;
-    float x[L], u[L];
-    __half2 e2[L / 2];
+    float x[L];
     const float4* rp = reinterpret_cast<const float4*>(sm.xs + c * T);
 #pragma unroll
     for (int q = 0; q < L / 4; ++q) {
@@ -537,48 +589,17 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
       const uint32_t lo = sm.fm[c * W + q], hi = (q + 1 < W) ? sm.fm[c * W + q + 1] : 0u;
       fb = __funnelshift_r(lo, hi, r) & maskL;
     }
-    if (nlt > 0) {
-      const float T0 = sm.thr[0];
-      int k_next = 1;
-      bool again = true;
-#pragma unroll 1
-      while (again) {
-        // level 0 (I = 1) under the current mask: x > threshold_1 on samples not yet flagged
+    // as soon as level 0 has moved the row into registers its shared-memory slot takes the next stream's row
+    auto prefetch_row = [&]() {
+      if (next_stream) {
+        float4* dst = reinterpret_cast<float4*>(sm.xs + c * T);
+        const float4* src = reinterpret_cast<const float4*>(next_stream + c * T);
 #pragma unroll
-        for (int j = 0; j < L; ++j) {
-          const bool f = ((fb >> j) & 1u) || (x[j] > T0);
-          fb |= f ? (1u << j) : 0u;
-          u[j] = f ? 0.f : x[j];
-        }
-#pragma unroll
-        for (int m = 0; m < L / 2; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
-        again = false;
-        // the row lives in registers now (level 0 consumed every x[j]): its shared-memory slot can
-        // already take the next stream's row
-        if (next_stream && k_next == 1) {
-          float4* dst = reinterpret_cast<float4*>(sm.xs + c * T);
-          const float4* src = reinterpret_cast<const float4*>(next_stream + c * T);
-#pragma unroll
-          for (int q = 0; q < L / 4; ++q) lof_cp_async16(dst + lof_swz_chunk(q * 32 + lane), src + q * 32 + lane);
-        }
-        if (__all_sync(0xffffffffu, fb == maskL)) break;   // nothing left to test in this row
-#define LOF_ROW_LEVEL(K)                                                                   \
-        if (K < (int)nlt && !again) {                                                      \
-          lof_row_step<L, (1 << (K - 1))>(u, e2, lane);                                     \
-          if (K >= k_next && lof_row_eval<L, K>(u, e2, lane, sm.thr[K], fb) && K + 1 < (int)nlt) { \
-            again = true; k_next = K + 1;                                                  \
-          }                                                                                \
-        }
-        LOF_ROW_LEVEL(1) LOF_ROW_LEVEL(2) LOF_ROW_LEVEL(3) LOF_ROW_LEVEL(4) LOF_ROW_LEVEL(5)
-        LOF_ROW_LEVEL(6) LOF_ROW_LEVEL(7) LOF_ROW_LEVEL(8) LOF_ROW_LEVEL(9)
-#undef LOF_ROW_LEVEL
+        for (int q = 0; q < L / 4; ++q) lof_cp_async16(dst + lof_swz_chunk(q * 32 + lane), src + q * 32 + lane);
       }
-    } else if (next_stream) {
-      float4* dst = reinterpret_cast<float4*>(sm.xs + c * T);
-      const float4* src = reinterpret_cast<const float4*>(next_stream + c * T);
-#pragma unroll
-      for (int q = 0; q < L / 4; ++q) lof_cp_async16(dst + lof_swz_chunk(q * 32 + lane), src + q * 32 + lane);
-    }
+    };
+    if (nlt > 0) lof_row_flag<L>(x, fb, sm.thr, (int)nlt, lane, prefetch_row);
+    else prefetch_row();
     // bit-pack: word w of the row = bits [32w, 32w+32) gathered from the lanes' L-bit masks
     {
       const int q0 = (32 * lane) / L, r0 = 32 * lane - L * q0;

@@ -136,7 +136,8 @@ def test_config5_cut_with_history(lof, lofo, wl):
 
 @pytest.mark.parametrize("S,C,T,mw,dirs", [
     (3, 5, 77, 8, 3), (2, 1, 100, 16, 3), (2, 7, 1, 4, 3), (1, 3, 33, 64, 3), (2, 16, 256, 32, 1),
-    (2, 16, 256, 32, 2), (1, 64, 768, 1, 3), (2, 48, 1000, 1024, 3), (1, 256, 40, 256, 3), (1, 2, 9000, 128, 3)])
+    (2, 16, 256, 32, 2), (1, 64, 768, 1, 3), (2, 48, 1000, 1024, 3), (1, 256, 40, 256, 3), (1, 2, 9000, 128, 3),
+    (2, 16, 3000, 128, 3), (1, 32, 5003, 64, 3), (3, 64, 2100, 32, 3), (2, 16, 1025, 64, 2), (1, 32, 4096, 256, 3)])
 def test_ragged_shapes(lof, lofo, S, C, T, mw, dirs):
     rng = np.random.default_rng(S * 1000 + C * 10 + T)
     x = rng.standard_exponential((S, C, T)).astype(np.float32)
@@ -226,3 +227,10 @@ def test_bench_configuration_sampled_streams(lof, lofo, wl):
     pop = np.unpackbits(g.view(np.uint8), axis=-1).reshape(S, -1).sum(axis=1)
     assert np.array_equal(pop.astype(np.uint64), st["n_flagged"])
     f.close()
+
+
+def test_ci16_long_rows_register_kernels(lof, lofo, wl):
+    # complex int16 input through the register-resident long-row kernels (max_window 64: row segments with halo)
+    w = wl.config4(1, n_stations=1, T=7001)
+    res, _ = check(lof, lofo, None, w.S, 32, 7001, volt=w.volt, max_window=64)
+    print("cfg4-like, windows 1..64", res)
