@@ -160,7 +160,7 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   const uint64_t N = (uint64_t)C * T;
   c->n_chunks = (uint32_t)((N + LOF_STATS_CHUNK - 1) / LOF_STATS_CHUNK);
   // groups: keep one group's input (read four to five times by the generic path) inside L2
-  const uint64_t group_bytes = 48ull << 20;
+  const uint64_t group_bytes = 80ull << 20;
   uint64_t g = group_bytes / (N * 4);
   if (g < 1) g = 1;
   if (g > S) g = S;

@@ -108,17 +108,25 @@ lof_k_scan(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_t* 
   } else {
     rank = st.rank;
   }
-  // 2048 bins, 8 per thread
+  // 2048 bins, 8 per thread; warp 0 scans the 256 per-thread totals
   uint32_t loc[8], tot = 0;
 #pragma unroll
   for (int j = 0; j < 8; ++j) { loc[j] = gh[tid * 8 + j]; tot += loc[j]; }
   sh_cnt[tid] = tot;
   __syncthreads();
-  if (tid == 0) {
-    uint32_t acc = 0;
-    int t = 0;
-    for (; t < 255; ++t) { if (acc + sh_cnt[t] > rank) break; acc += sh_cnt[t]; }
-    sh_sel[0] = t; sh_sel[1] = acc;
+  if (tid < 32) {
+    uint32_t p[8], sum = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { p[j] = sh_cnt[tid * 8 + j]; sum += p[j]; }
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (tid >= o) inc += v; }
+    const uint32_t exc = inc - sum;
+    if ((rank >= exc && rank < inc) || (tid == 31 && rank >= inc)) {
+      uint32_t acc = exc; int j = 0;
+      for (; j < 7; ++j) { if (acc + p[j] > rank) break; acc += p[j]; }
+      sh_sel[0] = tid * 8 + j; sh_sel[1] = acc;
+    }
   }
   __syncthreads();
   if (tid == (int)sh_sel[0]) {
