@@ -37,6 +37,7 @@ struct lof_ctx {
   uint32_t TT, halo, n_tiles;     // time tiling
   bool lr_freq, lr_time;          // register-resident long-row kernels usable (lof_longrow.cuh)
   uint32_t seg_out, seg_halo, n_seg;
+  uint32_t co_out, n_co;          // cooperative 8192-sample tiles for wide cones
   size_t smem_freq, smem_time;
   // device memory owned by the context
   LofStreamState* d_state;
@@ -125,6 +126,8 @@ static cudaError_t lof_generic_set_attributes(size_t smem_freq, size_t smem_time
   A(cudaFuncSetAttribute(lof_k_freq_generic<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, f));
   A(cudaFuncSetAttribute(lof_k_time_generic<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, t));
   A(cudaFuncSetAttribute(lof_k_time_generic<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, t));
+  A(cudaFuncSetAttribute(lof_k_time_coop<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LofCoopSmem)));
+  A(cudaFuncSetAttribute(lof_k_time_coop<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LofCoopSmem)));
   return e;
 }
 
@@ -178,6 +181,8 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   c->lr_time = c->seg_halo <= 256;
   c->seg_out = c->lr_time ? LOF_LR_TILE - 2 * c->seg_halo : LOF_LR_TILE;
   c->n_seg = (T + c->seg_out - 1) / c->seg_out;
+  c->co_out = LOF_CO_TILE - 2 * c->seg_halo;             // seg_halo <= 2048 for max_window <= 1024
+  c->n_co = (T + c->co_out - 1) / c->co_out;
   c->smem_freq = (size_t)C * 32 * LOF_GEN_BYTES_PER_ELEM;
   c->smem_time = (size_t)((c->TT + 2 * c->halo + 31) & ~31u) * LOF_GEN_BYTES_PER_ELEM;
 
@@ -187,7 +192,8 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   A(dev_alloc(&c->d_hist, (size_t)c->group * LOF_HIST_BINS));
   A(dev_alloc(&c->d_partial, (size_t)c->group * c->n_chunks * 2));
   A(dev_alloc(&c->d_fmask, (size_t)S * C * W));
-  const size_t n_part = c->n_tiles > c->n_seg ? c->n_tiles : c->n_seg;
+  size_t n_part = c->n_tiles > c->n_seg ? c->n_tiles : c->n_seg;
+  if (c->n_co > n_part) n_part = c->n_co;
   A(dev_alloc(&c->d_part_sum, (size_t)c->group * C * n_part));
   A(dev_alloc(&c->d_part_cnt, (size_t)c->group * C * n_part));
   A(dev_alloc(&c->d_rowsum, (size_t)S * C));
@@ -244,6 +250,10 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
       const uint32_t nb_t = (uint32_t)(((uint64_t)rows * n_part + LOF_LR_WARPS - 1) / LOF_LR_WARPS);
       lof_k_time_seg<In><<<nb_t, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum,
                                                         c->d_part_cnt, c->d_stats, c->seg_out, c->seg_halo, n_part, rows);
+    } else if (fast) {
+      n_part = c->n_co;
+      lof_k_time_coop<In><<<rows * n_part, LOF_CO_WARPS * 32, sizeof(LofCoopSmem), st>>>(
+          in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum, c->d_part_cnt, c->d_stats, c->co_out, c->seg_halo, n_part);
     } else {
       n_part = c->n_tiles;
       lof_k_time_generic<In><<<rows * c->n_tiles, LOF_GEN_THREADS, c->smem_time, st>>>(

@@ -106,3 +106,207 @@ lof_k_time_seg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
     if (nf) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[s].n_flagged), (unsigned long long)nf);
   }
 }
+
+// ---- CTA-cooperative time run for wide cones (max_window >= 256): 8 warps share a tile of 8192 samples
+// (halo H on each side), each warp holding 1024 of them as in lof_k_time_seg.  Per iteration the warps
+// exchange only what crosses their borders, through shared memory: the first D window sums / counts of the
+// next warp (partners of the last lanes), and the last fired window start of the previous warps (dilation).
+#define LOF_CO_WARPS 8
+#define LOF_CO_TILE (LOF_CO_WARPS * LOF_LR_TILE)
+
+struct LofCoopSmem {
+  float stage[LOF_CO_WARPS][LOF_LR_TILE];               // load staging, one 1024-sample strip per warp
+  float bu[2][LOF_CO_WARPS][256];                       // published window sums (double-buffered by level)
+  uint32_t be[2][LOF_CO_WARPS][128];                    // published counts (packed halves)
+  int wmax[LOF_CO_WARPS];                               // last fired window start per warp
+};
+
+template <int D>
+__device__ __forceinline__ void lof_row_step_coop(float (&u)[32], __half2 (&e2)[16], int lane, const float* nb_u,
+                                                  const uint32_t* nb_e, bool has_nb) {
+  if constexpr (D == 1) {
+    float pu = __shfl_down_sync(0xffffffffu, u[0], 1);
+    uint32_t pe = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[0]), 1);
+    if (lane == 31) { pu = has_nb ? nb_u[0] : -INFINITY; pe = has_nb ? nb_e[0] : 0u; }
+#pragma unroll
+    for (int j = 0; j < 32; ++j) u[j] += (j + 1 < 32) ? u[j + 1] : pu;
+#pragma unroll
+    for (int m = 0; m < 16; ++m)
+      e2[m] = __hadd2(e2[m], lof_h2_shift1(e2[m], (m + 1 < 16) ? e2[m + 1] : lof_h2_bits(pe)));
+  } else {
+    constexpr int NP = D < 32 ? D : 32;
+    float pu[NP];
+    uint32_t pe[NP / 2];
+#pragma unroll
+    for (int jj = 0; jj < NP; ++jj) {
+      const int j = 32 - NP + jj, src = (j + D) % 32, off = (j + D) / 32;
+      pu[jj] = __shfl_down_sync(0xffffffffu, u[src], off);
+      if ((jj & 1) == 0) pe[jj / 2] = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[src / 2]), off);
+      if (lane + off > 31) {                            // the partner lives in the next warp's strip
+        const int p = (lane + off - 32) * 32 + src;     // its position there, < D
+        pu[jj] = has_nb ? nb_u[p] : -INFINITY;
+        if ((jj & 1) == 0) pe[jj / 2] = has_nb ? nb_e[p >> 1] : 0u;
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 32; ++j) u[j] += (j + D < 32) ? u[j + D] : pu[j - (32 - NP)];
+#pragma unroll
+    for (int m = 0; m < 16; ++m)
+      e2[m] = __hadd2(e2[m], (2 * m + D < 32) ? e2[m + D / 2] : lof_h2_bits(pe[(2 * m - (32 - NP)) / 2]));
+  }
+}
+
+// Test of iteration I = 2^K on a strip; like lof_row_eval, but windows fired in previous warps' strips dilate
+// into this one (carry through wmax[]), and "any" is taken over the CTA.  Contains __syncthreads: CTA-uniform.
+template <int K>
+__device__ __forceinline__ bool lof_row_eval_coop(const float (&u)[32], const __half2 (&e2)[16], int lane, int warp,
+                                                  float thr, uint32_t& fb, int* wmax) {
+  constexpr int I = 1 << K;
+  const float negT = -thr;
+  float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+  for (int m = 0; m < 16; ++m) {
+    const float2 ef = __half22float2(e2[m]);
+    tm[(2 * m) & 3] = fmaxf(tm[(2 * m) & 3], fmaf(ef.x, negT, u[2 * m]));
+    tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], fmaf(ef.y, negT, u[2 * m + 1]));
+  }
+  if (!__syncthreads_or(fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f)) return false;
+  uint32_t trig = 0;
+#pragma unroll
+  for (int m = 0; m < 16; ++m) {
+    const float2 ef = __half22float2(e2[m]);
+    trig |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
+    trig |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
+  }
+  uint32_t own = trig;
+#pragma unroll
+  for (int s = 1; s < I && s < 32; s <<= 1) own |= own << s;
+  const int pos0 = warp * LOF_LR_TILE + lane * 32;        // tile coordinate of this lane's first sample
+  int pm = trig ? (pos0 + 31 - __clz(trig)) : -(1 << 20);
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pm, o); if (lane >= o) pm = max(pm, v); }
+  if (lane == 31) wmax[warp] = pm;
+  __syncthreads();
+  int prev = __shfl_up_sync(0xffffffffu, pm, 1);
+  if (lane == 0) prev = -(1 << 20);
+  for (int w = 0; w < warp; ++w) prev = max(prev, wmax[w]);
+  int cnt = prev + I - pos0;
+  cnt = cnt < 0 ? 0 : (cnt > 32 ? 32 : cnt);
+  const uint32_t pre = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
+  const uint32_t nf = fb | own | pre;
+  const bool changed = nf != fb;
+  fb = nf;
+  return __syncthreads_or(changed) != 0;
+}
+
+// grid.x = n_rows * n_tile; a CTA of 8 warps covers [t_lo, t_lo + 8192) of one row and writes the words of
+// its OUT = 8192 - 2H central samples.  All control flow around barriers is CTA-uniform.
+template <class In>
+__global__ void __launch_bounds__(LOF_CO_WARPS * 32, 2)
+lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state, const uint32_t* __restrict__ fmask,
+                uint32_t* __restrict__ flags, double* __restrict__ part_sum, uint32_t* __restrict__ part_cnt,
+                lof_stream_stats* __restrict__ stats, uint32_t OUT, uint32_t H, uint32_t n_tile) {
+  extern __shared__ __align__(16) unsigned char co_raw[];
+  LofCoopSmem& sm = *reinterpret_cast<LofCoopSmem*>(co_raw);
+  __shared__ double red_sum[LOF_CO_WARPS];
+  __shared__ uint32_t red_cnt[2][LOF_CO_WARPS];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t rl = blockIdx.x / n_tile, tile = blockIdx.x - rl * n_tile;
+  const uint32_t W = prm.W, C = prm.C, T = prm.T;
+  const uint64_t row = (uint64_t)prm.s0 * C + rl;
+  const uint32_t s = (uint32_t)(row / C);
+  const LofStreamState& st = state[s];
+  const uint32_t o_lo = tile * OUT, o_hi = min(T, o_lo + OUT);
+  const uint32_t t_lo = (o_lo >= H ? o_lo - H : 0) + warp * LOF_LR_TILE;   // this warp's strip
+  float* sg = sm.stage[warp];
+  const uint64_t base = row * T;
+#pragma unroll 4
+  for (int q = 0; q < LOF_LR_TILE / 32; ++q) {
+    const int i = q * 32 + lane;
+    const uint32_t t = t_lo + i;
+    sg[lof_lr_swz(i)] = t < T ? in.ld(base + t) : -INFINITY;
+  }
+  __syncwarp();
+  float x[32];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    const float4 v = reinterpret_cast<const float4*>(sg)[(8 * lane + q) ^ (lane & 7)];
+    x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
+  }
+  const uint32_t t_w = t_lo + 32 * lane;
+  const uint32_t valid = t_w >= T ? 0u : (T - t_w >= 32 ? 0xFFFFFFFFu : ((1u << (T - t_w)) - 1u));
+  uint32_t fb = 0;
+  if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];
+  const int nlt = (int)prm.n_lev_t;
+  if (st.nonfinite) fb = valid;
+  else if (nlt > 0) {
+    const float* thr = st.thr_f;
+    const float T0 = thr[0];
+    float u[32];
+    __half2 e2[16];
+    int k_next = 1;
+    bool again = true;
+    const bool has_nb = warp + 1 < LOF_CO_WARPS;
+#pragma unroll 1
+    while (again) {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) {
+        const bool f = ((fb >> j) & 1u) || (x[j] > T0);
+        fb |= f ? (1u << j) : 0u;
+        u[j] = f ? 0.f : x[j];
+      }
+#pragma unroll
+      for (int m = 0; m < 16; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
+      again = false;
+#define LOF_CO_LEVEL(K)                                                                          \
+      if (K < nlt && !again) {                                                                   \
+        constexpr int D = 1 << (K - 1);                                                          \
+        float* pbu = sm.bu[K & 1][warp]; uint32_t* pbe = sm.be[K & 1][warp];                     \
+        /* publish the first D sums / counts of this strip for the previous warp */             \
+        if (lane * 32 < D) {                                                                     \
+          _Pragma("unroll") for (int j = 0; j < 32; ++j) if (lane * 32 + j < D) pbu[lane * 32 + j] = u[j];        \
+          _Pragma("unroll") for (int m = 0; m < 16; ++m) if (lane * 32 + 2 * m < D) pbe[lane * 16 + m] = lof_bits_h2(e2[m]); \
+        }                                                                                        \
+        __syncthreads();                                                                         \
+        lof_row_step_coop<D>(u, e2, lane, sm.bu[K & 1][has_nb ? warp + 1 : warp],                \
+                             sm.be[K & 1][has_nb ? warp + 1 : warp], has_nb);                    \
+        if (K >= k_next && lof_row_eval_coop<K>(u, e2, lane, warp, thr[K], fb, sm.wmax) && K + 1 < nlt) { \
+          again = true; k_next = K + 1;                                                          \
+        }                                                                                        \
+      }
+      LOF_CO_LEVEL(1) LOF_CO_LEVEL(2) LOF_CO_LEVEL(3) LOF_CO_LEVEL(4) LOF_CO_LEVEL(5)
+      LOF_CO_LEVEL(6) LOF_CO_LEVEL(7) LOF_CO_LEVEL(8) LOF_CO_LEVEL(9)
+#undef LOF_CO_LEVEL
+      __syncthreads();                                    // a restart republishes into the same buffers
+    }
+  }
+  fb &= valid;
+  const bool mine = t_w >= o_lo && t_w < o_hi;
+  if (mine) flags[row * W + (t_w >> 5)] = fb;
+  float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
+  const uint32_t skip = fb | ~valid;
+#pragma unroll
+  for (int j = 0; j < 32; j += 4) {
+    p0 += ((skip >> j) & 1u) ? 0.f : x[j];
+    p1 += ((skip >> (j + 1)) & 1u) ? 0.f : x[j + 1];
+    p2 += ((skip >> (j + 2)) & 1u) ? 0.f : x[j + 2];
+    p3 += ((skip >> (j + 3)) & 1u) ? 0.f : x[j + 3];
+  }
+  double rs = mine ? (double)((p0 + p1) + (p2 + p3)) : 0.0;
+  rs = lof_warp_sum(rs);
+  uint32_t nf = mine ? __popc(fb) : 0u, nu = mine ? __popc(valid & ~fb) : 0u;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    nf += __shfl_down_sync(0xffffffffu, nf, o);
+    nu += __shfl_down_sync(0xffffffffu, nu, o);
+  }
+  if (lane == 0) { red_sum[warp] = rs; red_cnt[0][warp] = nu; red_cnt[1][warp] = nf; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0.0; uint32_t cu = 0, cf = 0;
+    for (int w = 0; w < LOF_CO_WARPS; ++w) { a += red_sum[w]; cu += red_cnt[0][w]; cf += red_cnt[1][w]; }
+    part_sum[(uint64_t)rl * n_tile + tile] = a;
+    part_cnt[(uint64_t)rl * n_tile + tile] = cu;
+    if (cf) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[s].n_flagged), (unsigned long long)cf);
+  }
+}
