@@ -91,12 +91,17 @@ lof_k_scan(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_t* 
   uint32_t rank;
   if (PASS == 0) {
     rank = (uint32_t)(N / 2);                           // rank floor(N/2), 0-based (S3)
+    // chunk partials reduced in a fixed order: each thread a contiguous run of chunks, then a fixed tree
+    __shared__ double sh_red2[32];
+    const uint32_t per = (n_chunks + 255) / 256;
+    double a = 0.0, q = 0.0;
+    for (uint32_t c = tid * per; c < min(n_chunks, (tid + 1) * per); ++c) {
+      a += partial[((size_t)sl * n_chunks + c) * 2 + 0];
+      q += partial[((size_t)sl * n_chunks + c) * 2 + 1];
+    }
+    a = lof_block_sum(a, sh_red2);
+    q = lof_block_sum(q, sh_red2);
     if (tid == 0) {
-      double a = 0.0, q = 0.0;
-      for (uint32_t c = 0; c < n_chunks; ++c) {
-        a += partial[((size_t)sl * n_chunks + c) * 2 + 0];
-        q += partial[((size_t)sl * n_chunks + c) * 2 + 1];
-      }
       const double K = (double)in.ld((uint64_t)s * N);
       const double n = (double)N;
       double var = (q - a * a / n) / n;
