@@ -61,17 +61,17 @@ struct LofFusedSmem {
 // ctl slots
 enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS, CT_NFLAG, CT_BAD, CT_SELP, CT_SELACC, CT_PREFIX, CT_RANK, CT_FOUND };
 
-// Find the bin holding `rank` in hist[NB] (NB a multiple of 256, blockDim >= 256).
+// Find the bin holding `rank` in hist[NB] (NB a multiple of 256, any blockDim >= 32).
 // Results in ctl[CT_BIN] (bin) and ctl[CT_BEFORE] (number of entries in lower bins).
 template <int NB>
 __device__ void lof_find_bin(const uint32_t* hist, uint32_t rank, uint32_t* part /*256*/, uint32_t* ctl) {
   constexpr int PER = NB / 256;
   const int tid = threadIdx.x, lane = tid & 31;
-  uint32_t loc[PER], tot = 0;
-  if (tid < 256) {
+  for (int p = tid; p < 256; p += blockDim.x) {
+    uint32_t tot = 0;
 #pragma unroll
-    for (int j = 0; j < PER; ++j) { loc[j] = hist[tid * PER + j]; tot += loc[j]; }
-    part[tid] = tot;
+    for (int j = 0; j < PER; ++j) tot += hist[p * PER + j];
+    part[p] = tot;
   }
   __syncthreads();
   if (tid < 32) {
@@ -86,14 +86,12 @@ __device__ void lof_find_bin(const uint32_t* hist, uint32_t rank, uint32_t* part
     if (mine) {
       uint32_t acc = exc; int j = 0;
       for (; j < 7; ++j) { if (acc + p[j] > rank) break; acc += p[j]; }
-      ctl[CT_SELP] = lane * 8 + j; ctl[CT_SELACC] = acc;
+      // within the selected group of PER bins
+      const int g = lane * 8 + j;
+      int b = 0;
+      for (; b < PER - 1; ++b) { const uint32_t hv = hist[g * PER + b]; if (acc + hv > rank) break; acc += hv; }
+      ctl[CT_BIN] = g * PER + b; ctl[CT_BEFORE] = acc;
     }
-  }
-  __syncthreads();
-  if (tid == (int)ctl[CT_SELP]) {
-    uint32_t acc = ctl[CT_SELACC]; int j = 0;
-    for (; j < PER - 1; ++j) { if (acc + loc[j] > rank) break; acc += loc[j]; }
-    ctl[CT_BIN] = tid * PER + j; ctl[CT_BEFORE] = acc;
   }
   __syncthreads();
 }
