@@ -137,6 +137,20 @@ uint64_t lof_launch_count(const lof_ctx* ctx);
  * generic multi-kernel path.  Both compute the same results; for tests and profiling. */
 int lof_set_path(lof_ctx* ctx, int path);
 
+/* Diagnostics of the fused kernels (streams that fit one SM's shared memory): how the exact median
+ * of each stream was found since the last reset, summed over every context of the process on the
+ * context's device: h_out[0] from samples gathered during the statistics pass (the fast case),
+ * h_out[1] by one more gather pass, h_out[2] by a radix select over the whole stream, h_out[3]
+ * streams with non-finite samples.  Synchronises the device.  reset != 0 zeroes the counters. */
+int lof_fused_counters(lof_ctx* ctx, uint64_t* h_out /*[4]*/, int reset);
+
+/* Profiling builds only (nvcc -DLOF_FUSED_PROF, see build.py LOF_NVCC_EXTRA): SM cycles thread 0 of
+ * every CTA spent per phase of the fused kernel since the last lof_fused_counters(reset): h_out[0]
+ * first load + statistics, [1] frequency pass, [2] plan of the next stream, [3] time pass with
+ * the next stream's row statistics, [4] end of the next stream's statistics, [5..7] zero.
+ * All zero in a normal build.  Synchronises the device. */
+int lof_fused_cycles(lof_ctx* ctx, uint64_t* h_out /*[8]*/);
+
 const char* lof_strerror(int code);
 const char* lof_last_cuda_error(void);
 

@@ -29,7 +29,8 @@ def build_lib(force=False, verbose=False):
     if not force and os.path.exists(LIB) and all(os.path.getmtime(s) <= os.path.getmtime(LIB) for s in srcs):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    extra = os.environ.get("LOF_NVCC_EXTRA", "").split()      # e.g. -DLOF_FUSED_PROF for per-phase cycle counters
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", LIB, os.path.join(CSRC, "lof_api.cu")]
     subprocess.check_call(cmd)
     return LIB

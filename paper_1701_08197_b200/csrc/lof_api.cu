@@ -415,6 +415,31 @@ extern "C" int lof_flag_block_host(lof_ctx* c, const void* h_input, int is_ci16,
 
 extern "C" uint64_t lof_launch_count(const lof_ctx* c) { return c ? c->launches : 0; }
 
+extern "C" int lof_fused_counters(lof_ctx* c, uint64_t* h_out, int reset) {
+  if (!c || !h_out) return LOF_E_NULL;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  LOF_CUDA(cudaDeviceSynchronize());
+  unsigned long long v[4] = {0, 0, 0, 0};
+  LOF_CUDA(cudaMemcpyFromSymbol(v, lof_fused_counters_dev, sizeof v));
+  for (int i = 0; i < 4; ++i) h_out[i] = v[i];
+  if (reset) {
+    const unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    LOF_CUDA(cudaMemcpyToSymbol(lof_fused_counters_dev, z, 4 * sizeof z[0]));
+    LOF_CUDA(cudaMemcpyToSymbol(lof_fused_cycles_dev, z, sizeof z));
+  }
+  return LOF_OK;
+}
+
+extern "C" int lof_fused_cycles(lof_ctx* c, uint64_t* h_out) {
+  if (!c || !h_out) return LOF_E_NULL;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  LOF_CUDA(cudaDeviceSynchronize());
+  unsigned long long v[8];
+  LOF_CUDA(cudaMemcpyFromSymbol(v, lof_fused_cycles_dev, sizeof v));
+  for (int i = 0; i < 8; ++i) h_out[i] = v[i];
+  return LOF_OK;
+}
+
 extern "C" int lof_set_path(lof_ctx* c, int path) {
   if (!c) return LOF_E_NULL;
   if (path < 0 || path > 1) return LOF_E_PARAM;

@@ -22,7 +22,7 @@
 
 #include "lof_common.cuh"
 
-#define LOF_F_NBINS 2048
+#define LOF_F_NBINS 4096
 #define LOF_F_CAP 1024
 #define LOF_F_MAGIC 12582912.0f   // 1.5 * 2^23: adding it leaves round-to-nearest(x) in the low mantissa bits
 
@@ -37,12 +37,21 @@ struct LofFusedCfg {
   static constexpr int NT = (C >= 64) ? 384 : 256;
 #endif
   static constexpr int MINB = (C >= 64) ? 1 : 2;
+  // the next stream's statistics pass runs inside the time pass when the SM holds a single CTA; with two
+  // CTAs per SM their phases interleave anyway and the plain order measured faster
+#ifdef LOF_STAT_OVERLAP
+  static constexpr bool OVL = LOF_STAT_OVERLAP != 0;
+#else
+  static constexpr bool OVL = MINB == 1;
+#endif
   static constexpr size_t smem_bytes =
-      (size_t)N * 4 + (size_t)C * W * 4 + 2048 * 4 + LOF_F_CAP * 4 + 64 * 8 + 64 * 4 + 256 * 4;
+      (size_t)N * 4 + (size_t)C * W * 4 + LOF_F_NBINS * 4 + LOF_F_CAP * 4 + 64 * 8 + (size_t)3 * C * 8 +
+      64 * 4 + 256 * 4;
 };
 
 struct LofFusedSmem {
-  float* xs; uint32_t* fm; uint32_t* hist; float* cand; double* red; float* thr; uint32_t* ctl; uint32_t* part;
+  float* xs; uint32_t* fm; uint32_t* hist; float* cand; double* red; double* rowpart; unsigned long long* rowbar; float* thr;
+  uint32_t* ctl; uint32_t* part;
   template <int C, int L>
   __device__ static LofFusedSmem make(unsigned char* base) {
     LofFusedSmem s;
@@ -50,48 +59,71 @@ struct LofFusedSmem {
     s.xs = reinterpret_cast<float*>(base);
     s.fm = reinterpret_cast<uint32_t*>(s.xs + N);
     s.hist = s.fm + C * L;
-    s.cand = reinterpret_cast<float*>(s.hist + 2048);
+    s.cand = reinterpret_cast<float*>(s.hist + LOF_F_NBINS);
     s.red = reinterpret_cast<double*>(s.cand + LOF_F_CAP);
-    s.thr = reinterpret_cast<float*>(s.red + 64);
+    s.rowpart = s.red + 64;
+    s.rowbar = reinterpret_cast<unsigned long long*>(s.rowpart + 2 * C);
+    s.thr = reinterpret_cast<float*>(s.rowbar + C);
     s.ctl = reinterpret_cast<uint32_t*>(s.thr + 16);
     s.part = s.ctl + 48;
     return s;
   }
 };
 // ctl slots
-enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS, CT_NFLAG, CT_BAD, CT_SELP, CT_SELACC, CT_PREFIX, CT_RANK, CT_FOUND };
+enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS, CT_NFLAG, CT_BAD, CT_SELP, CT_SELACC, CT_PREFIX, CT_RANK, CT_FOUND, CT_SROW = 13 };
 
-// Find the bin holding `rank` in hist[NB] (NB a multiple of 256, any blockDim >= 32).
-// Results in ctl[CT_BIN] (bin) and ctl[CT_BEFORE] (number of entries in lower bins).
+// how the median of each stream was found: [0] rank count among the samples of the median's bin, [1] radix
+// select among them (a crowded bin), [2] radix select over the whole stream, [3] stream with non-finite samples
+// (diagnostics, lof_fused_counters)
+__device__ unsigned long long lof_fused_counters_dev[4];
+// cycles of thread 0 per phase, summed over CTAs and streams, when built with -DLOF_FUSED_PROF (bench/profiling
+// only): [0] first load + statistics, [1] frequency pass, [2] plan of the next stream, [3] time pass with
+// the next stream's row statistics, [4] end of the next stream's statistics
+__device__ unsigned long long lof_fused_cycles_dev[8];
+#ifdef LOF_FUSED_PROF
+#define LOF_PROF_T(var) const long long var = clock64()
+#define LOF_PROF_ADD(i, a, b) do { if (threadIdx.x == 0) atomicAdd(&lof_fused_cycles_dev[i], (unsigned long long)((b) - (a))); } while (0)
+#else
+#define LOF_PROF_T(var)
+#define LOF_PROF_ADD(i, a, b)
+#endif
+
+// Find the bin holding `rank` in hist[NB] (NB a multiple of 1024, any blockDim that is a multiple of 32).
+// Results in ctl[CT_BIN] (bin) and ctl[CT_BEFORE] (number of entries in lower bins); rank beyond the total
+// gives the last bin.  Groups of 32 bins are summed by warps (one bin per lane: no bank conflicts), warp 0
+// scans the group sums and then the 32 bins of the group it lands in.
 template <int NB>
-__device__ void lof_find_bin(const uint32_t* hist, uint32_t rank, uint32_t* part /*256*/, uint32_t* ctl) {
-  constexpr int PER = NB / 256;
-  const int tid = threadIdx.x, lane = tid & 31;
-  for (int p = tid; p < 256; p += blockDim.x) {
-    uint32_t tot = 0;
-#pragma unroll
-    for (int j = 0; j < PER; ++j) tot += hist[p * PER + j];
-    part[p] = tot;
+__device__ void lof_find_bin(const uint32_t* hist, uint32_t rank, uint32_t* part /*>= NB/32*/, uint32_t* ctl) {
+  constexpr int NG = NB / 32, PERL = NG / 32;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, nw = blockDim.x >> 5;
+  for (int g = w; g < NG; g += nw) {
+    const uint32_t s = __reduce_add_sync(0xffffffffu, hist[g * 32 + lane]);
+    if (lane == 0) part[g] = s;
   }
   __syncthreads();
   if (tid < 32) {
-    uint32_t p[8], s = 0;
+    uint32_t p[PERL], s = 0;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) { p[j] = part[lane * 8 + j]; s += p[j]; }
+    for (int j = 0; j < PERL; ++j) { p[j] = part[lane * PERL + j]; s += p[j]; }
     uint32_t inc = s;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
     const uint32_t exc = inc - s;
     const bool mine = (rank >= exc && rank < inc) || (lane == 31 && rank >= inc);
-    if (mine) {
-      uint32_t acc = exc; int j = 0;
-      for (; j < 7; ++j) { if (acc + p[j] > rank) break; acc += p[j]; }
-      // within the selected group of PER bins
-      const int g = lane * 8 + j;
-      int b = 0;
-      for (; b < PER - 1; ++b) { const uint32_t hv = hist[g * PER + b]; if (acc + hv > rank) break; acc += hv; }
-      ctl[CT_BIN] = g * PER + b; ctl[CT_BEFORE] = acc;
-    }
+    uint32_t acc = exc; int j = 0;
+#pragma unroll
+    for (int jj = 0; jj < PERL - 1; ++jj) { if (j == jj && acc + p[jj] <= rank) { acc += p[jj]; j = jj + 1; } }
+    const int src = __ffs(__ballot_sync(0xffffffffu, mine)) - 1;
+    const int g = __shfl_sync(0xffffffffu, lane * PERL + j, src);
+    acc = __shfl_sync(0xffffffffu, acc, src);
+    const uint32_t hv = hist[g * 32 + lane];
+    uint32_t binc = hv;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, binc, o); if (lane >= o) binc += v; }
+    const uint32_t hit = __ballot_sync(0xffffffffu, acc + binc > rank);
+    const int bl = hit ? __ffs(hit) - 1 : 31;
+    const uint32_t before = acc + __shfl_sync(0xffffffffu, binc - hv, bl);
+    if (lane == 0) { ctl[CT_BIN] = g * 32 + bl; ctl[CT_BEFORE] = before; }
   }
   __syncthreads();
 }
@@ -137,60 +169,110 @@ __device__ __forceinline__ void lof_block_sum2(double& a, double& b, double* red
   __syncthreads();
 }
 
-// Statistics of the stream in xs[0..N): mean, stddev (population), exact median of
-// rank floor(N/2), thresholds.  Writes sm.thr[], the stats record, and returns the number of
-// non-finite samples (then everything else is unspecified, S6).
+// ---- S: statistics, organised by channel row so that the pass over a row can run
+// anywhere: for the first stream of a CTA right after the load, for every later stream inside the time
+// pass of the stream before it, on rows whose prefetch has landed.
+//
+// LofStatPlan places the value histogram of one stream; every thread holds the same values.
+struct LofStatPlan {
+  float K, scale, off;     // K: centre of the shifted sums; bin(x) = round(clamp(x*scale + off)) in [0, LOF_F_NBINS)
+};
+
+__device__ __forceinline__ uint32_t lof_stat_bin(float x, float scale, float off) {
+  float yb = fmaf(x, scale, off);
+  yb = fminf(fmaxf(yb, 0.f), (float)(LOF_F_NBINS - 1) + 0.4f);
+  return __float_as_uint(yb + LOF_F_MAGIC) & (uint32_t)(LOF_F_NBINS - 1);
+}
+
+// Plan from one strided sample per thread: each warp sorts its 32 samples (bitonic, shuffles) and reads off
+// their median and interquartile range; the plan centres the histogram on the mean of the warp medians with
+// a half-width of 2.5 mean interquartile ranges.  Rank statistics, because RFI of 100 sigma in a few per cent
+// of the samples inflates a plain standard deviation tenfold and the bins with it.  Any K and any range give
+// the same exact results; they only decide how fast the median is found.  Contains __syncthreads.
+template <int NT>
+__device__ __forceinline__ LofStatPlan lof_stat_plan(float v, float* red /* >= 2*NT/32 floats */) {
+  constexpr int NW = NT / 32;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (!lof_finite(v)) v = 0.f;
+#pragma unroll
+  for (int k = 2; k <= 32; k <<= 1) {
+#pragma unroll
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      const float o = __shfl_xor_sync(0xffffffffu, v, j);
+      const bool up = ((lane & k) == 0) == ((lane & j) == 0);     // keep the smaller of the pair
+      v = up ? fminf(v, o) : fmaxf(v, o);
+    }
+  }
+  const float q1 = __shfl_sync(0xffffffffu, v, 8), m0 = __shfl_sync(0xffffffffu, v, 15),
+              m1 = __shfl_sync(0xffffffffu, v, 16), q3 = __shfl_sync(0xffffffffu, v, 24);
+  __syncthreads();
+  if (lane == 0) { red[w] = 0.5f * (m0 + m1); red[NW + w] = q3 - q1; }
+  __syncthreads();
+  float K = 0.f, iqr = 0.f;
+#pragma unroll
+  for (int i = 0; i < NW; ++i) { K += red[i]; iqr += red[NW + i]; }
+  K *= 1.0f / NW; iqr *= 1.0f / NW;
+  __syncthreads();
+  float h = 2.5f * iqr;                                   // Gaussian: +-3.4 sigma; exponential: 96 % of the samples
+  if (!(h > 0.f) || !lof_finite(h)) h = fmaxf(fabsf(K) * 1e-6f, 1e-30f);
+  LofStatPlan pl;
+  pl.K = K;
+  pl.scale = (float)(LOF_F_NBINS - 2) / (2.0f * h);
+  pl.off = fmaf(-(K - h), pl.scale, 1.0f);               // x = K-h -> 1, x = K+h -> NBINS-1
+  return pl;
+}
+
+// One channel row of the stream in shared memory, by one warp: partial sums of d = x-K and d^2 (fp32 over
+// groups of 8, then fp64, fixed order) and the row's samples into the value histogram.  Row partials land
+// in rowpart[2c], [2c+1].
 template <int C, int L>
-__device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParams& prm, lof_stream_stats* out) {
+__device__ __forceinline__ void lof_stat_row(const LofFusedSmem& sm, int c, const LofStatPlan& pl, int lane) {
+  constexpr int T = 32 * L;
+  const float4* rp = reinterpret_cast<const float4*>(sm.xs + c * T);
+  const float K = pl.K, scale = pl.scale, off = pl.off;
+  double da = 0.0, dq = 0.0;
+  float ga = 0.f, gq = 0.f;
+#pragma unroll
+  for (int q = 0; q < L / 4; ++q) {
+    const float4 v = rp[q * 32 + lane];
+    const float xv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float d = xv[i] - K;
+      ga += d; gq = fmaf(d, d, gq);
+      atomicAdd(&sm.hist[lof_stat_bin(xv[i], scale, off)], 1u);
+    }
+    if ((q & 1) == 1 || q == L / 4 - 1) { da += (double)ga; dq += (double)gq; ga = 0.f; gq = 0.f; }
+  }
+  da = lof_warp_sum(da); dq = lof_warp_sum(dq);
+  if (lane == 0) { sm.rowpart[2 * c] = da; sm.rowpart[2 * c + 1] = dq; }
+}
+
+// After every row of the stream went through lof_stat_row (and a __syncthreads): mean and stddev from the
+// row partials in row order, the exact median (rank floor(N/2), S3) from the histogram and the
+// gathered samples, thresholds, the stats record.  Leaves the histogram zeroed and the work counters reset for
+// the passes that follow.  Returns the number of non-finite samples (then everything else is unspecified,
+// DESIGN.md S6); `median_out` is valid in every thread.
+template <int C, int L>
+__device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& prm, const LofStatPlan& pl,
+                                      lof_stream_stats* out, float& median_out) {
   using Cfg = LofFusedCfg<C, L>;
   constexpr int N = Cfg::N, NT = Cfg::NT;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31;
   uint32_t* part = sm.part;
-  // --- S1: centre K and spread from a strided sample (one sample per thread): makes the shifted sums
-  // well conditioned and places the value histogram.  Any K gives the same exact results.
-  double sa, sq;
-  {
-    const int idx = (int)(((long long)tid * N) / NT) + (tid * 7) % (N / NT > 0 ? N / NT : 1);
-    const float v = sm.xs[idx < N ? idx : N - 1];
-    sa = (double)v; sq = (double)v * (double)v;
-    lof_block_sum2<NT>(sa, sq, sm.red);
-  }
-  float K = (float)(sa / NT);
-  float sd = sqrtf(fmaxf((float)(sq / NT) - K * K, 0.f));
-  if (!lof_finite(K) || !lof_finite(sd)) { K = 0.f; sd = 1.f; }
-  float h = 1.25f * sd;
-  if (!(h > 0.f)) h = fmaxf(fabsf(K) * 1e-6f, 1e-30f);
-  const float scale = 2046.0f / (2.0f * h);
-  const float off = fmaf(-(K - h), scale, 1.0f);        // x = K-h -> 1, x = K+h -> 2047
-  for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
-  if (tid == 0) { sm.ctl[CT_NCAND] = 0; sm.ctl[CT_BAD] = 0; sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_FOUND] = 0; sm.ctl[CT_ROW] = 0; sm.ctl[CT_COLGRP] = 0; }
-  __syncthreads();
-  // --- S2: one pass: sums of d = x-K and d^2 in fp32 over groups of 8, folded into fp64; histogram of
-  // round(clamp((x-lo)*scale)) (a monotone map of x, so bins are value-ordered).
-  double da = 0.0, dq = 0.0;
   const float4* x4 = reinterpret_cast<const float4*>(sm.xs);
-  for (int i = tid; i < N / 4; i += 2 * NT) {
-    float ga = 0.f, gq = 0.f;
+  if (tid < 32) {
+    double a = 0.0, q = 0.0;
 #pragma unroll
-    for (int r = 0; r < 2; ++r) {
-      const int ii = i + r * NT;
-      if (ii < N / 4) {
-        const float4 v = x4[ii];
-        const float xv[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const float d = xv[q] - K;
-          ga += d; gq = fmaf(d, d, gq);
-          float yb = fmaf(xv[q], scale, off);
-          yb = fminf(fmaxf(yb, 0.f), 2047.4f);
-          const uint32_t bin = __float_as_uint(yb + LOF_F_MAGIC) & 2047u;
-          atomicAdd(&sm.hist[bin], 1u);
-        }
-      }
+    for (int c = lane; c < C; c += 32) { a += sm.rowpart[2 * c]; q += sm.rowpart[2 * c + 1]; }
+    a = lof_warp_sum(a); q = lof_warp_sum(q);
+    if (lane == 0) {
+      sm.red[0] = a; sm.red[1] = q;
+      sm.ctl[CT_NCAND] = 0; sm.ctl[CT_BAD] = 0; sm.ctl[CT_FOUND] = 0;
     }
-    da += (double)ga; dq += (double)gq;
   }
-  lof_block_sum2<NT>(da, dq, sm.red);
+  __syncthreads();
+  double da = sm.red[0], dq = sm.red[1];
   uint32_t n_bad = 0;
   if (!isfinite(da) || !isfinite(dq)) {
     // rare: a non-finite sample, or d^2 overflowed fp32: count exactly and redo the sums in fp64
@@ -198,45 +280,51 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
     for (int i = tid; i < N; i += NT) {
       const float x = sm.xs[i];
       bad += lof_finite(x) ? 0u : 1u;
-      const double d = (double)x - (double)K; a2 += d; q2 = fma(d, d, q2);
+      const double d = (double)x - (double)pl.K; a2 += d; q2 = fma(d, d, q2);
     }
     if (bad) atomicAdd(&sm.ctl[CT_BAD], bad);
     lof_block_sum2<NT>(a2, q2, sm.red);
     da = a2; dq = q2;
     n_bad = sm.ctl[CT_BAD];
   }
-  const double n = (double)N;
-  double var = (dq - da * da / n) / n;
-  if (!(var > 0.0)) var = 0.0;
-  const double mean = (double)K + da / n, stddev = sqrt(var);
-  // --- S3..S5: median
-  const uint32_t rank = N / 2;                          // DESIGN.md S3: rank floor(N/2), 0-based
+  LOF_PROF_T(ta);
+  const uint32_t rank = N / 2;
   float median = 0.f;
+  int how = 3;
   if (n_bad == 0) {
     lof_find_bin<LOF_F_NBINS>(sm.hist, rank, part, sm.ctl);
+    LOF_PROF_T(tb);
     const uint32_t bin = sm.ctl[CT_BIN], before = sm.ctl[CT_BEFORE];
     const uint32_t n_b = sm.hist[bin];
     __syncthreads();
-    bool ok = bin > 0 && bin < 2047 && n_b <= LOF_F_CAP;
+    bool ok = bin > 0 && bin < LOF_F_NBINS - 1 && n_b <= LOF_F_CAP;
     if (ok) {
-      // S4: gather the samples of the median's bin
+      // gather the samples of the median's bin: two compares per sample against value bounds that enclose
+      // the bin (a few ulps wide of it), then the exact bin function on the few that pass
+      const float inv = 1.0f / pl.scale;
+      const float v0 = ((float)bin - 0.5f - pl.off) * inv, v1 = ((float)bin + 0.5f - pl.off) * inv;
+      const float eps = 8e-7f * (fabsf(v0) + fabsf(v1) + fabsf(pl.off) * inv) + 8e-4f * inv;
+      const float vmid = 0.5f * (v0 + v1), vhalf = 0.5f * (v1 - v0) + eps;
+      auto take = [&](float xq) {
+        if (fabsf(xq - vmid) <= vhalf && lof_stat_bin(xq, pl.scale, pl.off) == bin) {
+          const uint32_t slot = atomicAdd(&sm.ctl[CT_NCAND], 1u);
+          if (slot < LOF_F_CAP) sm.cand[slot] = xq;
+        }
+      };
+#pragma unroll 2
       for (int i = tid; i < N / 4; i += NT) {
         const float4 v = x4[i];
-        const float xv[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          float yb = fmaf(xv[q], scale, off);
-          yb = fminf(fmaxf(yb, 0.f), 2047.4f);
-          if ((__float_as_uint(yb + LOF_F_MAGIC) & 2047u) == bin) {
-            const uint32_t slot = atomicAdd(&sm.ctl[CT_NCAND], 1u);
-            if (slot < LOF_F_CAP) sm.cand[slot] = xv[q];
-          }
-        }
+        const float dmin = fminf(fminf(fabsf(v.x - vmid), fabsf(v.y - vmid)), fminf(fabsf(v.z - vmid), fabsf(v.w - vmid)));
+        if (dmin <= vhalf) { take(v.x); take(v.y); take(v.z); take(v.w); }
       }
       __syncthreads();
-      // S5: the candidate with exactly (rank - before) candidates ordered before it
+      LOF_PROF_T(tg);
+      LOF_PROF_ADD(5, tb, tg);
+      // the candidate with exactly (rank - before) candidates ordered before it
       const uint32_t want = rank - before, nc = sm.ctl[CT_NCAND];
-      if (nc <= 256) {
+      if (nc != n_b) ok = false;                         // bounds too tight (cannot happen): stay exact anyway
+      else if (nc <= 256) {
+        how = 0;
         for (uint32_t i = tid; i < nc; i += NT) {
           const float v = sm.cand[i];
           uint32_t less = 0;
@@ -247,26 +335,52 @@ __device__ uint32_t lof_fused_statistics(const LofFusedSmem& sm, const LofKParam
           if (less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
         }
         __syncthreads();
+        ok = sm.ctl[CT_FOUND] != 0;
+        median = __uint_as_float(sm.ctl[CT_MEDBITS]);
       } else {
-        const float m = lof_radix_select_smem<NT>(sm.cand, (int)nc, want, sm.hist, part, sm.ctl);
-        if (tid == 0) { sm.ctl[CT_MEDBITS] = __float_as_uint(m); sm.ctl[CT_FOUND] = 1; }
-        __syncthreads();
+        how = 1;
+        median = lof_radix_select_smem<NT>(sm.cand, (int)nc, want, sm.hist, part, sm.ctl);
       }
-      ok = sm.ctl[CT_FOUND] != 0;
-      median = __uint_as_float(sm.ctl[CT_MEDBITS]);
     }
-    if (!ok) median = lof_radix_select_smem<NT>(sm.xs, N, rank, sm.hist, part, sm.ctl);
+    if (!ok) { how = 2; median = lof_radix_select_smem<NT>(sm.xs, N, rank, sm.hist, part, sm.ctl); }
   }
+  __syncthreads();
+  LOF_PROF_T(tc);
+  LOF_PROF_ADD(6, ta, tc);
+  for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
   if (tid == 0) {
+    const double n = (double)N;
+    double var = (dq - da * da / n) / n;
+    if (!(var > 0.0)) var = 0.0;
+    const double mean = (double)pl.K + da / n, stddev = sqrt(var);
     for (uint32_t k = 0; k < prm.n_levels; ++k)
       sm.thr[k] = (float)((double)median + stddev * prm.factor[k] * prm.sensitivity);
     lof_stream_stats o;
     o.median = median; o.n_nonfinite = n_bad; o.mean = mean; o.stddev = stddev;
     o.n_flagged = n_bad ? (uint64_t)N : 0;
     *out = o;
+    sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_ROW] = 0; sm.ctl[CT_COLGRP] = 0; sm.ctl[CT_SROW] = 0;
+    atomicAdd(&lof_fused_counters_dev[how], 1ull);
   }
   __syncthreads();
+  LOF_PROF_T(td);
+  LOF_PROF_ADD(7, tc, td);
+  median_out = median;
   return n_bad;
+}
+
+// Statistics of a stream that is completely in shared memory (first stream of a CTA): plan from a strided
+// sample, every row through lof_stat_row, then lof_stat_finalize.
+template <int C, int L>
+__device__ uint32_t lof_stat_whole(const LofFusedSmem& sm, const LofKParams& prm, float sample,
+                                   lof_stream_stats* out, float& median_out) {
+  using Cfg = LofFusedCfg<C, L>;
+  constexpr int NT = Cfg::NT, NW = NT / 32;
+  const LofStatPlan pl = lof_stat_plan<NT>(sample, reinterpret_cast<float*>(sm.red));
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int c = warp; c < C; c += NW) lof_stat_row<C, L>(sm, c, pl, lane);
+  __syncthreads();
+  return lof_stat_finalize<C, L>(sm, prm, pl, out, median_out);
 }
 
 __host__ __device__ constexpr int lof_ilog2c(int v) { return v <= 1 ? 0 : 1 + lof_ilog2c(v / 2); }
@@ -284,6 +398,22 @@ __device__ __forceinline__ void lof_cp_async16(void* smem_dst, const void* gsrc)
 }
 __device__ __forceinline__ void lof_cp_async_wait_all() {
   asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
+
+// mbarrier per channel row: the 32 lanes that prefetch a row of the next stream make the row's barrier track
+// their copies; any warp can then wait for the row (cp.async.wait_group would only serve the issuing thread).
+__device__ __forceinline__ void lof_mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void lof_mbar_arrive_on_copies(unsigned long long* bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void lof_mbar_wait(unsigned long long* bar, unsigned parity) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile(
+      "{\n.reg .pred p;\nLOF_MBAR_WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@!p bra LOF_MBAR_WAIT_%=;\n}" ::"r"(a), "r"(parity) : "memory");
 }
 
 // ---- F: SumThreshold along frequency.  One thread per time column; u[c], e[c] in registers.
@@ -559,7 +689,8 @@ __device__ __forceinline__ void lof_row_flag(const float (&x)[L], uint32_t& fb, 
 template <int C, int L>
 __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, uint32_t s, bool have_f,
                                uint32_t* __restrict__ flags, double* __restrict__ rowsum,
-                               uint32_t* __restrict__ rowcnt, const float* __restrict__ next_stream) {
+                               uint32_t* __restrict__ rowcnt, const float* __restrict__ next_stream,
+                               const LofStatPlan& plan_next, unsigned bar_parity) {
   using Cfg = LofFusedCfg<C, L>;
   constexpr int T = Cfg::T, NT = Cfg::NT, W = Cfg::W, NW = NT / 32;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -594,6 +725,7 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
         const float4* src = reinterpret_cast<const float4*>(next_stream + c * T);
 #pragma unroll
         for (int q = 0; q < L / 4; ++q) lof_cp_async16(dst + lof_swz_chunk(q * 32 + lane), src + q * 32 + lane);
+        lof_mbar_arrive_on_copies(sm.rowbar + c);
       }
     };
     if (nlt > 0) lof_row_flag<L>(x, fb, sm.thr, (int)nlt, lane, prefetch_row);
@@ -633,10 +765,26 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
       n_flag_acc += nf;
     }
   }
+  // statistics pass of the next stream: warps that run out of rows above take the prefetched rows in the
+  // order they were asked for and wait on the row's barrier; the slower warps find little left to do
+  if (Cfg::OVL && next_stream) {
+#pragma unroll 1
+    for (;;) {
+      int c = 0;
+      if (lane == 0) c = (int)atomicAdd(&sm.ctl[CT_SROW], 1u);
+      c = __shfl_sync(0xffffffffu, c, 0);
+      if (c >= C) break;
+      lof_mbar_wait(sm.rowbar + c, bar_parity);
+      lof_stat_row<C, L>(sm, c, plan_next, lane);
+    }
+  }
   if (lane == 0 && n_flag_acc) atomicAdd(&sm.ctl[CT_NFLAG], n_flag_acc);
 }
 
-// The kernel: persistent CTAs, one stream at a time.
+
+// The kernel: persistent CTAs, one stream at a time.  Steady state per stream: frequency pass, time pass
+// (which also brings in the next stream row by row and runs that stream's statistics pass on the rows that
+// have landed), then the short serial end of the next stream's statistics (median, thresholds).
 template <int C, int L>
 __global__ void __launch_bounds__(LofFusedCfg<C, L>::NT, LofFusedCfg<C, L>::MINB)
 lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_stream_stats* __restrict__ stats,
@@ -645,36 +793,66 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
   constexpr int N = Cfg::N, NT = Cfg::NT, W = Cfg::W;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const LofFusedSmem sm = LofFusedSmem::make<C, L>(smem_raw);
-  bool loaded = false;
+  const int tid = threadIdx.x;
+  // position of this thread's sample for the plan (one strided sample per thread)
+  const int samp_idx0 = (int)(((long long)tid * N) / NT) + (tid * 7) % (N / NT > 0 ? N / NT : 1);
+  const int samp_idx = samp_idx0 < N ? samp_idx0 : N - 1;
+  bool ready = false;          // shared memory holds stream s and its statistics are done
+  float median = 0.f;
+  uint32_t n_bad = 0;
+  unsigned bar_parity = 0;     // phase of the row barriers the next prefetch completes
+  if (tid < C) lof_mbar_init(sm.rowbar + tid, 32);
+  __syncthreads();
 #pragma unroll 1
   for (uint32_t s = blockIdx.x; s < prm.S; s += gridDim.x) {
-    if (!loaded) {                                      // first stream of this CTA (or after a skipped one)
-      const float4* g4 = reinterpret_cast<const float4*>(power + (size_t)s * N);
+    LOF_PROF_T(t0);
+    if (!ready) {                                         // first stream of this CTA (or after a skipped one)
+      const float* gs = power + (size_t)s * N;
+      const float4* g4 = reinterpret_cast<const float4*>(gs);
       float4* s4 = reinterpret_cast<float4*>(sm.xs);
-      for (int i = threadIdx.x; i < N / 4; i += NT) lof_cp_async16(s4 + lof_swz_chunk(i), g4 + i);
+      for (int i = tid; i < N / 4; i += NT) lof_cp_async16(s4 + lof_swz_chunk(i), g4 + i);
+      const float sample = __ldg(gs + samp_idx);
+      for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
+      lof_cp_async_wait_all();
+      __syncthreads();
+      n_bad = lof_stat_whole<C, L>(sm, prm, sample, stats + s, median);
     }
-    lof_cp_async_wait_all();
-    __syncthreads();
-    loaded = false;
-    const uint32_t n_bad = lof_fused_statistics<C, L>(sm, prm, stats + s);
+    ready = false;
     if (n_bad) {
       // DESIGN.md S6: the whole stream is flagged
-      for (int i = threadIdx.x; i < C * W; i += NT) flags[(size_t)s * C * W + i] = 0xFFFFFFFFu;
-      for (int i = threadIdx.x; i < C; i += NT) { rowsum[(size_t)s * C + i] = 0.0; rowcnt[(size_t)s * C + i] = 0; }
+      for (int i = tid; i < C * W; i += NT) flags[(size_t)s * C * W + i] = 0xFFFFFFFFu;
+      for (int i = tid; i < C; i += NT) { rowsum[(size_t)s * C + i] = 0.0; rowcnt[(size_t)s * C + i] = 0; }
+      if (tid == 0) atomicAdd(&lof_fused_counters_dev[3], 1ull);
       __syncthreads();
       continue;
     }
+    const uint32_t s_next = s + gridDim.x;
+    const bool more = s_next < prm.S;
+    const float* next = more ? power + (size_t)s_next * N : nullptr;
+    const float sample_next = more ? __ldg(next + samp_idx) : 0.f;
     const bool have_f = prm.n_lev_f > 0;
+    LOF_PROF_T(t1);
     if (have_f) lof_fused_freq<C, L>(sm, prm.n_lev_f);
     __syncthreads();
-    const uint32_t s_next = s + gridDim.x;
-    // the time pass prefetches the next stream row by row, as each row moves into registers
-    const bool prefetch = s_next < prm.S;
-    lof_fused_time<C, L>(sm, prm, s, have_f, flags, rowsum, rowcnt, prefetch ? power + (size_t)s_next * N : nullptr);
-    loaded = prefetch;
+    LOF_PROF_T(t2);
+    LofStatPlan plan_next;
+    if (Cfg::OVL) plan_next = lof_stat_plan<NT>(sample_next, reinterpret_cast<float*>(sm.red));
+    LOF_PROF_T(t3);
+    lof_fused_time<C, L>(sm, prm, s, have_f, flags, rowsum, rowcnt, next, plan_next, bar_parity);
+    if (more) bar_parity ^= 1u;
+    lof_cp_async_wait_all();
     __syncthreads();
-    if (threadIdx.x == 0) stats[s].n_flagged = sm.ctl[CT_NFLAG];
+    LOF_PROF_T(t4);
+    if (tid == 0) stats[s].n_flagged = sm.ctl[CT_NFLAG];
     __syncthreads();
+    if (more) {
+      if (Cfg::OVL) n_bad = lof_stat_finalize<C, L>(sm, prm, plan_next, stats + s_next, median);
+      else n_bad = lof_stat_whole<C, L>(sm, prm, sample_next, stats + s_next, median);
+      ready = true;
+    }
+    LOF_PROF_T(t5);
+    LOF_PROF_ADD(0, t0, t1); LOF_PROF_ADD(1, t1, t2); LOF_PROF_ADD(2, t2, t3); LOF_PROF_ADD(3, t3, t4);
+    LOF_PROF_ADD(4, t4, t5);
   }
   lof_cp_async_wait_all();
 }

@@ -17,7 +17,7 @@ E_NULL, E_PARAM, E_ALIGN, E_STATE, E_CUDA = -1, -2, -3, -4, -5
 
 EXPORTS = ["lof_create", "lof_destroy", "lof_flag_block", "lof_flag_block_ci16", "lof_history_update",
            "lof_reset", "lof_row_sums", "lof_history_export", "lof_flag_block_host", "lof_factor_table",
-           "lof_launch_count", "lof_set_path", "lof_strerror", "lof_last_cuda_error"]
+           "lof_launch_count", "lof_set_path", "lof_fused_counters", "lof_fused_cycles", "lof_strerror", "lof_last_cuda_error"]
 
 
 class Params(C.Structure):
@@ -56,7 +56,7 @@ def lib():
         L.lof_launch_count.argtypes = [C.c_void_p]
         for name in ("lof_create", "lof_destroy", "lof_flag_block", "lof_flag_block_ci16",
                      "lof_history_update", "lof_reset", "lof_row_sums", "lof_history_export",
-                     "lof_flag_block_host", "lof_factor_table", "lof_set_path"):
+                     "lof_flag_block_host", "lof_factor_table", "lof_set_path", "lof_fused_counters", "lof_fused_cycles"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -178,6 +178,16 @@ class Flagger:
 
     def set_path(self, path):
         _check(lib().lof_set_path(self.h, C.c_int(path)))
+
+    def fused_cycles(self):
+        out = (C.c_uint64 * 8)()
+        _check(lib().lof_fused_cycles(self.h, out))
+        return [int(v) for v in out]
+
+    def fused_counters(self, reset=False):
+        out = (C.c_uint64 * 4)()
+        _check(lib().lof_fused_counters(self.h, out, C.c_int(1 if reset else 0)))
+        return [int(v) for v in out]
 
 
 def stats_to_numpy(stats):
