@@ -34,7 +34,7 @@ struct LofFusedCfg {
 #ifdef LOF_FUSED_NT
   static constexpr int NT = LOF_FUSED_NT;
 #else
-  static constexpr int NT = (C >= 64) ? 384 : 256;
+  static constexpr int NT = (C >= 64) ? 512 : 256;
 #endif
   static constexpr int MINB = (C >= 64) ? 1 : 2;
   // the next stream's statistics pass runs inside the time pass when the SM holds a single CTA; with two
@@ -571,6 +571,154 @@ __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
   }
 }
 
+// ---- F, 64 channels: two lanes per time column.  Lane l of the warp holds column p = l & 15 of the warp's 16
+// columns, channels [32h, 32h+32) with h = l >> 4; the lane holding the other half is l ^ 16.  Same doubling
+// as lof_col_flag with half the registers per thread (16 warps per SM instead of 12) and half the columns per
+// task (48 tasks per stream instead of 24: a shorter wait at the barrier that ends the pass).  Windows that
+// start in the lower half reach into the upper half through shuffles of the upper half's first D sums; a
+// window that would leave the column gets -inf and never fires.
+template <int D>
+__device__ __forceinline__ void lof_pcol_step(float (&u)[32], __half2 (&e2)[16], int h) {
+  if constexpr (D == 1) {
+    float pu = __shfl_xor_sync(0xffffffffu, u[0], 16);
+    const uint32_t pe = __shfl_xor_sync(0xffffffffu, lof_bits_h2(e2[0]), 16);
+    if (h) pu = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) u[j] += (j + 1 < 32) ? u[j + 1] : pu;
+#pragma unroll
+    for (int m = 0; m < 16; ++m)
+      e2[m] = __hadd2(e2[m], lof_h2_shift1(e2[m], (m + 1 < 16) ? e2[m + 1] : lof_h2_bits(pe)));
+  } else {
+    float pu[D];
+    uint32_t pe[D / 2];
+#pragma unroll
+    for (int jj = 0; jj < D; ++jj) {
+      pu[jj] = __shfl_xor_sync(0xffffffffu, u[jj], 16);
+      if (h) pu[jj] = -INFINITY;
+      if ((jj & 1) == 0) pe[jj / 2] = __shfl_xor_sync(0xffffffffu, lof_bits_h2(e2[jj / 2]), 16);
+    }
+#pragma unroll
+    for (int j = 0; j < 32; ++j) u[j] += (j + D < 32) ? u[j + D] : pu[j + D - 32];
+#pragma unroll
+    for (int m = 0; m < 16; ++m)
+      e2[m] = __hadd2(e2[m], (2 * m + D < 32) ? e2[m + D / 2] : lof_h2_bits(pe[(2 * m + D - 32) / 2]));
+  }
+}
+
+// Test of iteration I = 2^K <= 32 after its doubling step.  Returns (warp-uniform) whether any flag is new.
+template <int K>
+__device__ __forceinline__ bool lof_pcol_eval(const float (&u)[32], const __half2 (&e2)[16], int h, float thr,
+                                              uint32_t& fb) {
+  constexpr int I = 1 << K;
+  const float negT = -thr;
+  float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+  for (int m = 0; m < 16; ++m) {
+    const float2 ef = __half22float2(e2[m]);
+    tm[(2 * m) & 3] = fmaxf(tm[(2 * m) & 3], fmaf(ef.x, negT, u[2 * m]));
+    tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], fmaf(ef.y, negT, u[2 * m + 1]));
+  }
+  const bool fired = fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f;
+  if (!__any_sync(0xffffffffu, fired)) return false;
+  uint32_t trig = 0;
+  if (fired) {
+#pragma unroll
+    for (int m = 0; m < 16; ++m) {
+      const float2 ef = __half22float2(e2[m]);
+      trig |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
+      trig |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
+    }
+  }
+  uint64_t dil = trig;
+#pragma unroll
+  for (int s = 1; s < I; s <<= 1) dil |= dil << s;
+  // windows started in the lower half reach into the upper half
+  const uint32_t spill = __shfl_xor_sync(0xffffffffu, (uint32_t)(dil >> 32), 16);
+  const uint32_t nf = fb | (uint32_t)dil | (h ? spill : 0u);
+  const bool changed = nf != fb;
+  fb = nf;
+  return __any_sync(0xffffffffu, changed);
+}
+
+// The frequency run of 16 columns x 64 channels by one warp: ld(j) returns this lane's sample of channel
+// 32h + j (called again on a restart).  Returns the lane's flag mask (bit j = channel 32h + j).
+template <class Ld>
+__device__ __forceinline__ uint32_t lof_pcol_flag(Ld ld, const float* thr, int nlf, int h) {
+  float u[32];
+  __half2 e2[16];
+  uint32_t fb = 0;
+  const float T0 = thr[0];
+  int k_next = 1;
+  bool again = true;
+#pragma unroll 1
+  while (again) {
+    float m0 = -INFINITY, m1 = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+      u[j] = ld(j); u[j + 1] = ld(j + 1);
+      m0 = fmaxf(m0, u[j]); m1 = fmaxf(m1, u[j + 1]);
+      e2[j / 2] = lof_h2_bits(LOF_H2_ONES);
+    }
+    if (fb != 0 || fmaxf(m0, m1) > T0) {
+#pragma unroll
+      for (int j = 0; j < 32; ++j)
+        if (((fb >> j) & 1u) || u[j] > T0) { fb |= 1u << j; u[j] = 0.f; }
+#pragma unroll
+      for (int m = 0; m < 16; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
+    }
+    again = false;
+#define LOF_PCOL_LEVEL(K)                                                          \
+    if (K < nlf && !again) {                                                       \
+      lof_pcol_step<(1 << (K - 1))>(u, e2, h);                                     \
+      if (K >= k_next && lof_pcol_eval<K>(u, e2, h, thr[K], fb) && K + 1 < nlf) {  \
+        again = true; k_next = K + 1;                                              \
+      }                                                                            \
+    }
+    LOF_PCOL_LEVEL(1) LOF_PCOL_LEVEL(2) LOF_PCOL_LEVEL(3) LOF_PCOL_LEVEL(4) LOF_PCOL_LEVEL(5)
+#undef LOF_PCOL_LEVEL
+    if (6 < nlf && !again && 6 >= k_next) {
+      // I = 64: the one window that is the whole column
+      const float ub = __shfl_xor_sync(0xffffffffu, u[0], 16);
+      const float eb = __shfl_xor_sync(0xffffffffu, __low2float(e2[0]), 16);
+      const float v = (u[0] + ub) - (__low2float(e2[0]) + eb) * thr[6];
+      if (v > 0.f) fb = 0xFFFFFFFFu;             // both lanes of the pair see the same v
+    }
+  }
+  return fb;
+}
+
+template <int C, int L>
+__device__ void lof_fused_freq_pair(const LofFusedSmem& sm, uint32_t n_lev_f) {
+  static_assert(C == 64, "two lanes per column: 64 channels");
+  using Cfg = LofFusedCfg<C, L>;
+  constexpr int T = Cfg::T, W = Cfg::W;
+  const int lane = threadIdx.x & 31, h = lane >> 4, p = lane & 15;
+  uint16_t* fm16 = reinterpret_cast<uint16_t*>(sm.fm);
+#pragma unroll 1
+  for (;;) {
+    int g = 0;
+    if (lane == 0) g = (int)atomicAdd(&sm.ctl[CT_COLGRP], 1u);
+    g = __shfl_sync(0xffffffffu, g, 0);
+    if (g >= T / 16) break;
+    const int col = g * 16 + p;
+    const float* cp = sm.xs + (32 * h) * T + lof_swz_elem(col);
+    const uint32_t fb = lof_pcol_flag([cp](int j) { return cp[j * T]; }, sm.thr, (int)n_lev_f, h);
+    // 16 columns x 64 channels of flags -> half a mask word per channel: the ballot of bit j has channel j
+    // of the 16 columns in its low half and channel 32 + j in its high half; lane j keeps it
+    uint32_t mine = 0;
+    if (__any_sync(0xffffffffu, fb != 0)) {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) {
+        const uint32_t word = __ballot_sync(0xffffffffu, (fb >> j) & 1u);
+        if (j == lane) mine = word;
+      }
+    }
+    const int w = g >> 1, half = g & 1;
+    fm16[(lane * W + w) * 2 + half] = (uint16_t)(mine & 0xFFFFu);
+    fm16[((lane + 32) * W + w) * 2 + half] = (uint16_t)(mine >> 16);
+  }
+}
+
 // ---- T: SumThreshold along time.  One warp per channel row; lane l holds samples [l*L, l*L+L).
 // One doubling step of distance D (window 2D): partners beyond the lane's own L samples come from the
 // following lanes by shuffle; a partner outside the row is -inf, so such windows never fire.
@@ -832,7 +980,10 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
     const float sample_next = more ? __ldg(next + samp_idx) : 0.f;
     const bool have_f = prm.n_lev_f > 0;
     LOF_PROF_T(t1);
-    if (have_f) lof_fused_freq<C, L>(sm, prm.n_lev_f);
+    if (have_f) {
+      if constexpr (C == 64) lof_fused_freq_pair<C, L>(sm, prm.n_lev_f);
+      else lof_fused_freq<C, L>(sm, prm.n_lev_f);
+    }
     __syncthreads();
     LOF_PROF_T(t2);
     LofStatPlan plan_next;
