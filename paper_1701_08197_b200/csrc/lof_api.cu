@@ -8,6 +8,7 @@
 
 #include "lof_common.cuh"
 #include "lof_stats.cuh"
+#include "lof_stats_lr.cuh"
 #include "lof_flag_generic.cuh"
 #include "lof_history.cuh"
 #include "lof_fused.cuh"
@@ -41,7 +42,8 @@ struct lof_ctx {
   size_t smem_freq, smem_time;
   // device memory owned by the context
   LofStreamState* d_state;
-  uint32_t* d_hist;               // [group][2048]
+  uint32_t* d_hist;               // [group][4096] (the radix passes use 2048 of them)
+  float* d_cand;                  // [group][LOF_LR_CAND] samples of the median's bin (lof_stats_lr.cuh)
   double* d_partial;              // [group][n_chunks][2]
   uint32_t* d_fmask;              // [S][C][W] mask after the frequency run
   double* d_part_sum;             // [group*C][n_tiles]
@@ -109,7 +111,7 @@ extern "C" int lof_destroy(lof_ctx* c) {
   if (!c) return LOF_OK;
   cudaSetDevice(c->prm.device);
   cudaDeviceSynchronize();
-  cudaFree(c->d_state); cudaFree(c->d_hist); cudaFree(c->d_partial); cudaFree(c->d_fmask);
+  cudaFree(c->d_state); cudaFree(c->d_hist); cudaFree(c->d_cand); cudaFree(c->d_partial); cudaFree(c->d_fmask);
   cudaFree(c->d_part_sum); cudaFree(c->d_part_cnt); cudaFree(c->d_rowsum); cudaFree(c->d_rowcnt);
   cudaFree(c->d_stats); cudaFree(c->d_ring); cudaFree(c->d_head); cudaFree(c->d_count);
   cudaFree(c->d_row_flagged); cudaFree(c->d_in_stage); cudaFree(c->d_flags_stage);
@@ -189,7 +191,8 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   cudaError_t e = cudaSuccess;
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   A(dev_alloc(&c->d_state, S));
-  A(dev_alloc(&c->d_hist, (size_t)c->group * LOF_HIST_BINS));
+  A(dev_alloc(&c->d_hist, (size_t)c->group * LOF_LR_NBINS));
+  A(dev_alloc(&c->d_cand, (size_t)c->group * LOF_LR_CAND));
   A(dev_alloc(&c->d_partial, (size_t)c->group * c->n_chunks * 2));
   A(dev_alloc(&c->d_fmask, (size_t)S * C * W));
   size_t n_part = c->n_tiles > c->n_seg ? c->n_tiles : c->n_seg;
@@ -222,14 +225,31 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
     LofKParams kp = c->kp;
     kp.s0 = s0;
     const uint32_t nb = G * c->n_chunks;
-    lof_k_clear_state<<<(G + 255) / 256, 256, 0, st>>>(c->d_state, s0, G);
-    lof_k_hist<In, 0><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
-    lof_k_scan<In, 0><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
-    lof_k_hist<In, 1><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
-    lof_k_scan<In, 1><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
-    lof_k_hist<In, 2><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
-    lof_k_scan<In, 2><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
-    c->launches += 7;
+    if (c->path == 0) {
+      // two passes over the group's input (lof_stats_lr.cuh)
+      lof_k_lr_plan<In><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist);
+      // about four CTAs per SM, each over consecutive chunks of one stream
+      uint32_t cpb = (nb + (uint32_t)c->sm_count * 4 - 1) / ((uint32_t)c->sm_count * 4);
+      if (cpb < 1) cpb = 1;
+      const uint32_t n_blk = (c->n_chunks + cpb - 1) / cpb;
+      lof_k_lr_hist<In><<<G * n_blk, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial,
+                                                               c->n_chunks, cpb, n_blk);
+      lof_k_lr_select1<In><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
+      lof_k_lr_gather<In><<<G * n_blk, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_cand, c->n_chunks, cpb, n_blk);
+      lof_k_lr_select2<In><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_cand, c->d_stats);
+      c->launches += 5;
+    } else {
+      // three radix passes (lof_stats.cuh): the second implementation, kept for tests and as a reference
+      lof_k_clear_state<<<(G + 255) / 256, 256, 0, st>>>(c->d_state, s0, G);
+      lof_k_zero_u32<<<(unsigned)(((size_t)G * LOF_HIST_BINS + 255) / 256), 256, 0, st>>>(c->d_hist, (size_t)G * LOF_HIST_BINS);
+      lof_k_hist<In, 0><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
+      lof_k_scan<In, 0><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
+      lof_k_hist<In, 1><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
+      lof_k_scan<In, 1><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
+      lof_k_hist<In, 2><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
+      lof_k_scan<In, 2><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
+      c->launches += 8;
+    }
     const bool fast = c->path == 0;                     // path 1 forces the shared-memory generic kernels
     if (kp.n_lev_f) {
       const uint32_t nb_f = (uint32_t)(((uint64_t)G * kp.W + LOF_LR_WARPS - 1) / LOF_LR_WARPS);

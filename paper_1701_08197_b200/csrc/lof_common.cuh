@@ -19,7 +19,12 @@ struct LofStreamState {
   uint32_t prefix;                 // radix select: key bits fixed so far
   uint32_t rank;                   // rank still to find among keys matching prefix
   float    median;
-  uint32_t pad_;
+  // two-pass statistics of long streams (lof_stats_lr.cuh): histogram placement, the median's bin, candidates
+  float    pl_scale, pl_off;       // bin(x) = round(clamp(x*pl_scale + pl_off)); shift is the centre K
+  float    vmid, vhalf;            // |x - vmid| <= vhalf encloses the median's bin
+  uint32_t bin, before, nb;        // that bin, the number of samples in lower bins, the number in the bin
+  uint32_t ncand;                  // candidates gathered so far
+  uint32_t fallback;               // 1: the histogram could not isolate the median; radix select over the stream
 };
 
 // Parameters every kernel needs, passed by value.
@@ -50,6 +55,11 @@ __device__ __forceinline__ bool lof_finite(float x) {
 struct InF32 {
   const float* p;
   __device__ __forceinline__ float ld(size_t i) const { return __ldg(p + i); }
+  // four consecutive samples, i a multiple of 4 (the API requires 16-byte aligned input)
+  __device__ __forceinline__ void ld4(size_t i, float (&x)[4]) const {
+    const float4 v = __ldg(reinterpret_cast<const float4*>(p + i));
+    x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
+  }
   static constexpr int kBytes = 4;
 };
 struct InCI16 {
@@ -58,6 +68,15 @@ struct InCI16 {
     const short2 v = __ldg(reinterpret_cast<const short2*>(p) + i);
     const int re = v.x, im = v.y;
     return __uint2float_rn((unsigned)(re * re + im * im));
+  }
+  __device__ __forceinline__ void ld4(size_t i, float (&x)[4]) const {
+    const int4 v = __ldg(reinterpret_cast<const int4*>(p + 2 * i));
+    const int w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int re = (int)(short)(w[k] & 0xFFFF), im = w[k] >> 16;
+      x[k] = __uint2float_rn((unsigned)(re * re + im * im));
+    }
   }
   static constexpr int kBytes = 4;
 };

@@ -83,9 +83,11 @@ __device__ unsigned long long lof_fused_cycles_dev[8];
 #ifdef LOF_FUSED_PROF
 #define LOF_PROF_T(var) const long long var = clock64()
 #define LOF_PROF_ADD(i, a, b) do { if (threadIdx.x == 0) atomicAdd(&lof_fused_cycles_dev[i], (unsigned long long)((b) - (a))); } while (0)
+#define LOF_PROF_CNT(i) do { if ((threadIdx.x & 31) == 0) atomicAdd(&lof_fused_cycles_dev[i], 1ull); } while (0)
 #else
 #define LOF_PROF_T(var)
 #define LOF_PROF_ADD(i, a, b)
+#define LOF_PROF_CNT(i)
 #endif
 
 // Find the bin holding `rank` in hist[NB] (NB a multiple of 1024, any blockDim that is a multiple of 32).
@@ -346,7 +348,6 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
   }
   __syncthreads();
   LOF_PROF_T(tc);
-  LOF_PROF_ADD(6, ta, tc);
   for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
   if (tid == 0) {
     const double n = (double)N;
@@ -364,7 +365,6 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
   }
   __syncthreads();
   LOF_PROF_T(td);
-  LOF_PROF_ADD(7, tc, td);
   median_out = median;
   return n_bad;
 }
@@ -671,7 +671,7 @@ __device__ __forceinline__ uint32_t lof_pcol_flag(Ld ld, const float* thr, int n
     if (K < nlf && !again) {                                                       \
       lof_pcol_step<(1 << (K - 1))>(u, e2, h);                                     \
       if (K >= k_next && lof_pcol_eval<K>(u, e2, h, thr[K], fb) && K + 1 < nlf) {  \
-        again = true; k_next = K + 1;                                              \
+        again = true; k_next = K + 1; LOF_PROF_CNT(6);                              \
       }                                                                            \
     }
     LOF_PCOL_LEVEL(1) LOF_PCOL_LEVEL(2) LOF_PCOL_LEVEL(3) LOF_PCOL_LEVEL(4) LOF_PCOL_LEVEL(5)
@@ -721,13 +721,14 @@ __device__ void lof_fused_freq_pair(const LofFusedSmem& sm, uint32_t n_lev_f) {
 
 // ---- T: SumThreshold along time.  One warp per channel row; lane l holds samples [l*L, l*L+L).
 // One doubling step of distance D (window 2D): partners beyond the lane's own L samples come from the
-// following lanes by shuffle; a partner outside the row is -inf, so such windows never fire.
+// following lanes by shuffle.  A window that leaves the row picks up some lane's own sums instead (the shuffle
+// wraps): a harmless finite value, because a valid window only ever adds valid windows, and lof_row_eval drops
+// the window starts beyond T - I before they can flag anything.
 template <int L, int D>
 __device__ __forceinline__ void lof_row_step(float (&u)[L], __half2 (&e2)[L / 2], int lane) {
   if constexpr (D == 1) {
-    float pu = __shfl_down_sync(0xffffffffu, u[0], 1);
+    const float pu = __shfl_down_sync(0xffffffffu, u[0], 1);
     const uint32_t pe = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[0]), 1);
-    if (lane == 31) pu = -INFINITY;
 #pragma unroll
     for (int j = 0; j < L; ++j) u[j] += (j + 1 < L) ? u[j + 1] : pu;
 #pragma unroll
@@ -741,7 +742,6 @@ __device__ __forceinline__ void lof_row_step(float (&u)[L], __half2 (&e2)[L / 2]
     for (int jj = 0; jj < NP; ++jj) {
       const int j = L - NP + jj, src = (j + D) % L, off = (j + D) / L;
       pu[jj] = __shfl_down_sync(0xffffffffu, u[src], off);
-      if (lane + off > 31) pu[jj] = -INFINITY;
       if ((jj & 1) == 0) pe[jj / 2] = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[src / 2]), off);
     }
 #pragma unroll
@@ -773,6 +773,12 @@ __device__ __forceinline__ bool lof_row_eval(const float (&u)[L], const __half2 
     const float2 ef = __half22float2(e2[m]);
     trig |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
     trig |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
+  }
+  {
+    // only windows that lie inside the row: starts t = lane*L + j <= 32*L - I
+    int nv = 32 * L - I + 1 - lane * L;
+    nv = nv < 0 ? 0 : (nv > L ? L : nv);
+    trig &= nv >= 32 ? 0xFFFFFFFFu : ((1u << nv) - 1u);
   }
   // own windows, inside the lane's L bits
   uint32_t own = trig;
@@ -825,7 +831,7 @@ __device__ __forceinline__ void lof_row_flag(const float (&x)[L], uint32_t& fb, 
     if (K < nlt && !again) {                                                             \
       lof_row_step<L, (1 << (K - 1))>(u, e2, lane);                                      \
       if (K >= k_next && lof_row_eval<L, K>(u, e2, lane, thr[K], fb) && K + 1 < nlt) {   \
-        again = true; k_next = K + 1;                                                    \
+        again = true; k_next = K + 1; LOF_PROF_CNT(7);                                    \
       }                                                                                  \
     }
     LOF_ROW_LEVEL(1) LOF_ROW_LEVEL(2) LOF_ROW_LEVEL(3) LOF_ROW_LEVEL(4) LOF_ROW_LEVEL(5)
@@ -977,7 +983,8 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
     const uint32_t s_next = s + gridDim.x;
     const bool more = s_next < prm.S;
     const float* next = more ? power + (size_t)s_next * N : nullptr;
-    const float sample_next = more ? __ldg(next + samp_idx) : 0.f;
+    // issued here, consumed after the frequency pass: no select on the loaded value, or the wait moves up here
+    const float sample_next = __ldg((more ? next : power + (size_t)s * N) + samp_idx);
     const bool have_f = prm.n_lev_f > 0;
     LOF_PROF_T(t1);
     if (have_f) {

@@ -1,0 +1,365 @@
+// lof_stats_lr.cuh — statistics of long streams (configs 4, 5: a stream does not fit one SM) in two passes
+// over the group's input instead of the three radix passes of lof_stats.cuh:
+//   lof_k_lr_plan     per stream: a strided sample, sorted per warp -> centre K and scale of a 4096-bin value
+//                     histogram (rank statistics, so RFI does not widen the bins); clears the stream's counters
+//   lof_k_lr_hist     per 8192-sample chunk: shifted sums (fp32 over 8, then fp64, fixed order) and the value
+//                     histogram (shared memory, merged into the stream's by atomics)
+//   lof_k_lr_select1  per stream: mean, stddev from the chunk partials in chunk order; the bin that holds rank
+//                     floor(N/2) and value bounds that enclose it
+//   lof_k_lr_gather   per chunk: two compares per sample against those bounds; the bin's samples are appended
+//                     to the stream's candidate list
+//   lof_k_lr_select2  per stream: exact rank select among the candidates (radix select on the float keys);
+//                     median, thresholds, stats record.  If the histogram could not isolate the median (bin at
+//                     an end of the range, list overflow) the same CTA runs the radix select over the whole
+//                     stream: slower, same result.
+// The bin function is the fused kernel's (monotone in x, so bins are value-ordered and selection is exact).
+#pragma once
+#include "lof_common.cuh"
+#include "lof_stats.cuh"
+
+#define LOF_LR_NBINS 4096
+#define LOF_LR_CAND 32768          // candidate list entries per stream
+#define LOF_LR_STAGE 8192          // ... of which this many can be selected from shared memory
+
+__device__ __forceinline__ uint32_t lof_lr_bin(float x, float scale, float off) {
+  float yb = fmaf(x, scale, off);
+  yb = fminf(fmaxf(yb, 0.f), (float)(LOF_LR_NBINS - 1) + 0.4f);
+  return __float_as_uint(yb + 12582912.0f) & (uint32_t)(LOF_LR_NBINS - 1);
+}
+
+template <class In>
+__global__ void __launch_bounds__(256)
+lof_k_lr_plan(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_t* __restrict__ hist) {
+  __shared__ float red[16];
+  const uint32_t sl = blockIdx.x, s = prm.s0 + sl;
+  const uint64_t N = (uint64_t)prm.C * prm.T;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const uint64_t step = N / 256 > 0 ? N / 256 : 1;
+  uint64_t idx = (uint64_t)tid * step + ((uint64_t)tid * 7) % step;
+  if (idx >= N) idx = N - 1;
+  float v = in.ld((uint64_t)s * N + idx);
+  if (!lof_finite(v)) v = 0.f;
+#pragma unroll
+  for (int k = 2; k <= 32; k <<= 1) {
+#pragma unroll
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      const float o = __shfl_xor_sync(0xffffffffu, v, j);
+      const bool up = ((lane & k) == 0) == ((lane & j) == 0);
+      v = up ? fminf(v, o) : fmaxf(v, o);
+    }
+  }
+  const float q1 = __shfl_sync(0xffffffffu, v, 8), m0 = __shfl_sync(0xffffffffu, v, 15),
+              m1 = __shfl_sync(0xffffffffu, v, 16), q3 = __shfl_sync(0xffffffffu, v, 24);
+  if (lane == 0) { red[w] = 0.5f * (m0 + m1); red[8 + w] = q3 - q1; }
+  uint32_t* gh = hist + (size_t)sl * LOF_LR_NBINS;
+  for (int b = tid; b < LOF_LR_NBINS; b += 256) gh[b] = 0;
+  __syncthreads();
+  if (tid == 0) {
+    float K = 0.f, iqr = 0.f;
+    for (int i = 0; i < 8; ++i) { K += red[i]; iqr += red[8 + i]; }
+    K *= 0.125f; iqr *= 0.125f;
+    float h = 2.5f * iqr;
+    if (!(h > 0.f) || !lof_finite(h)) h = fmaxf(fabsf(K) * 1e-6f, 1e-30f);
+    LofStreamState& st = state[s];
+    st.shift = (double)K;
+    st.pl_scale = (float)(LOF_LR_NBINS - 2) / (2.0f * h);
+    st.pl_off = fmaf(-(K - h), st.pl_scale, 1.0f);
+    st.nonfinite = 0; st.prefix = 0; st.rank = 0; st.ncand = 0; st.fallback = 0;
+  }
+}
+
+// grid.x = group_streams * n_blk; a CTA takes `cpb` consecutive chunks of one stream (n_blk = ceil(n_chunks /
+// cpb)), keeps their histogram in shared memory and merges it into the stream's once: with one chunk per CTA
+// the merge would cost as many global atomics as half the samples.  Sums stay per chunk (fixed order).
+template <class In>
+__global__ void __launch_bounds__(LOF_STATS_THREADS)
+lof_k_lr_hist(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_t* __restrict__ hist,
+              double* __restrict__ partial, uint32_t n_chunks, uint32_t cpb, uint32_t n_blk) {
+  __shared__ uint32_t sh_hist[LOF_LR_NBINS];
+  __shared__ double sh_red[32];
+  const uint32_t sl = blockIdx.x / n_blk;
+  const uint32_t blk = blockIdx.x - sl * n_blk;
+  const uint32_t s = prm.s0 + sl;
+  const uint64_t N = (uint64_t)prm.C * prm.T;
+  const uint64_t base = (uint64_t)s * N;
+  for (int b = threadIdx.x; b < LOF_LR_NBINS; b += LOF_STATS_THREADS) sh_hist[b] = 0;
+  const float K = (float)state[s].shift, scale = state[s].pl_scale, off = state[s].pl_off;
+  __syncthreads();
+  uint32_t bad = 0;
+  const uint32_t c_end = min(n_chunks, (blk + 1) * cpb);
+  for (uint32_t chunk = blk * cpb; chunk < c_end; ++chunk) {
+    const uint64_t lo = (uint64_t)chunk * LOF_STATS_CHUNK;
+    const uint64_t hi = min(N, lo + (uint64_t)LOF_STATS_CHUNK);
+    double sum = 0.0, sumsq = 0.0;
+    if (((N | lo) & 3) == 0 && hi - lo == LOF_STATS_CHUNK) {
+      // full chunk, 16-byte aligned: 4 x 16-byte loads per thread in flight, two groups of 8 samples each
+#pragma unroll 1
+      for (int it = 0; it < LOF_STATS_PER_THREAD / 16; ++it) {
+        float xv[16];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+          float t4[4];
+          in.ld4(base + lo + ((uint64_t)(it * 4 + r) * LOF_STATS_THREADS + threadIdx.x) * 4, t4);
+          xv[4 * r] = t4[0]; xv[4 * r + 1] = t4[1]; xv[4 * r + 2] = t4[2]; xv[4 * r + 3] = t4[3];
+        }
+#pragma unroll
+        for (int g = 0; g < 2; ++g) {
+          float ga = 0.f, gq = 0.f;
+#pragma unroll
+          for (int r = 0; r < 8; ++r) {
+            const float x = xv[8 * g + r], d = x - K;
+            ga += d; gq = fmaf(d, d, gq);
+            bad += lof_finite(x) ? 0u : 1u;
+            atomicAdd(&sh_hist[lof_lr_bin(x, scale, off)], 1u);
+          }
+          sum += (double)ga; sumsq += (double)gq;
+        }
+      }
+    } else {
+      for (uint64_t i0 = lo + threadIdx.x; i0 < hi; i0 += 8 * LOF_STATS_THREADS) {
+        float ga = 0.f, gq = 0.f;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+          const uint64_t i = i0 + (uint64_t)r * LOF_STATS_THREADS;
+          if (i < hi) {
+            const float x = in.ld(base + i), d = x - K;
+            ga += d; gq = fmaf(d, d, gq);
+            bad += lof_finite(x) ? 0u : 1u;
+            atomicAdd(&sh_hist[lof_lr_bin(x, scale, off)], 1u);
+          }
+        }
+        sum += (double)ga; sumsq += (double)gq;
+      }
+    }
+    const double rs = lof_block_sum(sum, sh_red);
+    const double rq = lof_block_sum(sumsq, sh_red);
+    if (threadIdx.x == 0) {
+      partial[((size_t)sl * n_chunks + chunk) * 2 + 0] = rs;
+      partial[((size_t)sl * n_chunks + chunk) * 2 + 1] = rq;
+    }
+  }
+  __syncthreads();
+  uint32_t* gh = hist + (size_t)sl * LOF_LR_NBINS;
+  for (int b = threadIdx.x; b < LOF_LR_NBINS; b += LOF_STATS_THREADS) {
+    const uint32_t v = sh_hist[b];
+    if (v) atomicAdd(&gh[b], v);
+  }
+  if (bad) atomicAdd(&state[s].nonfinite, bad);
+}
+
+// One CTA per stream: chunk partials -> mean, stddev (as lof_k_scan<0>); the bin holding rank floor(N/2).
+template <class In>
+__global__ void __launch_bounds__(256)
+lof_k_lr_select1(In in, LofKParams prm, LofStreamState* __restrict__ state, const uint32_t* __restrict__ hist,
+                 const double* __restrict__ partial, uint32_t n_chunks) {
+  __shared__ uint32_t sh_cnt[256];
+  __shared__ uint32_t sh_sel[2];
+  __shared__ double sh_red2[32];
+  const uint32_t sl = blockIdx.x, s = prm.s0 + sl;
+  const uint64_t N = (uint64_t)prm.C * prm.T;
+  LofStreamState& st = state[s];
+  const uint32_t* gh = hist + (size_t)sl * LOF_LR_NBINS;
+  const int tid = threadIdx.x;
+  const uint32_t rank = (uint32_t)(N / 2);              // rank floor(N/2), 0-based (S3)
+  const uint32_t per = (n_chunks + 255) / 256;
+  double a = 0.0, q = 0.0;
+  for (uint32_t c = tid * per; c < min(n_chunks, (tid + 1) * per); ++c) {
+    a += partial[((size_t)sl * n_chunks + c) * 2 + 0];
+    q += partial[((size_t)sl * n_chunks + c) * 2 + 1];
+  }
+  a = lof_block_sum(a, sh_red2);
+  q = lof_block_sum(q, sh_red2);
+  if (tid == 0) {
+    const double n = (double)N;
+    double var = (q - a * a / n) / n;
+    if (!(var > 0.0)) var = 0.0;
+    st.sum = a; st.sumsq = q;
+    st.mean = st.shift + a / n;
+    st.stddev = sqrt(var);
+    sh_sel[0] = (isfinite(a) && isfinite(q)) ? 0u : 1u;
+  }
+  constexpr int PER = LOF_LR_NBINS / 256;
+  uint32_t tot = 0;
+#pragma unroll
+  for (int j = 0; j < PER; ++j) tot += gh[tid * PER + j];
+  sh_cnt[tid] = tot;
+  __syncthreads();
+  if (tid < 32) {
+    uint32_t p[8], sum = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { p[j] = sh_cnt[tid * 8 + j]; sum += p[j]; }
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (tid >= o) inc += v; }
+    const uint32_t exc = inc - sum;
+    if ((rank >= exc && rank < inc) || (tid == 31 && rank >= inc)) {
+      uint32_t acc = exc; int j = 0;
+      for (; j < 7; ++j) { if (acc + p[j] > rank) break; acc += p[j]; }
+      int b = 0;
+      const int g = tid * 8 + j;
+      for (; b < PER - 1; ++b) { const uint32_t hv = gh[g * PER + b]; if (acc + hv > rank) break; acc += hv; }
+      const uint32_t bin = g * PER + b;
+      const uint32_t n_b = gh[bin];
+      const float scale = st.pl_scale, off = st.pl_off, inv = 1.0f / scale;
+      const float v0 = ((float)bin - 0.5f - off) * inv, v1 = ((float)bin + 0.5f - off) * inv;
+      const float eps = 8e-7f * (fabsf(v0) + fabsf(v1) + fabsf(off) * inv) + 8e-4f * inv;
+      st.bin = bin; st.before = acc; st.nb = n_b;
+      st.vmid = 0.5f * (v0 + v1); st.vhalf = 0.5f * (v1 - v0) + eps;
+      st.fallback = (bin == 0 || bin >= LOF_LR_NBINS - 1 || n_b > LOF_LR_CAND || st.nonfinite != 0 ||
+                     sh_sel[0] != 0) ? 1u : 0u;
+    }
+  }
+  (void)in;
+}
+
+template <class In>
+__global__ void __launch_bounds__(LOF_STATS_THREADS)
+lof_k_lr_gather(In in, LofKParams prm, LofStreamState* __restrict__ state, float* __restrict__ cand,
+                uint32_t n_chunks, uint32_t cpb, uint32_t n_blk) {
+  const uint32_t sl = blockIdx.x / n_blk;
+  const uint32_t blk = blockIdx.x - sl * n_blk;
+  const uint32_t s = prm.s0 + sl;
+  LofStreamState& st = state[s];
+  if (st.fallback) return;
+  const uint64_t N = (uint64_t)prm.C * prm.T;
+  const uint64_t base = (uint64_t)s * N;
+  const uint64_t lo = (uint64_t)blk * cpb * LOF_STATS_CHUNK;
+  const uint64_t hi = min(N, lo + (uint64_t)cpb * LOF_STATS_CHUNK);
+  const float vmid = st.vmid, vhalf = st.vhalf, scale = st.pl_scale, off = st.pl_off;
+  const uint32_t bin = st.bin;
+  float* cl = cand + (size_t)sl * LOF_LR_CAND;
+  auto take = [&](float x) {
+    if (fabsf(x - vmid) <= vhalf && lof_lr_bin(x, scale, off) == bin) {
+      const uint32_t slot = atomicAdd(&st.ncand, 1u);
+      if (slot < LOF_LR_CAND) cl[slot] = x;
+    }
+  };
+  uint64_t i = lo;
+  if (((N | lo) & 3) == 0) {
+    const uint64_t hi4 = lo + ((hi - lo) & ~(uint64_t)3);
+#pragma unroll 4
+    for (uint64_t j = lo + (uint64_t)threadIdx.x * 4; j < hi4; j += 4 * LOF_STATS_THREADS) {
+      float x[4];
+      in.ld4(base + j, x);
+      const float dmin = fminf(fminf(fabsf(x[0] - vmid), fabsf(x[1] - vmid)), fminf(fabsf(x[2] - vmid), fabsf(x[3] - vmid)));
+      if (dmin <= vhalf) { take(x[0]); take(x[1]); take(x[2]); take(x[3]); }
+    }
+    i = hi4;
+  }
+  for (uint64_t j = i + threadIdx.x; j < hi; j += LOF_STATS_THREADS) take(in.ld(base + j));
+}
+
+// Exact rank-`rank` element of n values by a 3-pass radix select (11 + 11 + 10 bits of the key), one CTA of
+// 256 threads; ld(i) returns value i.  Result valid in every thread.
+template <class Ld>
+__device__ float lof_lr_radix_select(Ld ld, uint64_t n, uint32_t rank, uint32_t* sh_hist /*2048*/, uint32_t* sh_cnt /*256*/,
+                                     uint32_t* sh_sel /*2*/) {
+  const int tid = threadIdx.x;
+  uint32_t prefix = 0;
+  for (int pass = 0; pass < 3; ++pass) {
+    for (int b = tid; b < 2048; b += 256) sh_hist[b] = 0;
+    __syncthreads();
+#pragma unroll 8
+    for (uint64_t i = tid; i < n; i += 256) {
+      const uint32_t key = lof_key(ld(i));
+      if (pass == 0) atomicAdd(&sh_hist[key >> 21], 1u);
+      else if (pass == 1) { if ((key >> 21) == prefix) atomicAdd(&sh_hist[(key >> 10) & 2047u], 1u); }
+      else { if ((key >> 10) == prefix) atomicAdd(&sh_hist[key & 1023u], 1u); }
+    }
+    __syncthreads();
+    uint32_t loc[8], tot = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { loc[j] = sh_hist[tid * 8 + j]; tot += loc[j]; }
+    sh_cnt[tid] = tot;
+    __syncthreads();
+    if (tid < 32) {
+      uint32_t p[8], sum = 0;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) { p[j] = sh_cnt[tid * 8 + j]; sum += p[j]; }
+      uint32_t inc = sum;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (tid >= o) inc += v; }
+      const uint32_t exc = inc - sum;
+      if ((rank >= exc && rank < inc) || (tid == 31 && rank >= inc)) {
+        uint32_t acc = exc; int j = 0;
+        for (; j < 7; ++j) { if (acc + p[j] > rank) break; acc += p[j]; }
+        int b = 0;
+        const int g = tid * 8 + j;
+        for (; b < 7; ++b) { const uint32_t hv = sh_hist[g * 8 + b]; if (acc + hv > rank) break; acc += hv; }
+        sh_sel[0] = g * 8 + b; sh_sel[1] = acc;
+      }
+    }
+    __syncthreads();
+    const uint32_t bin = sh_sel[0];
+    rank -= sh_sel[1];
+    prefix = pass == 0 ? bin : (pass == 1 ? ((prefix << 11) | bin) : ((prefix << 10) | bin));
+    __syncthreads();
+  }
+  return lof_unkey(prefix);
+}
+
+template <class In>
+__global__ void __launch_bounds__(256)
+lof_k_lr_select2(In in, LofKParams prm, LofStreamState* __restrict__ state, const float* __restrict__ cand,
+                 lof_stream_stats* __restrict__ stats) {
+  __shared__ uint32_t sh_hist[2048];
+  __shared__ uint32_t sh_cnt[256];
+  __shared__ uint32_t sh_sel[2];
+  __shared__ double sh_red[32];
+  __shared__ float sh_c[LOF_LR_STAGE];
+  const uint32_t sl = blockIdx.x, s = prm.s0 + sl;
+  const uint64_t N = (uint64_t)prm.C * prm.T;
+  const uint64_t base = (uint64_t)s * N;
+  LofStreamState& st = state[s];
+  const uint32_t rank = (uint32_t)(N / 2);
+  const uint32_t nc = st.ncand, before = st.before, nb = st.nb, fb = st.fallback;
+  const bool direct = fb != 0 || nc != nb || nc > LOF_LR_CAND || before > rank || rank - before >= nc;
+  float median;
+  if (!direct) {
+    const float* cl = cand + (size_t)sl * LOF_LR_CAND;
+    if (nc <= LOF_LR_STAGE) {
+      // the usual case: the list fits shared memory; one round of global loads, then three passes on chip
+#pragma unroll 8
+      for (uint32_t i = threadIdx.x; i < nc; i += 256) sh_c[i] = __ldg(cl + i);
+      __syncthreads();
+      median = lof_lr_radix_select([&](uint64_t i) { return sh_c[i]; }, nc, rank - before, sh_hist, sh_cnt, sh_sel);
+    } else {
+      median = lof_lr_radix_select([cl](uint64_t i) { return cl[i]; }, nc, rank - before, sh_hist, sh_cnt, sh_sel);
+    }
+  } else {
+    median = lof_lr_radix_select([&](uint64_t i) { return in.ld(base + i); }, N, rank, sh_hist, sh_cnt, sh_sel);
+    if (st.nonfinite == 0 && (!isfinite(st.sum) || !isfinite(st.sumsq))) {
+      // the fp32 group sums overflowed on finite data: redo them in fp64
+      double a = 0.0, q = 0.0;
+      for (uint64_t i = threadIdx.x; i < N; i += 256) {
+        const double d = (double)in.ld(base + i) - st.shift; a += d; q = fma(d, d, q);
+      }
+      a = lof_block_sum(a, sh_red);
+      q = lof_block_sum(q, sh_red);
+      if (threadIdx.x == 0) {
+        const double n = (double)N;
+        double var = (q - a * a / n) / n;
+        if (!(var > 0.0)) var = 0.0;
+        st.sum = a; st.sumsq = q; st.mean = st.shift + a / n; st.stddev = sqrt(var);
+      }
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < LOF_MAX_LEVELS) {
+    // one threshold per thread: threshold_I = median + stddev * factor_I * sensitivity, fp64
+    const double sd = st.stddev;
+    const uint32_t k = threadIdx.x;
+    if (k < prm.n_levels) {
+      const double t = (double)median + sd * prm.factor[k] * prm.sensitivity;
+      st.thr_d[k] = t;
+      st.thr_f[k] = (float)t;
+    }
+    if (k == 0) {
+      st.median = median;
+      lof_stream_stats o;
+      o.median = median; o.n_nonfinite = st.nonfinite; o.mean = st.mean; o.stddev = sd;
+      o.n_flagged = 0;
+      stats[s] = o;
+    }
+  }
+}
