@@ -293,32 +293,44 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
   const uint32_t rank = N / 2;
   float median = 0.f;
   int how = 3;
+  bool dp_done = false;
   if (n_bad == 0) {
     lof_find_bin<LOF_F_NBINS>(sm.hist, rank, part, sm.ctl);
     LOF_PROF_T(tb);
     const uint32_t bin = sm.ctl[CT_BIN], before = sm.ctl[CT_BEFORE];
     const uint32_t n_b = sm.hist[bin];
-    __syncthreads();
     bool ok = bin > 0 && bin < LOF_F_NBINS - 1 && n_b <= LOF_F_CAP;
     if (ok) {
       // gather the samples of the median's bin: two compares per sample against value bounds that enclose
-      // the bin (a few ulps wide of it), then the exact bin function on the few that pass
-      const float inv = 1.0f / pl.scale;
-      const float v0 = ((float)bin - 0.5f - pl.off) * inv, v1 = ((float)bin + 0.5f - pl.off) * inv;
-      const float eps = 8e-7f * (fabsf(v0) + fabsf(v1) + fabsf(pl.off) * inv) + 8e-4f * inv;
-      const float vmid = 0.5f * (v0 + v1), vhalf = 0.5f * (v1 - v0) + eps;
-      auto take = [&](float xq) {
-        if (fabsf(xq - vmid) <= vhalf && lof_stat_bin(xq, pl.scale, pl.off) == bin) {
-          const uint32_t slot = atomicAdd(&sm.ctl[CT_NCAND], 1u);
-          if (slot < LOF_F_CAP) sm.cand[slot] = xq;
+      // the bin (a few ulps wide of it), then the exact bin function on the few that pass.  The last warp
+      // does the fp64 end of mean and stddev meanwhile (a long dependent chain that would otherwise sit
+      // on one thread between two barriers).
+      if (tid >= NT - 32) {
+        if (lane == 0) {
+          const double n = (double)N;
+          double var = (dq - da * da / n) / n;
+          if (!(var > 0.0)) var = 0.0;
+          sm.red[2] = (double)pl.K + da / n; sm.red[3] = sqrt(var);
         }
-      };
-#pragma unroll 2
-      for (int i = tid; i < N / 4; i += NT) {
-        const float4 v = x4[i];
-        const float dmin = fminf(fminf(fabsf(v.x - vmid), fabsf(v.y - vmid)), fminf(fabsf(v.z - vmid), fabsf(v.w - vmid)));
-        if (dmin <= vhalf) { take(v.x); take(v.y); take(v.z); take(v.w); }
+      } else {
+        const float inv = 1.0f / pl.scale;
+        const float v0 = ((float)bin - 0.5f - pl.off) * inv, v1 = ((float)bin + 0.5f - pl.off) * inv;
+        const float eps = 8e-7f * (fabsf(v0) + fabsf(v1) + fabsf(pl.off) * inv) + 8e-4f * inv;
+        const float vmid = 0.5f * (v0 + v1), vhalf = 0.5f * (v1 - v0) + eps;
+        auto take = [&](float xq) {
+          if (fabsf(xq - vmid) <= vhalf && lof_stat_bin(xq, pl.scale, pl.off) == bin) {
+            const uint32_t slot = atomicAdd(&sm.ctl[CT_NCAND], 1u);
+            if (slot < LOF_F_CAP) sm.cand[slot] = xq;
+          }
+        };
+#pragma unroll 4
+        for (int i = tid; i < N / 4; i += NT - 32) {
+          const float4 v = x4[i];
+          const float dmin = fminf(fminf(fabsf(v.x - vmid), fabsf(v.y - vmid)), fminf(fabsf(v.z - vmid), fabsf(v.w - vmid)));
+          if (dmin <= vhalf) { take(v.x); take(v.y); take(v.z); take(v.w); }
+        }
       }
+      dp_done = true;
       __syncthreads();
       LOF_PROF_T(tg);
       LOF_PROF_ADD(5, tb, tg);
@@ -346,22 +358,27 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
     }
     if (!ok) { how = 2; median = lof_radix_select_smem<NT>(sm.xs, N, rank, sm.hist, part, sm.ctl); }
   }
-  __syncthreads();
   LOF_PROF_T(tc);
   for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
-  if (tid == 0) {
-    const double n = (double)N;
-    double var = (dq - da * da / n) / n;
-    if (!(var > 0.0)) var = 0.0;
-    const double mean = (double)pl.K + da / n, stddev = sqrt(var);
-    for (uint32_t k = 0; k < prm.n_levels; ++k)
-      sm.thr[k] = (float)((double)median + stddev * prm.factor[k] * prm.sensitivity);
-    lof_stream_stats o;
-    o.median = median; o.n_nonfinite = n_bad; o.mean = mean; o.stddev = stddev;
-    o.n_flagged = n_bad ? (uint64_t)N : 0;
-    *out = o;
-    sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_ROW] = 0; sm.ctl[CT_COLGRP] = 0; sm.ctl[CT_SROW] = 0;
-    atomicAdd(&lof_fused_counters_dev[how], 1ull);
+  if (tid < 32) {
+    double mean, stddev;
+    if (dp_done) { mean = sm.red[2]; stddev = sm.red[3]; }
+    else {
+      const double n = (double)N;
+      double var = (dq - da * da / n) / n;
+      if (!(var > 0.0)) var = 0.0;
+      mean = (double)pl.K + da / n; stddev = sqrt(var);
+    }
+    if ((uint32_t)lane < prm.n_levels)                   // threshold_I, one per lane
+      sm.thr[lane] = (float)((double)median + stddev * prm.factor[lane] * prm.sensitivity);
+    if (lane == 0) {
+      lof_stream_stats o;
+      o.median = median; o.n_nonfinite = n_bad; o.mean = mean; o.stddev = stddev;
+      o.n_flagged = n_bad ? (uint64_t)N : 0;
+      *out = o;
+      sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_ROW] = 0; sm.ctl[CT_COLGRP] = 0; sm.ctl[CT_SROW] = 0;
+      atomicAdd(&lof_fused_counters_dev[how], 1ull);
+    }
   }
   __syncthreads();
   LOF_PROF_T(td);
