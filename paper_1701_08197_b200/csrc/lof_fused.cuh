@@ -490,13 +490,14 @@ __device__ __forceinline__ bool lof_col_eval(const float (&u)[C], const __half2 
   bool changed = false;
   if (__any_sync(0xffffffffu, fired)) {
     if (fired) {
-      uint64_t trig = 0;
+      uint32_t tg[4] = {0u, 0u, 0u, 0u};                   // partial masks: no serial chain
 #pragma unroll
       for (int m = 0; 2 * m + I <= C; ++m) {
         LOF_COL_V(m, v0, v1)
-        if (v0 > 0.f) trig |= 1ull << (2 * m);
-        if (2 * m + 1 + I <= C && v1 > 0.f) trig |= 1ull << (2 * m + 1);
+        tg[(2 * m) >> 5] |= (v0 > 0.f) ? (1u << ((2 * m) & 31)) : 0u;
+        if (2 * m + 1 + I <= C) tg[2 + ((2 * m) >> 5)] |= (v1 > 0.f) ? (2u << ((2 * m) & 31)) : 0u;
       }
+      const uint64_t trig = (uint64_t)(tg[0] | tg[2]) | ((uint64_t)(tg[1] | tg[3]) << 32);
       uint64_t dil = trig;
 #pragma unroll
       for (int s = 1; s < I; s <<= 1) dil |= dil << s;
@@ -531,9 +532,13 @@ __device__ __forceinline__ uint64_t lof_col_flag(Ld ld, const float* thr, int nl
       e2[c / 2] = lof_h2_bits(LOF_H2_ONES);
     }
     if (fb != 0 || fmaxf(m0, m1) > T0) {
+      // independent partial masks (one per 32 channels and parity): no serial chain through fb
+      uint32_t g[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
-      for (int c = 0; c < C; ++c)
-        if (((fb >> c) & 1ull) || u[c] > T0) { fb |= 1ull << c; u[c] = 0.f; }
+      for (int c = 0; c < C; ++c) g[((c >> 5) << 1) | (c & 1)] |= (u[c] > T0) ? (1u << (c & 31)) : 0u;
+      fb |= (uint64_t)(g[0] | g[1]) | ((uint64_t)(g[2] | g[3]) << 32);
+#pragma unroll
+      for (int c = 0; c < C; ++c) u[c] = ((fb >> c) & 1ull) ? 0.f : u[c];
 #pragma unroll
       for (int m = 0; m < C / 2; ++m) e2[m] = lof_h2_unflagged((uint32_t)(fb >> (2 * m)) & 3u);
     }
@@ -637,15 +642,16 @@ __device__ __forceinline__ bool lof_pcol_eval(const float (&u)[32], const __half
   }
   const bool fired = fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f;
   if (!__any_sync(0xffffffffu, fired)) return false;
-  uint32_t trig = 0;
+  uint32_t tg[4] = {0u, 0u, 0u, 0u};                       // partial masks: no serial chain
   if (fired) {
 #pragma unroll
     for (int m = 0; m < 16; ++m) {
       const float2 ef = __half22float2(e2[m]);
-      trig |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
-      trig |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
+      tg[m & 1] |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
+      tg[2 + (m & 1)] |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
     }
   }
+  const uint32_t trig = (tg[0] | tg[1]) | (tg[2] | tg[3]);
   uint64_t dil = trig;
 #pragma unroll
   for (int s = 1; s < I; s <<= 1) dil |= dil << s;
@@ -677,9 +683,12 @@ __device__ __forceinline__ uint32_t lof_pcol_flag(Ld ld, const float* thr, int n
       e2[j / 2] = lof_h2_bits(LOF_H2_ONES);
     }
     if (fb != 0 || fmaxf(m0, m1) > T0) {
+      uint32_t g[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
-      for (int j = 0; j < 32; ++j)
-        if (((fb >> j) & 1u) || u[j] > T0) { fb |= 1u << j; u[j] = 0.f; }
+      for (int j = 0; j < 32; ++j) g[j & 3] |= (u[j] > T0) ? (1u << j) : 0u;
+      fb |= (g[0] | g[1]) | (g[2] | g[3]);
+#pragma unroll
+      for (int j = 0; j < 32; ++j) u[j] = ((fb >> j) & 1u) ? 0.f : u[j];
 #pragma unroll
       for (int m = 0; m < 16; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
     }
@@ -784,13 +793,14 @@ __device__ __forceinline__ bool lof_row_eval(const float (&u)[L], const __half2 
     tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], fmaf(ef.y, negT, u[2 * m + 1]));
   }
   if (!__any_sync(0xffffffffu, fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f)) return false;
-  uint32_t trig = 0;
+  uint32_t tg[4] = {0u, 0u, 0u, 0u};                       // partial masks: no serial chain
 #pragma unroll
   for (int m = 0; m < L / 2; ++m) {
     const float2 ef = __half22float2(e2[m]);
-    trig |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
-    trig |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
+    tg[m & 1] |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
+    tg[2 + (m & 1)] |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
   }
+  uint32_t trig = (tg[0] | tg[1]) | (tg[2] | tg[3]);
   {
     // only windows that lie inside the row: starts t = lane*L + j <= 32*L - I
     int nv = 32 * L - I + 1 - lane * L;
@@ -833,11 +843,14 @@ __device__ __forceinline__ void lof_row_flag(const float (&x)[L], uint32_t& fb, 
 #pragma unroll 1
   while (again) {
     // level 0 (I = 1) under the current mask: x > threshold_1 on samples not yet flagged
+    {
+      // four independent partial masks: no serial chain through fb
+      uint32_t g[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
-    for (int j = 0; j < L; ++j) {
-      const bool f = ((fb >> j) & 1u) || (x[j] > T0);
-      fb |= f ? (1u << j) : 0u;
-      u[j] = f ? 0.f : x[j];
+      for (int j = 0; j < L; ++j) g[j & 3] |= (x[j] > T0) ? (1u << j) : 0u;
+      fb |= (g[0] | g[1]) | (g[2] | g[3]);
+#pragma unroll
+      for (int j = 0; j < L; ++j) u[j] = ((fb >> j) & 1u) ? 0.f : x[j];
     }
 #pragma unroll
     for (int m = 0; m < L / 2; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);

@@ -171,13 +171,14 @@ __device__ __forceinline__ bool lof_row_eval_coop(const float (&u)[32], const __
     tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], fmaf(ef.y, negT, u[2 * m + 1]));
   }
   if (!__syncthreads_or(fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f)) return false;
-  uint32_t trig = 0;
+  uint32_t tg[4] = {0u, 0u, 0u, 0u};                       // partial masks: no serial chain
 #pragma unroll
   for (int m = 0; m < 16; ++m) {
     const float2 ef = __half22float2(e2[m]);
-    trig |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
-    trig |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
+    tg[m & 1] |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
+    tg[2 + (m & 1)] |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
   }
+  const uint32_t trig = (tg[0] | tg[1]) | (tg[2] | tg[3]);
   uint32_t own = trig;
 #pragma unroll
   for (int s = 1; s < I && s < 32; s <<= 1) own |= own << s;
@@ -249,11 +250,13 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
     const bool has_nb = warp + 1 < LOF_CO_WARPS;
 #pragma unroll 1
     while (again) {
+      {
+        uint32_t g[4] = {0u, 0u, 0u, 0u};                  // partial masks: no serial chain through fb
 #pragma unroll
-      for (int j = 0; j < 32; ++j) {
-        const bool f = ((fb >> j) & 1u) || (x[j] > T0);
-        fb |= f ? (1u << j) : 0u;
-        u[j] = f ? 0.f : x[j];
+        for (int j = 0; j < 32; ++j) g[j & 3] |= (x[j] > T0) ? (1u << j) : 0u;
+        fb |= (g[0] | g[1]) | (g[2] | g[3]);
+#pragma unroll
+        for (int j = 0; j < 32; ++j) u[j] = ((fb >> j) & 1u) ? 0.f : x[j];
       }
 #pragma unroll
       for (int m = 0; m < 16; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
