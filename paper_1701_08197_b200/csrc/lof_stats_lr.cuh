@@ -237,8 +237,21 @@ lof_k_lr_gather(In in, LofKParams prm, LofStreamState* __restrict__ state, float
   uint64_t i = lo;
   if (((N | lo) & 3) == 0) {
     const uint64_t hi4 = lo + ((hi - lo) & ~(uint64_t)3);
-#pragma unroll 4
-    for (uint64_t j = lo + (uint64_t)threadIdx.x * 4; j < hi4; j += 4 * LOF_STATS_THREADS) {
+    // four 16-byte loads in flight per thread, then the compares
+    constexpr uint64_t STEP = 4 * LOF_STATS_THREADS;
+    uint64_t j = lo + (uint64_t)threadIdx.x * 4;
+    for (; j + 3 * STEP < hi4; j += 4 * STEP) {
+      float x[4][4];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) in.ld4(base + j + r * STEP, x[r]);
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const float dmin = fminf(fminf(fabsf(x[r][0] - vmid), fabsf(x[r][1] - vmid)),
+                                 fminf(fabsf(x[r][2] - vmid), fabsf(x[r][3] - vmid)));
+        if (dmin <= vhalf) { take(x[r][0]); take(x[r][1]); take(x[r][2]); take(x[r][3]); }
+      }
+    }
+    for (; j < hi4; j += STEP) {
       float x[4];
       in.ld4(base + j, x);
       const float dmin = fminf(fminf(fabsf(x[0] - vmid), fabsf(x[1] - vmid)), fminf(fabsf(x[2] - vmid), fabsf(x[3] - vmid)));
