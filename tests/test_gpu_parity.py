@@ -234,3 +234,55 @@ def test_ci16_long_rows_register_kernels(lof, lofo, wl):
     w = wl.config4(1, n_stations=1, T=7001)
     res, _ = check(lof, lofo, None, w.S, 32, 7001, volt=w.volt, max_window=64)
     print("cfg4-like, windows 1..64", res)
+
+
+# ---- statistics: the cases in which the value histogram cannot isolate the median by itself
+
+def _stats_cases(rng, C, T):
+    """Streams that stress the exact-median selection: heavy ties (a bin holding thousands of equal samples),
+    a two-level distribution whose median sits far outside the sampled interquartile range, tiny spread
+    around a large offset, and plain noise."""
+    N = C * T
+    a = rng.integers(0, 3, size=N).astype(np.float32)                         # quantised: crowded bins
+    b = np.where(rng.random(N) < 0.505, 1.0, 1000.0).astype(np.float32)       # upper median 1.0, IQR huge
+    b += (rng.random(N) < 0.5).astype(np.float32) * 1e-3
+    c = (1.0e6 + 1e-2 * rng.standard_normal(N)).astype(np.float32)            # spread of a few ulps
+    d = rng.standard_exponential(N).astype(np.float32)
+    e = np.zeros(N, np.float32); e[: N // 2 - 3] = -1.0; e[N // 2 + 5:] = 7.0  # median among a few zeros
+    return np.stack([a, b, c, d, rng.permutation(e)]).reshape(5, C, T)
+
+
+@pytest.mark.parametrize("C,T,mw", [(64, 768, 64), (16, 768, 64), (16, 256, 32),      # fused kernels
+                                    (16, 20011, 64), (32, 9000, 256)])                  # long-row kernels
+def test_statistics_hard_medians(lof, lofo, C, T, mw):
+    rng = np.random.default_rng(C * 7 + T)
+    x = _stats_cases(rng, C, T)
+    ora = run_oracle(lofo, x, 5, C, T, max_window=mw)
+    for path in (0, 1):
+        g = run_gpu(lof, x, 5, C, T, path=path, max_window=mw)
+        assert_stats(g["stats"], ora["stats"])
+        assert_flags(g["flags"], ora, T, mw)
+
+
+def test_long_row_candidate_list_overflow(lof, lofo):
+    """More samples in the median's bin than the candidate list holds (quantised data, 16 x 40000): the
+    selection falls back to the radix select over the whole stream."""
+    rng = np.random.default_rng(11)
+    x = rng.integers(0, 2, size=(2, 16, 40000)).astype(np.float32)
+    x[1] += rng.standard_exponential((16, 40000)).astype(np.float32) * 1e-3
+    ora = run_oracle(lofo, x, 2, 16, 40000, max_window=64)
+    g = run_gpu(lof, x, 2, 16, 40000, max_window=64)
+    assert_stats(g["stats"], ora["stats"])
+    assert_flags(g["flags"], ora, 40000, 64)
+
+
+def test_fused_counters_account_for_every_stream(lof, wl):
+    import torch
+    w = wl.config2(3, n_stations=3)
+    f = lof.Flagger(w.S, w.C, w.T, max_window=64)
+    f.fused_counters(reset=True)
+    f.flag_block(torch.from_numpy(w.power).cuda())
+    c = f.fused_counters()
+    f.close()
+    assert sum(c) == w.S and c[3] == 0, c
+    assert c[0] >= w.S - 1, c          # noise-like streams: the median comes from the rank count in its bin
