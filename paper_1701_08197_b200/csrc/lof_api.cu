@@ -35,6 +35,7 @@ struct lof_ctx {
   // geometry of the generic path
   uint32_t group;                 // streams per group (bounded so a group's input stays in L2)
   uint32_t n_chunks;              // statistics chunks per stream
+  bool lr_dirty;                  // path 1 ran since path 0 last left its histogram slots zeroed
   uint32_t TT, halo, n_tiles;     // time tiling
   bool lr_freq, lr_time;          // register-resident long-row kernels usable (lof_longrow.cuh)
   uint32_t seg_out, seg_halo, n_seg;
@@ -44,6 +45,7 @@ struct lof_ctx {
   LofStreamState* d_state;
   uint32_t* d_hist;               // [group][4096] (the radix passes use 2048 of them)
   float* d_cand;                  // [group][LOF_LR_CAND] samples of the median's bin (lof_stats_lr.cuh)
+  uint32_t* d_ctr;                // [group][2] non-finite samples, candidates gathered (lof_stats_lr.cuh)
   double* d_partial;              // [group][n_chunks][2]
   uint32_t* d_fmask;              // [S][C][W] mask after the frequency run
   double* d_part_sum;             // [group*C][n_tiles]
@@ -111,7 +113,7 @@ extern "C" int lof_destroy(lof_ctx* c) {
   if (!c) return LOF_OK;
   cudaSetDevice(c->prm.device);
   cudaDeviceSynchronize();
-  cudaFree(c->d_state); cudaFree(c->d_hist); cudaFree(c->d_cand); cudaFree(c->d_partial); cudaFree(c->d_fmask);
+  cudaFree(c->d_state); cudaFree(c->d_hist); cudaFree(c->d_cand); cudaFree(c->d_ctr); cudaFree(c->d_partial); cudaFree(c->d_fmask);
   cudaFree(c->d_part_sum); cudaFree(c->d_part_cnt); cudaFree(c->d_rowsum); cudaFree(c->d_rowcnt);
   cudaFree(c->d_stats); cudaFree(c->d_ring); cudaFree(c->d_head); cudaFree(c->d_count);
   cudaFree(c->d_row_flagged); cudaFree(c->d_in_stage); cudaFree(c->d_flags_stage);
@@ -193,6 +195,7 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   A(dev_alloc(&c->d_state, S));
   A(dev_alloc(&c->d_hist, (size_t)c->group * LOF_LR_NBINS));
   A(dev_alloc(&c->d_cand, (size_t)c->group * LOF_LR_CAND));
+  A(dev_alloc(&c->d_ctr, (size_t)c->group * 2));
   A(dev_alloc(&c->d_partial, (size_t)c->group * c->n_chunks * 2));
   A(dev_alloc(&c->d_fmask, (size_t)S * C * W));
   size_t n_part = c->n_tiles > c->n_seg ? c->n_tiles : c->n_seg;
@@ -226,20 +229,27 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
     kp.s0 = s0;
     const uint32_t nb = G * c->n_chunks;
     if (c->path == 0) {
-      // two passes over the group's input (lof_stats_lr.cuh)
-      lof_k_lr_plan<In><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist);
-      // about four CTAs per SM, each over consecutive chunks of one stream
+      // two passes over the group's input, three launches (lof_stats_lr.cuh): about four CTAs per SM, each
+      // over consecutive chunks of one stream
       uint32_t cpb = (nb + (uint32_t)c->sm_count * 4 - 1) / ((uint32_t)c->sm_count * 4);
       if (cpb < 1) cpb = 1;
       const uint32_t n_blk = (c->n_chunks + cpb - 1) / cpb;
-      lof_k_lr_hist<In><<<G * n_blk, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial,
+      if (c->lr_dirty) {        // the radix passes of path 1 used the slots' histograms since the last group here
+        lof_k_zero_u32<<<(unsigned)(((size_t)c->group * LOF_LR_NBINS + 255) / 256), 256, 0, st>>>(c->d_hist, (size_t)c->group * LOF_LR_NBINS);
+        lof_k_zero_u32<<<1, 256, 0, st>>>(c->d_ctr, (size_t)c->group * 2);
+        c->lr_dirty = false;
+        c->launches += 2;
+      }
+      lof_k_lr_hist<In><<<G * n_blk, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_ctr, c->d_partial,
                                                                c->n_chunks, cpb, n_blk);
-      lof_k_lr_select1<In><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
-      lof_k_lr_gather<In><<<G * n_blk, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_cand, c->n_chunks, cpb, n_blk);
-      lof_k_lr_select2<In><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_cand, c->d_stats);
-      c->launches += 5;
+      lof_k_lr_gather<In><<<G * n_blk, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_ctr, c->d_cand,
+                                                                 c->n_chunks, cpb, n_blk);
+      lof_k_lr_select2<In><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_ctr, c->d_partial, c->n_chunks,
+                                              c->d_cand, c->d_stats);
+      c->launches += 3;
     } else {
       // three radix passes (lof_stats.cuh): the second implementation, kept for tests and as a reference
+      c->lr_dirty = true;
       lof_k_clear_state<<<(G + 255) / 256, 256, 0, st>>>(c->d_state, s0, G);
       lof_k_zero_u32<<<(unsigned)(((size_t)G * LOF_HIST_BINS + 255) / 256), 256, 0, st>>>(c->d_hist, (size_t)G * LOF_HIST_BINS);
       lof_k_hist<In, 0><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);

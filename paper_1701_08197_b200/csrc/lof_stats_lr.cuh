@@ -1,17 +1,19 @@
 // lof_stats_lr.cuh — statistics of long streams (configs 4, 5: a stream does not fit one SM) in two passes
-// over the group's input instead of the three radix passes of lof_stats.cuh:
-//   lof_k_lr_plan     per stream: a strided sample, sorted per warp -> centre K and scale of a 4096-bin value
-//                     histogram (rank statistics, so RFI does not widen the bins); clears the stream's counters
-//   lof_k_lr_hist     per 8192-sample chunk: shifted sums (fp32 over 8, then fp64, fixed order) and the value
-//                     histogram (shared memory, merged into the stream's by atomics)
-//   lof_k_lr_select1  per stream: mean, stddev from the chunk partials in chunk order; the bin that holds rank
-//                     floor(N/2) and value bounds that enclose it
-//   lof_k_lr_gather   per chunk: two compares per sample against those bounds; the bin's samples are appended
-//                     to the stream's candidate list
-//   lof_k_lr_select2  per stream: exact rank select among the candidates (radix select on the float keys);
-//                     median, thresholds, stats record.  If the histogram could not isolate the median (bin at
-//                     an end of the range, list overflow) the same CTA runs the radix select over the whole
-//                     stream: slower, same result.
+// over the group's input instead of the three radix passes of lof_stats.cuh, three launches:
+//   lof_k_lr_hist     a CTA over consecutive 8192-sample chunks of one stream.  First the plan, recomputed by
+//                     every CTA of the stream (same inputs, same result): a strided sample of 256, sorted per
+//                     warp -> centre K and scale of a 4096-bin value histogram (rank statistics, so RFI does
+//                     not widen the bins).  Then per chunk the shifted sums (fp32 over 8, then fp64, fixed
+//                     order) and the value histogram (shared memory, merged into the group slot's by atomics).
+//   lof_k_lr_gather   same decomposition.  First, again per CTA, the bin that holds rank floor(N/2) from the
+//                     slot's histogram and value bounds that enclose it; then two compares per sample against
+//                     those bounds: the bin's samples are appended to the slot's candidate list.
+//   lof_k_lr_select2  per stream: mean, stddev from the chunk partials in chunk order; exact rank select among
+//                     the candidates (radix select on the float keys, from shared memory); median, thresholds,
+//                     stats record; leaves the slot's histogram and counters zeroed for the next group.  If the
+//                     histogram could not isolate the median (bin at an end of the range, list overflow,
+//                     non-finite sums) the same CTA runs the radix select over the whole stream: slower, same
+//                     result.
 // The bin function is the fused kernel's (monotone in x, so bins are value-ordered and selection is exact).
 #pragma once
 #include "lof_common.cuh"
@@ -27,17 +29,16 @@ __device__ __forceinline__ uint32_t lof_lr_bin(float x, float scale, float off) 
   return __float_as_uint(yb + 12582912.0f) & (uint32_t)(LOF_LR_NBINS - 1);
 }
 
+// The histogram placement of stream s, by all 256 threads of a CTA; K, scale, off valid in every thread.
+// Contains __syncthreads.
 template <class In>
-__global__ void __launch_bounds__(256)
-lof_k_lr_plan(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_t* __restrict__ hist) {
-  __shared__ float red[16];
-  const uint32_t sl = blockIdx.x, s = prm.s0 + sl;
-  const uint64_t N = (uint64_t)prm.C * prm.T;
+__device__ __forceinline__ void lof_lr_plan(const In& in, uint64_t base, uint64_t N, float* red /*17 floats*/,
+                                            float& K, float& scale, float& off) {
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const uint64_t step = N / 256 > 0 ? N / 256 : 1;
   uint64_t idx = (uint64_t)tid * step + ((uint64_t)tid * 7) % step;
   if (idx >= N) idx = N - 1;
-  float v = in.ld((uint64_t)s * N + idx);
+  float v = in.ld(base + idx);
   if (!lof_finite(v)) v = 0.f;
 #pragma unroll
   for (int k = 2; k <= 32; k <<= 1) {
@@ -51,21 +52,16 @@ lof_k_lr_plan(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_
   const float q1 = __shfl_sync(0xffffffffu, v, 8), m0 = __shfl_sync(0xffffffffu, v, 15),
               m1 = __shfl_sync(0xffffffffu, v, 16), q3 = __shfl_sync(0xffffffffu, v, 24);
   if (lane == 0) { red[w] = 0.5f * (m0 + m1); red[8 + w] = q3 - q1; }
-  uint32_t* gh = hist + (size_t)sl * LOF_LR_NBINS;
-  for (int b = tid; b < LOF_LR_NBINS; b += 256) gh[b] = 0;
   __syncthreads();
-  if (tid == 0) {
-    float K = 0.f, iqr = 0.f;
-    for (int i = 0; i < 8; ++i) { K += red[i]; iqr += red[8 + i]; }
-    K *= 0.125f; iqr *= 0.125f;
-    float h = 2.5f * iqr;
-    if (!(h > 0.f) || !lof_finite(h)) h = fmaxf(fabsf(K) * 1e-6f, 1e-30f);
-    LofStreamState& st = state[s];
-    st.shift = (double)K;
-    st.pl_scale = (float)(LOF_LR_NBINS - 2) / (2.0f * h);
-    st.pl_off = fmaf(-(K - h), st.pl_scale, 1.0f);
-    st.nonfinite = 0; st.prefix = 0; st.rank = 0; st.ncand = 0; st.fallback = 0;
-  }
+  float Ks = 0.f, iqr = 0.f;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { Ks += red[i]; iqr += red[8 + i]; }
+  Ks *= 0.125f; iqr *= 0.125f;
+  float h = 2.5f * iqr;
+  if (!(h > 0.f) || !lof_finite(h)) h = fmaxf(fabsf(Ks) * 1e-6f, 1e-30f);
+  K = Ks;
+  scale = (float)(LOF_LR_NBINS - 2) / (2.0f * h);
+  off = fmaf(-(Ks - h), scale, 1.0f);
 }
 
 // grid.x = group_streams * n_blk; a CTA takes `cpb` consecutive chunks of one stream (n_blk = ceil(n_chunks /
@@ -74,16 +70,24 @@ lof_k_lr_plan(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_
 template <class In>
 __global__ void __launch_bounds__(LOF_STATS_THREADS)
 lof_k_lr_hist(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_t* __restrict__ hist,
-              double* __restrict__ partial, uint32_t n_chunks, uint32_t cpb, uint32_t n_blk) {
+              uint32_t* __restrict__ ctr, double* __restrict__ partial, uint32_t n_chunks, uint32_t cpb,
+              uint32_t n_blk) {
   __shared__ uint32_t sh_hist[LOF_LR_NBINS];
   __shared__ double sh_red[32];
+  __shared__ float sh_plan[17];
   const uint32_t sl = blockIdx.x / n_blk;
   const uint32_t blk = blockIdx.x - sl * n_blk;
   const uint32_t s = prm.s0 + sl;
   const uint64_t N = (uint64_t)prm.C * prm.T;
   const uint64_t base = (uint64_t)s * N;
   for (int b = threadIdx.x; b < LOF_LR_NBINS; b += LOF_STATS_THREADS) sh_hist[b] = 0;
-  const float K = (float)state[s].shift, scale = state[s].pl_scale, off = state[s].pl_off;
+  float K, scale, off;
+  lof_lr_plan(in, base, N, sh_plan, K, scale, off);
+  if (blk == 0 && threadIdx.x == 0) {
+    LofStreamState& st = state[s];
+    st.shift = (double)K; st.pl_scale = scale; st.pl_off = off;
+    st.prefix = 0; st.rank = 0;
+  }
   __syncthreads();
   uint32_t bad = 0;
   const uint32_t c_end = min(n_chunks, (blk + 1) * cpb);
@@ -144,41 +148,15 @@ lof_k_lr_hist(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_
     const uint32_t v = sh_hist[b];
     if (v) atomicAdd(&gh[b], v);
   }
-  if (bad) atomicAdd(&state[s].nonfinite, bad);
+  if (bad) atomicAdd(&ctr[2 * sl], bad);
 }
 
-// One CTA per stream: chunk partials -> mean, stddev (as lof_k_scan<0>); the bin holding rank floor(N/2).
-template <class In>
-__global__ void __launch_bounds__(256)
-lof_k_lr_select1(In in, LofKParams prm, LofStreamState* __restrict__ state, const uint32_t* __restrict__ hist,
-                 const double* __restrict__ partial, uint32_t n_chunks) {
-  __shared__ uint32_t sh_cnt[256];
-  __shared__ uint32_t sh_sel[2];
-  __shared__ double sh_red2[32];
-  const uint32_t sl = blockIdx.x, s = prm.s0 + sl;
-  const uint64_t N = (uint64_t)prm.C * prm.T;
-  LofStreamState& st = state[s];
-  const uint32_t* gh = hist + (size_t)sl * LOF_LR_NBINS;
-  const int tid = threadIdx.x;
-  const uint32_t rank = (uint32_t)(N / 2);              // rank floor(N/2), 0-based (S3)
-  const uint32_t per = (n_chunks + 255) / 256;
-  double a = 0.0, q = 0.0;
-  for (uint32_t c = tid * per; c < min(n_chunks, (tid + 1) * per); ++c) {
-    a += partial[((size_t)sl * n_chunks + c) * 2 + 0];
-    q += partial[((size_t)sl * n_chunks + c) * 2 + 1];
-  }
-  a = lof_block_sum(a, sh_red2);
-  q = lof_block_sum(q, sh_red2);
-  if (tid == 0) {
-    const double n = (double)N;
-    double var = (q - a * a / n) / n;
-    if (!(var > 0.0)) var = 0.0;
-    st.sum = a; st.sumsq = q;
-    st.mean = st.shift + a / n;
-    st.stddev = sqrt(var);
-    sh_sel[0] = (isfinite(a) && isfinite(q)) ? 0u : 1u;
-  }
+// The bin of the slot's histogram that holds `rank`, by the 256 threads of a CTA: sh[0] = bin, sh[1] = number
+// of samples in lower bins (rank beyond the total gives the last bin).  Contains __syncthreads.
+__device__ __forceinline__ void lof_lr_find_bin(const uint32_t* __restrict__ gh, uint32_t rank, uint32_t* sh_cnt /*256*/,
+                                                uint32_t* sh /*2*/) {
   constexpr int PER = LOF_LR_NBINS / 256;
+  const int tid = threadIdx.x;
   uint32_t tot = 0;
 #pragma unroll
   for (int j = 0; j < PER; ++j) tot += gh[tid * PER + j];
@@ -198,39 +176,46 @@ lof_k_lr_select1(In in, LofKParams prm, LofStreamState* __restrict__ state, cons
       int b = 0;
       const int g = tid * 8 + j;
       for (; b < PER - 1; ++b) { const uint32_t hv = gh[g * PER + b]; if (acc + hv > rank) break; acc += hv; }
-      const uint32_t bin = g * PER + b;
-      const uint32_t n_b = gh[bin];
-      const float scale = st.pl_scale, off = st.pl_off, inv = 1.0f / scale;
-      const float v0 = ((float)bin - 0.5f - off) * inv, v1 = ((float)bin + 0.5f - off) * inv;
-      const float eps = 8e-7f * (fabsf(v0) + fabsf(v1) + fabsf(off) * inv) + 8e-4f * inv;
-      st.bin = bin; st.before = acc; st.nb = n_b;
-      st.vmid = 0.5f * (v0 + v1); st.vhalf = 0.5f * (v1 - v0) + eps;
-      st.fallback = (bin == 0 || bin >= LOF_LR_NBINS - 1 || n_b > LOF_LR_CAND || st.nonfinite != 0 ||
-                     sh_sel[0] != 0) ? 1u : 0u;
+      sh[0] = g * PER + b; sh[1] = acc;
     }
   }
-  (void)in;
+  __syncthreads();
 }
 
 template <class In>
 __global__ void __launch_bounds__(LOF_STATS_THREADS)
-lof_k_lr_gather(In in, LofKParams prm, LofStreamState* __restrict__ state, float* __restrict__ cand,
-                uint32_t n_chunks, uint32_t cpb, uint32_t n_blk) {
+lof_k_lr_gather(In in, LofKParams prm, LofStreamState* __restrict__ state, const uint32_t* __restrict__ hist,
+                uint32_t* __restrict__ ctr, float* __restrict__ cand, uint32_t n_chunks, uint32_t cpb, uint32_t n_blk) {
+  __shared__ uint32_t sh_cnt[256];
+  __shared__ uint32_t sh_sel[2];
   const uint32_t sl = blockIdx.x / n_blk;
   const uint32_t blk = blockIdx.x - sl * n_blk;
   const uint32_t s = prm.s0 + sl;
   LofStreamState& st = state[s];
-  if (st.fallback) return;
   const uint64_t N = (uint64_t)prm.C * prm.T;
   const uint64_t base = (uint64_t)s * N;
+  const uint32_t* gh = hist + (size_t)sl * LOF_LR_NBINS;
+  // every CTA of the stream finds the median's bin itself (same histogram, same result)
+  lof_lr_find_bin(gh, (uint32_t)(N / 2), sh_cnt, sh_sel);
+  const uint32_t bin = sh_sel[0], before = sh_sel[1], n_b = gh[bin], n_bad = ctr[2 * sl];
+  const float scale = st.pl_scale, off = st.pl_off, inv = 1.0f / scale;
+  const float v0 = ((float)bin - 0.5f - off) * inv, v1 = ((float)bin + 0.5f - off) * inv;
+  const float eps = 8e-7f * (fabsf(v0) + fabsf(v1) + fabsf(off) * inv) + 8e-4f * inv;
+  const float vmid = 0.5f * (v0 + v1), vhalf = 0.5f * (v1 - v0) + eps;
+  const bool fallback = bin == 0 || bin >= LOF_LR_NBINS - 1 || n_b > LOF_LR_CAND || n_bad != 0;
+  if (blk == 0 && threadIdx.x == 0) {
+    st.bin = bin; st.before = before; st.nb = n_b; st.vmid = vmid; st.vhalf = vhalf;
+    st.nonfinite = n_bad; st.fallback = fallback ? 1u : 0u;
+  }
+  if (fallback) return;
   const uint64_t lo = (uint64_t)blk * cpb * LOF_STATS_CHUNK;
   const uint64_t hi = min(N, lo + (uint64_t)cpb * LOF_STATS_CHUNK);
-  const float vmid = st.vmid, vhalf = st.vhalf, scale = st.pl_scale, off = st.pl_off;
-  const uint32_t bin = st.bin;
+  uint32_t* ncand = ctr + 2 * sl + 1;
+
   float* cl = cand + (size_t)sl * LOF_LR_CAND;
   auto take = [&](float x) {
     if (fabsf(x - vmid) <= vhalf && lof_lr_bin(x, scale, off) == bin) {
-      const uint32_t slot = atomicAdd(&st.ncand, 1u);
+      const uint32_t slot = atomicAdd(ncand, 1u);
       if (slot < LOF_LR_CAND) cl[slot] = x;
     }
   };
@@ -313,8 +298,9 @@ __device__ float lof_lr_radix_select(Ld ld, uint64_t n, uint32_t rank, uint32_t*
 
 template <class In>
 __global__ void __launch_bounds__(256)
-lof_k_lr_select2(In in, LofKParams prm, LofStreamState* __restrict__ state, const float* __restrict__ cand,
-                 lof_stream_stats* __restrict__ stats) {
+lof_k_lr_select2(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_t* __restrict__ hist,
+                 uint32_t* __restrict__ ctr, const double* __restrict__ partial, uint32_t n_chunks,
+                 const float* __restrict__ cand, lof_stream_stats* __restrict__ stats) {
   __shared__ uint32_t sh_hist[2048];
   __shared__ uint32_t sh_cnt[256];
   __shared__ uint32_t sh_sel[2];
@@ -324,9 +310,39 @@ lof_k_lr_select2(In in, LofKParams prm, LofStreamState* __restrict__ state, cons
   const uint64_t N = (uint64_t)prm.C * prm.T;
   const uint64_t base = (uint64_t)s * N;
   LofStreamState& st = state[s];
+  const int tid = threadIdx.x;
+  // chunk partials reduced in a fixed order: each thread a contiguous run of chunks, then a fixed tree
+  {
+    const uint32_t per = (n_chunks + 255) / 256;
+    double a = 0.0, q = 0.0;
+    for (uint32_t c = tid * per; c < min(n_chunks, (tid + 1) * per); ++c) {
+      a += partial[((size_t)sl * n_chunks + c) * 2 + 0];
+      q += partial[((size_t)sl * n_chunks + c) * 2 + 1];
+    }
+    a = lof_block_sum(a, sh_red);
+    q = lof_block_sum(q, sh_red);
+    if (tid == 0) {
+      const double n = (double)N;
+      double var = (q - a * a / n) / n;
+      if (!(var > 0.0)) var = 0.0;
+      st.sum = a; st.sumsq = q;
+      st.mean = st.shift + a / n;
+      st.stddev = sqrt(var);
+      sh_sel[0] = (isfinite(a) && isfinite(q)) ? 0u : 1u;
+    }
+    __syncthreads();
+  }
+  const bool sums_bad = sh_sel[0] != 0;
   const uint32_t rank = (uint32_t)(N / 2);
-  const uint32_t nc = st.ncand, before = st.before, nb = st.nb, fb = st.fallback;
-  const bool direct = fb != 0 || nc != nb || nc > LOF_LR_CAND || before > rank || rank - before >= nc;
+  const uint32_t nc = ctr[2 * sl + 1], before = st.before, nb = st.nb, fb = st.fallback;
+  __syncthreads();
+  // leave the slot's histogram and counters zeroed for the next group that uses it
+  {
+    uint32_t* gh = hist + (size_t)sl * LOF_LR_NBINS;
+    for (int b = tid; b < LOF_LR_NBINS; b += 256) gh[b] = 0;
+    if (tid < 2) ctr[2 * sl + tid] = 0;
+  }
+  const bool direct = fb != 0 || sums_bad || nc != nb || nc > LOF_LR_CAND || before > rank || rank - before >= nc;
   float median;
   if (!direct) {
     const float* cl = cand + (size_t)sl * LOF_LR_CAND;
