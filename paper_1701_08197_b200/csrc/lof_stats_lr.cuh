@@ -21,6 +21,7 @@
 
 #define LOF_LR_NBINS 4096
 #define LOF_LR_CAND 32768          // candidate list entries per stream
+#define LOF_LR_CTA_LIST 1024       // candidates a gather CTA collects before it reserves list space
 #define LOF_LR_STAGE 8192          // ... of which this many can be selected from shared memory
 
 __device__ __forceinline__ uint32_t lof_lr_bin(float x, float scale, float off) {
@@ -213,10 +214,20 @@ lof_k_lr_gather(In in, LofKParams prm, LofStreamState* __restrict__ state, const
   uint32_t* ncand = ctr + 2 * sl + 1;
 
   float* cl = cand + (size_t)sl * LOF_LR_CAND;
+  // candidates are collected per CTA in shared memory and appended with one reservation per CTA: thousands of
+  // atomics on the one list counter of a stream serialise in L2 (measured: 37 us instead of 10)
+  __shared__ float sh_list[LOF_LR_CTA_LIST];
+  __shared__ uint32_t sh_n, sh_base;
+  if (threadIdx.x == 0) sh_n = 0;
+  __syncthreads();
   auto take = [&](float x) {
     if (fabsf(x - vmid) <= vhalf && lof_lr_bin(x, scale, off) == bin) {
-      const uint32_t slot = atomicAdd(ncand, 1u);
-      if (slot < LOF_LR_CAND) cl[slot] = x;
+      const uint32_t slot = atomicAdd(&sh_n, 1u);
+      if (slot < LOF_LR_CTA_LIST) sh_list[slot] = x;
+      else {                                              // CTA list full: straight to the stream's list
+        const uint32_t g = atomicAdd(ncand, 1u);
+        if (g < LOF_LR_CAND) cl[g] = x;
+      }
     }
   };
   uint64_t i = lo;
@@ -245,6 +256,12 @@ lof_k_lr_gather(In in, LofKParams prm, LofStreamState* __restrict__ state, const
     i = hi4;
   }
   for (uint64_t j = i + threadIdx.x; j < hi; j += LOF_STATS_THREADS) take(in.ld(base + j));
+  __syncthreads();
+  const uint32_t n_loc = min(sh_n, (uint32_t)LOF_LR_CTA_LIST);
+  if (threadIdx.x == 0 && n_loc) sh_base = atomicAdd(ncand, n_loc);
+  __syncthreads();
+  for (uint32_t k = threadIdx.x; k < n_loc; k += LOF_STATS_THREADS)
+    if (sh_base + k < LOF_LR_CAND) cl[sh_base + k] = sh_list[k];
 }
 
 // Exact rank-`rank` element of n values by a 3-pass radix select (11 + 11 + 10 bits of the key), one CTA of
