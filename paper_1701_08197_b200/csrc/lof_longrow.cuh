@@ -61,11 +61,24 @@ lof_k_time_seg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
   const uint32_t t_lo = o_lo >= H ? o_lo - H : 0;        // multiple of 32
   float* sg = stage[warp];
   const uint64_t base = row * T;
+  if ((T & 3) == 0) {
+    // 16-byte loads, eight in flight per lane (t_lo is a multiple of 32, the row start of 4 when T is)
+    float4* sg4 = reinterpret_cast<float4*>(sg);
+#pragma unroll
+    for (int q = 0; q < LOF_LR_TILE / 128; ++q) {
+      const int g = q * 32 + lane;
+      const uint32_t t = t_lo + 4 * g;
+      float v[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};   // beyond the row: never flagged, kills windows
+      if (t < T) in.ld4(base + t, v);
+      sg4[g ^ ((g >> 3) & 7)] = make_float4(v[0], v[1], v[2], v[3]);
+    }
+  } else {
 #pragma unroll 4
-  for (int q = 0; q < LOF_LR_TILE / 32; ++q) {
-    const int i = q * 32 + lane;
-    const uint32_t t = t_lo + i;
-    sg[lof_lr_swz(i)] = t < T ? in.ld(base + t) : -INFINITY;   // beyond the row: never flagged, kills windows
+    for (int q = 0; q < LOF_LR_TILE / 32; ++q) {
+      const int i = q * 32 + lane;
+      const uint32_t t = t_lo + i;
+      sg[lof_lr_swz(i)] = t < T ? in.ld(base + t) : -INFINITY;
+    }
   }
   __syncwarp();
   float x[32];
@@ -221,11 +234,23 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
   const uint32_t t_lo = (o_lo >= H ? o_lo - H : 0) + warp * LOF_LR_TILE;   // this warp's strip
   float* sg = sm.stage[warp];
   const uint64_t base = row * T;
+  if ((T & 3) == 0) {
+    float4* sg4 = reinterpret_cast<float4*>(sg);
+#pragma unroll
+    for (int q = 0; q < LOF_LR_TILE / 128; ++q) {
+      const int g = q * 32 + lane;
+      const uint32_t t = t_lo + 4 * g;
+      float v[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+      if (t < T) in.ld4(base + t, v);
+      sg4[g ^ ((g >> 3) & 7)] = make_float4(v[0], v[1], v[2], v[3]);
+    }
+  } else {
 #pragma unroll 4
-  for (int q = 0; q < LOF_LR_TILE / 32; ++q) {
-    const int i = q * 32 + lane;
-    const uint32_t t = t_lo + i;
-    sg[lof_lr_swz(i)] = t < T ? in.ld(base + t) : -INFINITY;
+    for (int q = 0; q < LOF_LR_TILE / 32; ++q) {
+      const int i = q * 32 + lane;
+      const uint32_t t = t_lo + i;
+      sg[lof_lr_swz(i)] = t < T ? in.ld(base + t) : -INFINITY;
+    }
   }
   __syncwarp();
   float x[32];
