@@ -114,8 +114,12 @@ lof_k_lr_hist(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_
           for (int r = 0; r < 8; ++r) {
             const float x = xv[8 * g + r], d = x - K;
             ga += d; gq = fmaf(d, d, gq);
-            bad += lof_finite(x) ? 0u : 1u;
             atomicAdd(&sh_hist[lof_lr_bin(x, scale, off)], 1u);
+          }
+          // a non-finite sample makes its group's sums non-finite: count exactly only then
+          if (!lof_finite(ga) || !lof_finite(gq)) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) bad += lof_finite(xv[8 * g + r]) ? 0u : 1u;
           }
           sum += (double)ga; sumsq += (double)gq;
         }
