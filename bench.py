@@ -41,8 +41,9 @@ def measured_traffic(config):
     if os.path.exists(p):
         for r in csv.DictReader(open(p)):
             if r["config"] == config:
-                return float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]), r["kernel"]
-    return None, None
+                return float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]), r["kernel"], \
+                    float(r.get("thread_instr_per_sample") or 0) or None
+    return None, None, None
 
 
 def make_workload(name, seed=0):
@@ -247,7 +248,7 @@ def run_gpu(args):
     peak, peak_src = measured_peaks()
     ms_step = total_ms / args.steps
     achieved = n_samples * ALGO_BYTES_PER_SAMPLE / (ms_step * 1e-3) / 1e9
-    traffic, kname = measured_traffic(args.config)
+    traffic, kname, tips = measured_traffic(args.config)
     one_kernel = launches in (args.steps, 3 * args.steps)     # fused: 1 launch per step (+2 history kernels)
     cpu_val, cores, sample = oracle_rate(power, kw)
     line = {
@@ -270,6 +271,17 @@ def run_gpu(args):
                      "algorithmic_bytes_per_sample": ALGO_BYTES_PER_SAMPLE},
         "cpu_baseline": {"value": cpu_val / 1e9, "unit": "Gsamples/s", "cores": cores, "kind": "oracle", "sample": sample},
     }
+    if tips:
+        # the roof this kernel is actually pressed against: instruction issue.  Executed
+        # thread-instructions per sample from the committed ncu capture x the live rate, against
+        # SMs x 4 schedulers x 32 lanes x the SM clock sampled during the run
+        import torch
+        sms = torch.cuda.get_device_properties(0).multi_processor_count
+        mhz = line["clocks"].get("sm_mhz") or line["clocks"].get("sm_max_mhz") or 1965.0
+        peak_i = sms * 4 * 32 * mhz * 1e6
+        line["roofline"]["issue"] = {"thread_instr_per_sample": tips, "achieved": value * 1e9 * tips / world,
+                                     "peak": peak_i, "unit": "thread-instr/s",
+                                     "frac": value * 1e9 * tips / world / peak_i}
     print(json.dumps(line))
     f.close()
     if dist:

@@ -286,3 +286,33 @@ def test_fused_counters_account_for_every_stream(lof, wl):
     f.close()
     assert sum(c) == w.S and c[3] == 0, c
     assert c[0] >= w.S - 1, c          # noise-like streams: the median comes from the rank count in its bin
+
+
+@pytest.mark.parametrize("shape", ["fused64", "fused16", "longrow"])
+def test_repeated_runs_are_bit_identical(lof, wl, shape):
+    """The statistics are summed in a fixed order and every flag decision is deterministic: the same block
+    flagged five times (dynamic hand-out of columns and rows, atomics on histograms and candidate lists in
+    between) gives the same bytes, flags and statistics alike."""
+    import torch
+    if shape == "fused64":
+        w = wl.config2(5, n_stations=40); x, C, T, mw = w.power, w.C, w.T, 64          # 80 streams
+    elif shape == "fused16":
+        w = wl.config3(5, n_stations=12); x, C, T, mw = w.power, w.C, w.T, 64
+    else:
+        rng = np.random.default_rng(9)
+        x = rng.standard_exponential((6, 16, 12208)).astype(np.float32); C, T, mw = 16, 12208, 64
+        x[2, 3, 100:400] += 5.0
+    S = x.shape[0]
+    f = lof.Flagger(S, C, T, max_window=mw)
+    xd = torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    ref = None
+    for _ in range(5):
+        flags, stats = f.flag_block(xd)
+        torch.cuda.synchronize()
+        rs, rc = f.row_sums()
+        got = (lof.flags_to_numpy(flags).tobytes(), stats.cpu().numpy().tobytes(), rs.cpu().numpy().tobytes(),
+               rc.cpu().numpy().tobytes())
+        if ref is None:
+            ref = got
+        assert got == ref
+    f.close()
