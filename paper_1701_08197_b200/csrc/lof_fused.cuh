@@ -839,9 +839,8 @@ __device__ __forceinline__ void lof_row_flag(const float (&x)[L], uint32_t& fb, 
   __half2 e2[L / 2];
   const float T0 = thr[0];
   int k_next = 1;
-  bool again = true;
 #pragma unroll 1
-  while (again) {
+  for (;;) {
     // level 0 (I = 1) under the current mask: x > threshold_1 on samples not yet flagged
     {
       // four independent partial masks: no serial chain through fb
@@ -854,19 +853,21 @@ __device__ __forceinline__ void lof_row_flag(const float (&x)[L], uint32_t& fb, 
     }
 #pragma unroll
     for (int m = 0; m < L / 2; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
-    again = false;
     if (k_next == 1) after_level0();
     if (__all_sync(0xffffffffu, fb == maskL)) break;     // nothing left to test in this row
+    // one test per level on the way down: past the last level -> done; new flags with levels to go ->
+    // back to level 0 under the new mask (continue), re-doubling up to k_next without testing
 #define LOF_ROW_LEVEL(K)                                                                 \
-    if (K < nlt && !again) {                                                             \
-      lof_row_step<L, (1 << (K - 1))>(u, e2, lane);                                      \
-      if (K >= k_next && lof_row_eval<L, K>(u, e2, lane, thr[K], fb) && K + 1 < nlt) {   \
-        again = true; k_next = K + 1; LOF_PROF_CNT(7);                                    \
-      }                                                                                  \
+    if (K >= nlt) break;                                                                 \
+    lof_row_step<L, (1 << (K - 1))>(u, e2, lane);                                        \
+    if (K >= k_next && lof_row_eval<L, K>(u, e2, lane, thr[K], fb) && K + 1 < nlt) {     \
+      k_next = K + 1; LOF_PROF_CNT(7);                                                    \
+      continue;                                                                          \
     }
     LOF_ROW_LEVEL(1) LOF_ROW_LEVEL(2) LOF_ROW_LEVEL(3) LOF_ROW_LEVEL(4) LOF_ROW_LEVEL(5)
     LOF_ROW_LEVEL(6) LOF_ROW_LEVEL(7) LOF_ROW_LEVEL(8) LOF_ROW_LEVEL(9)
 #undef LOF_ROW_LEVEL
+    break;
   }
 }
 
