@@ -520,9 +520,8 @@ __device__ __forceinline__ uint64_t lof_col_flag(Ld ld, const float* thr, int nl
   uint64_t fb = 0;
   const float T0 = thr[0];
   int k_next = 1;
-  bool again = true;
 #pragma unroll 1
-  while (again) {
+  for (;;) {
     // level 0 under the current mask: I = 1 is the simple thresholder x > threshold_1
     float m0 = -INFINITY, m1 = -INFINITY;
 #pragma unroll
@@ -542,16 +541,17 @@ __device__ __forceinline__ uint64_t lof_col_flag(Ld ld, const float* thr, int nl
 #pragma unroll
       for (int m = 0; m < C / 2; ++m) e2[m] = lof_h2_unflagged((uint32_t)(fb >> (2 * m)) & 3u);
     }
-    again = false;
+    // one test per level on the way down: past the last level -> done; new flags with levels to go ->
+    // back to level 0 under the new mask
 #define LOF_COL_LEVEL(K)                                                             \
-    if (K <= KMAX && K < nlf && !again) {                                            \
-      lof_col_step<C, (K <= KMAX ? K : 1)>(u, e2);                                   \
-      if (K >= k_next && lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e2, thr[K], fb) &&  \
-          K + 1 <= KMAX && K + 1 < nlf) { again = true; k_next = K + 1; }            \
-    }
+    if (K > KMAX || K >= nlf) break;                                                 \
+    lof_col_step<C, (K <= KMAX ? K : 1)>(u, e2);                                     \
+    if (K >= k_next && lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e2, thr[K], fb) &&    \
+        K + 1 <= KMAX && K + 1 < nlf) { k_next = K + 1; LOF_PROF_CNT(6); continue; }
     LOF_COL_LEVEL(1) LOF_COL_LEVEL(2) LOF_COL_LEVEL(3) LOF_COL_LEVEL(4)
     LOF_COL_LEVEL(5) LOF_COL_LEVEL(6) LOF_COL_LEVEL(7) LOF_COL_LEVEL(8)
 #undef LOF_COL_LEVEL
+    break;
   }
   return fb;
 }
@@ -672,9 +672,8 @@ __device__ __forceinline__ uint32_t lof_pcol_flag(Ld ld, const float* thr, int n
   uint32_t fb = 0;
   const float T0 = thr[0];
   int k_next = 1;
-  bool again = true;
 #pragma unroll 1
-  while (again) {
+  for (;;) {
     float m0 = -INFINITY, m1 = -INFINITY;
 #pragma unroll
     for (int j = 0; j < 32; j += 2) {
@@ -692,23 +691,23 @@ __device__ __forceinline__ uint32_t lof_pcol_flag(Ld ld, const float* thr, int n
 #pragma unroll
       for (int m = 0; m < 16; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
     }
-    again = false;
 #define LOF_PCOL_LEVEL(K)                                                          \
-    if (K < nlf && !again) {                                                       \
-      lof_pcol_step<(1 << (K - 1))>(u, e2, h);                                     \
-      if (K >= k_next && lof_pcol_eval<K>(u, e2, h, thr[K], fb) && K + 1 < nlf) {  \
-        again = true; k_next = K + 1; LOF_PROF_CNT(6);                              \
-      }                                                                            \
+    if (K >= nlf) break;                                                           \
+    lof_pcol_step<(1 << (K - 1))>(u, e2, h);                                       \
+    if (K >= k_next && lof_pcol_eval<K>(u, e2, h, thr[K], fb) && K + 1 < nlf) {    \
+      k_next = K + 1; LOF_PROF_CNT(6);                                              \
+      continue;                                                                    \
     }
     LOF_PCOL_LEVEL(1) LOF_PCOL_LEVEL(2) LOF_PCOL_LEVEL(3) LOF_PCOL_LEVEL(4) LOF_PCOL_LEVEL(5)
 #undef LOF_PCOL_LEVEL
-    if (6 < nlf && !again && 6 >= k_next) {
+    if (6 < nlf) {
       // I = 64: the one window that is the whole column
       const float ub = __shfl_xor_sync(0xffffffffu, u[0], 16);
       const float eb = __shfl_xor_sync(0xffffffffu, __low2float(e2[0]), 16);
       const float v = (u[0] + ub) - (__low2float(e2[0]) + eb) * thr[6];
       if (v > 0.f) fb = 0xFFFFFFFFu;             // both lanes of the pair see the same v
     }
+    break;
   }
   return fb;
 }
