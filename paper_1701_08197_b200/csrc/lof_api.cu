@@ -166,10 +166,14 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
 
   const uint64_t N = (uint64_t)C * T;
   c->n_chunks = (uint32_t)((N + LOF_STATS_CHUNK - 1) / LOF_STATS_CHUNK);
-  // groups: keep one group's input (read four to five times by the generic path) inside L2
-  const uint64_t group_bytes = 80ull << 20;
+  // groups of streams per launch sequence.  Measured on B200: groups small enough to stay in L2 (80 MB, so
+  // that the five kernels of a group re-read the input from L2) were 23 % SLOWER than groups of 640 MB — the
+  // kernels are bound by instruction issue, not by bandwidth, and every launch of a small group pays its ramp
+  // and its tail.  The bound below only limits the per-group scratch (histograms, candidate lists, partials).
+  const uint64_t group_bytes = 640ull << 20;
   uint64_t g = group_bytes / (N * 4);
   if (g < 1) g = 1;
+  if (g > 1024) g = 1024;
   if (g > S) g = S;
   c->group = (uint32_t)g;
   // time tiling: halo = dependency cone sum_k (2^k - 1) of the time run, rounded up to 32
