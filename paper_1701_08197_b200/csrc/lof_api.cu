@@ -233,9 +233,9 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
     kp.s0 = s0;
     const uint32_t nb = G * c->n_chunks;
     if (c->path == 0) {
-      // two passes over the group's input, three launches (lof_stats_lr.cuh): about four CTAs per SM, each
+      // two passes over the group's input, three launches (lof_stats_lr.cuh): about twelve CTAs per SM over the launch, each
       // over consecutive chunks of one stream
-      uint32_t cpb = (nb + (uint32_t)c->sm_count * 4 - 1) / ((uint32_t)c->sm_count * 4);
+      uint32_t cpb = (nb + (uint32_t)c->sm_count * 12 - 1) / ((uint32_t)c->sm_count * 12);
       if (cpb < 1) cpb = 1;
       const uint32_t n_blk = (c->n_chunks + cpb - 1) / cpb;
       if (c->lr_dirty) {        // the radix passes of path 1 used the slots' histograms since the last group here
