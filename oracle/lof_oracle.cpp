@@ -111,10 +111,13 @@ void lofo_sumthreshold_1d_fast(const float* x, uint64_t n, int64_t stride, uint8
   }
 }
 
+// PAPER.md:75 "we may have to compute amplitudes first"; reading S5: x = re^2 + im^2 formed as an
+// integer (at most 2 * 32768^2 = 2^31, so 64-bit arithmetic keeps (-32768, -32768) defined) and
+// converted to float32 once, round-to-nearest.
 void lofo_power_from_ci16(const int16_t* volt, uint64_t n, float* power) {
   for (uint64_t i = 0; i < n; ++i) {
-    const int32_t re = volt[2 * i], im = volt[2 * i + 1];
-    power[i] = (float)(uint32_t)(re * re + im * im);   // integer-exact (S5)
+    const int64_t re = volt[2 * i], im = volt[2 * i + 1];
+    power[i] = (float)(re * re + im * im);
   }
 }
 

@@ -11,7 +11,10 @@ from concurrent.futures import ThreadPoolExecutor
 import numpy as np
 
 _DIR = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_DIR, "liblof_oracle.so")
+# LOFO_SANITIZE=1: a second build with -fsanitize=address,undefined (tests/test_oracle_sanitizers.py runs the
+# pins against it in a subprocess that preloads libasan)
+_SAN = bool(os.environ.get("LOFO_SANITIZE"))
+_SO = os.path.join(_DIR, "liblof_oracle_san.so" if _SAN else "liblof_oracle.so")
 _SRC = [os.path.join(_DIR, "lof_oracle.cpp"), os.path.join(_DIR, "lof_oracle.h")]
 MARGIN_REL = 1e-5     # north_star: "window sum lies within 1e-5 relative of its threshold"
 
@@ -19,8 +22,8 @@ MARGIN_REL = 1e-5     # north_star: "window sum lies within 1e-5 relative of its
 def build(force=False):
     """g++ -O2 build of the oracle shared library (building the checker is not using it)."""
     if force or not os.path.exists(_SO) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in _SRC):
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-Wall",
-                               "-o", _SO, _SRC[0]])
+        san = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] if _SAN else ["-O2"]
+        subprocess.check_call(["g++"] + san + ["-std=c++17", "-fPIC", "-shared", "-Wall", "-o", _SO, _SRC[0]])
     return _SO
 
 

@@ -342,3 +342,68 @@ def test_history_buffer_sizing_arithmetic():
     assert pre == 16252928 and round(pre / 2 ** 20, 1) == 15.5
     assert round(pre * 300 / 2 ** 30, 1) == 4.5
     assert round(post / 2 ** 20) == 504 and round(post * 300 / 2 ** 30) == 148
+
+
+# ---------------------------------------------------------------- a0: power from complex int16 (reading S5)
+def test_power_from_ci16_vs_numpy_int64(lofo):
+    """x = re^2 + im^2 as an integer, converted to float32 once: pinned against numpy int64 arithmetic on
+    random pairs and on the four corners of the int16 range ((-32768, -32768) gives 2^31, which a 32-bit
+    signed sum cannot hold)."""
+    rng = np.random.default_rng(75)
+    v = rng.integers(-32768, 32768, size=(4096, 2), dtype=np.int64)
+    corners = np.array([[32767, 32767], [-32768, -32768], [-32768, 32767], [32767, -32768],
+                        [0, 0], [-1, 1], [-32768, 0], [0, 32767]], np.int64)
+    v = np.concatenate([corners, v])
+    got = lofo.power_from_ci16(v.astype(np.int16))
+    exact = v[:, 0] * v[:, 0] + v[:, 1] * v[:, 1]                  # int64: exact
+    assert got.dtype == np.float32 and got.shape == (len(v),)
+    assert np.array_equal(got, exact.astype(np.float32))           # one rounding, to nearest-even
+    assert got[1] == np.float32(2147483648.0) and got[0] == np.float32(2 * 32767 ** 2)
+    # sigma-32 data (config 4): every value is below 2^24, so the conversion is exact
+    small = np.rint(rng.normal(0, 32, size=(4096, 2))).astype(np.int64)
+    g2 = lofo.power_from_ci16(small.astype(np.int16))
+    assert np.array_equal(g2.astype(np.int64), small[:, 0] ** 2 + small[:, 1] ** 2)
+
+
+# ---------------------------------------------------------------- P2 at the row lengths the fast form is used at
+@pytest.mark.parametrize("n,levels,seed", [(20011, 9, 0), (24001, 9, 1), (12208, 7, 2)])
+def test_fast_equals_literal_long_rows(lofo, n, levels, seed):
+    """lofo_sumthreshold_1d_fast (one fp64 prefix array over the whole row) against the literal double loop
+    on rows as long as configs 4 and 5 use (T = 20 011 cut / 12 208), 9 levels, data of mean 2048 (config 4's
+    power), injected bursts and random pre-set masks."""
+    rng = np.random.default_rng(seed)
+    re = np.rint(rng.normal(0, 32, n)); im = np.rint(rng.normal(0, 32, n))
+    x = (re * re + im * im).astype(np.float32)                      # mean 2048, exponential-like
+    for _ in range(12):                                             # bursts of 3..400 samples at 1.2..6 x the mean
+        d = int(rng.integers(3, 400)); t0 = int(rng.integers(0, n - d))
+        x[t0:t0 + d] += np.float32(2048.0 * rng.uniform(0.2, 5.0))
+    pre = (rng.random(n) < rng.choice([0.0, 0.02, 0.2])).astype(np.uint8)
+    pre[n // 3: n // 3 + 700] = 1                                   # a long pre-flagged run
+    st = lofo.statistics(x)
+    thr = lofo.threshold_table(float(st["median"]), float(st["stddev"]) * 0.5, levels)
+    a, mga = lofo.sumthreshold_1d(x, thr, mask=pre, literal=True)
+    b, mgb = lofo.sumthreshold_1d(x, thr, mask=pre, literal=False)
+    assert a.sum() > pre.sum()                                      # the run did flag something new
+    assert np.array_equal(a, b)
+    assert np.array_equal(mga, mgb)                                 # same near-threshold windows marked
+
+
+# ---------------------------------------------------------------- history_sensitivity <= 0 (PAPER.md:106)
+def test_history_sensitivity_fallback_is_sensitivity(lofo):
+    """The pseudocode reuses the name `sensitivity`: history_sensitivity <= 0 means "use
+    sensitivity".  Ring [1, 2, 3]: mean 2, stddev sqrt(2/3).  With sensitivity 2 the threshold is
+    2 + 2 * 0.8165 = 3.633: cur = 3.5 passes; with an explicit history_sensitivity 1 (thr 2.8165) it is flagged."""
+    def run(sens, hsens, cur):
+        prm = lofo.make_params(1, 1, 40, sensitivity=sens, history_length=4, history_min_fill=3,
+                               history_sensitivity=hsens)
+        h = lofo.History(prm)
+        for r in (1.0, 2.0, 3.0):
+            assert _push(h, r)[0] == 0
+        rf, _ = _push(h, cur)
+        return rf, h.export()[0][0, 0, 3]
+    thr2 = 2.0 + 2.0 * math.sqrt(2.0 / 3.0)
+    assert run(2.0, 0.0, 3.5) == (0, np.float32(3.5))               # fallback: threshold 3.633
+    assert run(2.0, -1.0, 3.7) == (1, np.float32(thr2))             # negative also falls back; 3.7 >= 3.633
+    assert run(2.0, 1.0, 3.5)[0] == 1                               # explicit 1.0: threshold 2.8165
+    assert run(0.5, 0.0, 2.5)[0] == 1                               # fallback to 0.5: threshold 2.408
+    assert run(0.5, 0.0, 2.3)[0] == 0
