@@ -18,6 +18,10 @@
  *    library never frees or retains caller pointers.
  *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
  *    calls only enqueue work on it and never synchronise the host.
+ *  - A context is not thread-safe, and its calls must be ordered on ONE stream at a time: it owns the scratch
+ *    (statistics, masks, row sums, history rings) that consecutive calls reuse.  lof_flag_block_host uses a
+ *    private stream and returns after synchronising it; do not call it while device calls on the same context
+ *    are still in flight on another stream.
  *  - Flag bit of sample t of row (s, c): word (s*n_channels + c)*ceil(n_time/32) + t/32,
  *    bit t%32 (LSB first), 1 = flagged.  Padding bits of a row's last word are 0.
  *  - Return value: 0 on success, a negative LOF_E_* code otherwise; nothing throws or aborts
@@ -74,7 +78,8 @@ typedef struct {
 
 /* Validate params (LOF_E_PARAM when: struct_size mismatch; S, C or T zero; C > 256; max_window
  * zero, not a power of two or > 1024; directions zero or with unknown bits; p, sensitivity or
- * start_threshold not > 0 and finite), select the device, allocate scratch and history rings
+ * start_threshold not > 0 and finite; history_length > 0 with history_min_fill == 0 — an empty ring has no
+ * mean; history_sensitivity not finite), select the device, allocate scratch and history rings
  * (zero-filled, all rings empty).  *out receives the handle; on failure *out = NULL. */
 int lof_create(const lof_params* params, lof_ctx** out);
 
@@ -105,7 +110,8 @@ int lof_flag_block_ci16(lof_ctx* ctx, const int16_t* d_volt, uint32_t* d_flags,
  * or if history_length == 0.  Asynchronous on cuda_stream. */
 int lof_history_update(lof_ctx* ctx, uint32_t* d_flags, uint8_t* d_row_flagged, void* cuda_stream);
 
-/* Empties every history ring (asynchronous on cuda_stream). */
+/* Empties every history ring and forgets a pending block.  Takes a stream (unlike the survey's sketch
+ * lof_reset(ctx)) because, like every device call here, it only enqueues work (memsets) on cuda_stream. */
 int lof_reset(lof_ctx* ctx, void* cuda_stream);
 
 /* Copies to caller DEVICE buffers (either may be NULL) what the last lof_flag_block left in the
@@ -137,9 +143,30 @@ uint64_t lof_launch_count(const lof_ctx* ctx);
  * generic multi-kernel path.  Both compute the same results; for tests and profiling. */
 int lof_set_path(lof_ctx* ctx, int path);
 
+/* Which kernels the last lof_flag_block[_ci16] of this context ran (the steps of PAPER.md:37-47, :83 are the
+ * same on every path; only the decomposition differs):
+ *   LOF_PATH_FUSED         one kernel per block: (n_channels, n_time) in {(64,768), (32,768), (16,768), (16,256)},
+ *                          float32 input — a stream fits one SM's shared memory;
+ *   LOF_PATH_LONGROW_SEG   statistics kernels + register-resident column kernel + independent row segments
+ *                          (16/32/64 channels, dependency cone of the time run <= 256 samples);
+ *   LOF_PATH_LONGROW_COOP  same with cooperative 8192-sample row tiles (wider cones, max_window <= 512);
+ *   LOF_PATH_GENERIC       at least one step ran in the shared-memory generic kernels (any shape, several times
+ *                          slower: other channel counts, max_window 1024 on long rows, or lof_set_path(ctx, 1)).
+ * LOF_PATH_NONE before the first block; LOF_E_NULL for a NULL context. */
+#define LOF_PATH_NONE          0
+#define LOF_PATH_FUSED         1
+#define LOF_PATH_LONGROW_SEG   2
+#define LOF_PATH_LONGROW_COOP  3
+#define LOF_PATH_GENERIC       4
+int lof_path_used(const lof_ctx* ctx);
+
+/* Tests only: lowers the number of streams the multi-kernel paths process per launch sequence (the default is
+ * as many as fit 640 MB of input, at most 1024; values above that are clamped to it), so that a small block
+ * exercises the loop over several groups.  LOF_E_PARAM for 0.  Results do not depend on it. */
+int lof_set_group(lof_ctx* ctx, uint32_t max_streams_per_group);
+
 /* Diagnostics of the fused kernels (streams that fit one SM's shared memory): how the exact median
- * of each stream was found since the last reset, summed over every context of the process on the
- * context's device: h_out[0] from samples gathered during the statistics pass (the fast case),
+ * of each stream of THIS context was found since the last reset: h_out[0] from samples gathered during the statistics pass (the fast case),
  * h_out[1] by one more gather pass, h_out[2] by a radix select over the whole stream, h_out[3]
  * streams with non-finite samples.  Synchronises the device.  reset != 0 zeroes the counters. */
 int lof_fused_counters(lof_ctx* ctx, uint64_t* h_out /*[4]*/, int reset);

@@ -29,7 +29,10 @@ struct lof_ctx {
   lof_params prm;
   LofKParams kp;
   int path;                       // 0 auto, 1 force generic
+  int path_used;                  // what the last lof_flag_block ran: LOF_PATH_* (lof.h)
   int sm_count;
+  uint32_t fused_grid;            // persistent grid of the fused kernel for this shape (0: no fused instantiation)
+  uint32_t group_alloc;           // streams per group the scratch was allocated for (lof_set_group lowers `group`)
   uint64_t launches;
   bool block_pending;             // a lof_flag_block result is waiting for lof_history_update
   // geometry of the generic path
@@ -56,6 +59,7 @@ struct lof_ctx {
   float* d_ring;                  // [S][C][H]
   uint32_t* d_head; uint32_t* d_count;
   uint8_t* d_row_flagged;
+  unsigned long long* d_diag;     // per-context diagnostics of the fused kernel: [0..4) counters, [8..16) cycles
   // staging for lof_flag_block_host
   void* d_in_stage; size_t in_stage_bytes;
   uint32_t* d_flags_stage;
@@ -75,6 +79,9 @@ static int validate(const lof_params* p) {
   if (!(p->sensitivity > 0.f) || !std::isfinite(p->sensitivity)) return LOF_E_PARAM;
   if (!(p->start_threshold > 0.f) || !std::isfinite(p->start_threshold)) return LOF_E_PARAM;
   if ((uint64_t)p->n_channels * p->n_time > 0xFFFFFFFFull) return LOF_E_PARAM;
+  // an empty ring has no mean: with min_fill = 0 the first threshold would be 0/0 and every later one NaN
+  if (p->history_length > 0 && p->history_min_fill == 0) return LOF_E_PARAM;
+  if (!std::isfinite(p->history_sensitivity)) return LOF_E_PARAM;
   return LOF_OK;
 }
 
@@ -116,7 +123,7 @@ extern "C" int lof_destroy(lof_ctx* c) {
   cudaFree(c->d_state); cudaFree(c->d_hist); cudaFree(c->d_cand); cudaFree(c->d_ctr); cudaFree(c->d_partial); cudaFree(c->d_fmask);
   cudaFree(c->d_part_sum); cudaFree(c->d_part_cnt); cudaFree(c->d_rowsum); cudaFree(c->d_rowcnt);
   cudaFree(c->d_stats); cudaFree(c->d_ring); cudaFree(c->d_head); cudaFree(c->d_count);
-  cudaFree(c->d_row_flagged); cudaFree(c->d_in_stage); cudaFree(c->d_flags_stage);
+  cudaFree(c->d_row_flagged); cudaFree(c->d_diag); cudaFree(c->d_in_stage); cudaFree(c->d_flags_stage);
   if (c->host_stream) cudaStreamDestroy(c->host_stream);
   delete c;
   return LOF_OK;
@@ -134,6 +141,8 @@ static cudaError_t lof_generic_set_attributes(size_t smem_freq, size_t smem_time
   A(cudaFuncSetAttribute(lof_k_time_coop<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LofCoopSmem)));
   return e;
 }
+
+static cudaError_t fused_prepare_any(lof_ctx* c);       // below, with the fused launch
 
 static uint32_t ilog2(uint32_t v) { uint32_t k = 0; while ((1u << (k + 1)) <= v) ++k; return k; }
 
@@ -153,7 +162,14 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   if (!c) return LOF_E_CUDA;
   memset(c, 0, sizeof *c);
   c->prm = *p;
-  LOF_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, p->device));
+  {
+    cudaError_t ea = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, p->device);
+    if (ea != cudaSuccess) {
+      snprintf(g_cuda_err, sizeof g_cuda_err, "cudaDeviceGetAttribute: %s", cudaGetErrorString(ea));
+      delete c;
+      return LOF_E_CUDA;
+    }
+  }
   const uint32_t S = p->n_streams, C = p->n_channels, T = p->n_time, W = (T + 31) / 32;
   LofKParams& kp = c->kp;
   kp.S = S; kp.C = C; kp.T = T; kp.W = W;
@@ -176,6 +192,7 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   if (g > 1024) g = 1024;
   if (g > S) g = S;
   c->group = (uint32_t)g;
+  c->group_alloc = c->group;
   // time tiling: halo = dependency cone sum_k (2^k - 1) of the time run, rounded up to 32
   uint32_t cone = 0;
   for (uint32_t k = 0; k < kp.n_lev_t; ++k) cone += (1u << k) - 1;
@@ -213,7 +230,9 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   A(dev_alloc(&c->d_head, (size_t)S * C));
   A(dev_alloc(&c->d_count, (size_t)S * C));
   A(dev_alloc(&c->d_row_flagged, (size_t)S * C));
+  A(dev_alloc(&c->d_diag, (size_t)LOF_DIAG_WORDS));
   if (e == cudaSuccess) e = lof_generic_set_attributes(c->smem_freq, c->smem_time);
+  if (e == cudaSuccess) e = fused_prepare_any(c);
   if (e != cudaSuccess) {
     snprintf(g_cuda_err, sizeof g_cuda_err, "lof_create: %s", cudaGetErrorString(e));
     lof_destroy(c);
@@ -265,6 +284,7 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
       c->launches += 8;
     }
     const bool fast = c->path == 0;                     // path 1 forces the shared-memory generic kernels
+    int used = LOF_PATH_GENERIC;
     if (kp.n_lev_f) {
       const uint32_t nb_f = (uint32_t)(((uint64_t)G * kp.W + LOF_LR_WARPS - 1) / LOF_LR_WARPS);
       if (fast && c->lr_freq && C == 16)
@@ -279,12 +299,15 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
     }
     const uint32_t rows = G * C;
     uint32_t n_part;
+    const bool freq_reg = !kp.n_lev_f || (fast && c->lr_freq);
     if (fast && c->lr_time) {
+      if (freq_reg) used = LOF_PATH_LONGROW_SEG;
       n_part = c->n_seg;
       const uint32_t nb_t = (uint32_t)(((uint64_t)rows * n_part + LOF_LR_WARPS - 1) / LOF_LR_WARPS);
       lof_k_time_seg<In><<<nb_t, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum,
                                                         c->d_part_cnt, c->d_stats, c->seg_out, c->seg_halo, n_part, rows);
-    } else if (fast) {
+    } else if (fast && kp.n_lev_t <= 10) {                // the cooperative kernel exchanges windows of up to 512
+      if (freq_reg) used = LOF_PATH_LONGROW_COOP;
       n_part = c->n_co;
       lof_k_time_coop<In><<<rows * n_part, LOF_CO_WARPS * 32, sizeof(LofCoopSmem), st>>>(
           in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum, c->d_part_cnt, c->d_stats, c->co_out, c->seg_halo, n_part);
@@ -296,42 +319,58 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
     lof_k_rowsum_final<<<(rows + 255) / 256, 256, 0, st>>>(c->d_part_sum, c->d_part_cnt, c->d_rowsum, c->d_rowcnt,
                                                            (uint64_t)s0 * C, rows, n_part);
     c->launches += 2;
+    c->path_used = used;
   }
   LOF_CUDA(cudaGetLastError());
   return LOF_OK;
 }
 
 // ---- fused path: streams that fit one SM's shared memory (lof_fused.cuh)
+// Shapes with a fused instantiation, as (C, L) with T = 32 L.
+#define LOF_FUSED_SHAPES(X) X(64, 24) X(16, 24) X(32, 24) X(16, 8)
+
+// lof_create: opt the kernel of this shape in to its shared memory and size the persistent grid (SMs x CTAs per
+// SM) once; both are per device, so every context does it for its own device (idempotent, no shared state).
 template <int C, int L>
-static cudaError_t fused_launch(lof_ctx* c, const float* d_power, uint32_t* d_flags, cudaStream_t st) {
+static cudaError_t fused_prepare(lof_ctx* c) {
   using Cfg = LofFusedCfg<C, L>;
-  static bool attr_done[64] = {};
-  cudaError_t e = cudaSuccess;
-  if (!attr_done[c->prm.device & 63]) {
-    e = cudaFuncSetAttribute(lof_k_fused<C, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes);
-    if (e != cudaSuccess) return e;
-    attr_done[c->prm.device & 63] = true;
-  }
+  cudaError_t e = cudaFuncSetAttribute(lof_k_fused<C, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes);
+  if (e != cudaSuccess) return e;
   int per_sm = 1;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lof_k_fused<C, L>, Cfg::NT, Cfg::smem_bytes);
   if (e != cudaSuccess) return e;
   if (per_sm < 1) per_sm = 1;
   uint32_t grid = (uint32_t)(c->sm_count * per_sm);
   if (grid > c->prm.n_streams) grid = c->prm.n_streams;
-  lof_k_fused<C, L><<<grid, Cfg::NT, Cfg::smem_bytes, st>>>(d_power, d_flags, c->d_stats, c->d_rowsum, c->d_rowcnt, c->kp);
-  c->launches += 1;
-  return cudaGetLastError();
+  c->fused_grid = grid;
+  return cudaSuccess;
+}
+
+static cudaError_t fused_prepare_any(lof_ctx* c) {
+  const uint32_t C = c->prm.n_channels, T = c->prm.n_time;
+  c->fused_grid = 0;
+#define X(CC, LL) if (C == CC && T == 32 * LL) return fused_prepare<CC, LL>(c);
+  LOF_FUSED_SHAPES(X)
+#undef X
+  return cudaSuccess;
 }
 
 // returns 1 if the shape has a fused instantiation and it was launched, 0 if not, <0 on error
 static int flag_block_fused(lof_ctx* c, const float* d_power, uint32_t* d_flags, cudaStream_t st) {
   const uint32_t C = c->prm.n_channels, T = c->prm.n_time;
-  cudaError_t e;
-  if (C == 64 && T == 768) e = fused_launch<64, 24>(c, d_power, d_flags, st);
-  else if (C == 16 && T == 768) e = fused_launch<16, 24>(c, d_power, d_flags, st);
-  else if (C == 32 && T == 768) e = fused_launch<32, 24>(c, d_power, d_flags, st);
-  else if (C == 16 && T == 256) e = fused_launch<16, 8>(c, d_power, d_flags, st);
-  else return 0;
+  if (!c->fused_grid) return 0;
+  bool done = false;
+#define X(CC, LL)                                                                                              \
+  if (!done && C == CC && T == 32 * LL) {                                                                      \
+    lof_k_fused<CC, LL><<<c->fused_grid, LofFusedCfg<CC, LL>::NT, LofFusedCfg<CC, LL>::smem_bytes, st>>>(      \
+        d_power, d_flags, c->d_stats, c->d_rowsum, c->d_rowcnt, c->kp, c->d_diag);                             \
+    done = true;                                                                                               \
+  }
+  LOF_FUSED_SHAPES(X)
+#undef X
+  if (!done) return 0;
+  c->launches += 1;
+  const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     snprintf(g_cuda_err, sizeof g_cuda_err, "fused launch: %s", cudaGetErrorString(e));
     return LOF_E_CUDA;
@@ -348,6 +387,7 @@ static int flag_block_any(lof_ctx* c, In in, uint32_t* d_flags, lof_stream_stats
   LOF_CUDA(cudaSetDevice(c->prm.device));
   int rc = c->path == 0 ? flag_block_fused(c, in.p, d_flags, st) : 0;
   if (rc < 0) return rc;
+  if (rc == 1) c->path_used = LOF_PATH_FUSED;
   if (rc == 0) { rc = flag_block_generic(c, in, d_flags, st); if (rc) return rc; }
   if (d_stats)
     LOF_CUDA(cudaMemcpyAsync(d_stats, c->d_stats, (size_t)c->prm.n_streams * sizeof(lof_stream_stats),
@@ -453,13 +493,15 @@ extern "C" int lof_fused_counters(lof_ctx* c, uint64_t* h_out, int reset) {
   if (!c || !h_out) return LOF_E_NULL;
   LOF_CUDA(cudaSetDevice(c->prm.device));
   LOF_CUDA(cudaDeviceSynchronize());
-  unsigned long long v[4] = {0, 0, 0, 0};
-  LOF_CUDA(cudaMemcpyFromSymbol(v, lof_fused_counters_dev, sizeof v));
+  unsigned long long v[LOF_DIAG_WORDS];
+  LOF_CUDA(cudaMemcpy(v, c->d_diag, sizeof v, cudaMemcpyDeviceToHost));
   for (int i = 0; i < 4; ++i) h_out[i] = v[i];
   if (reset) {
+    LOF_CUDA(cudaMemset(c->d_diag, 0, sizeof v));
+#ifdef LOF_FUSED_PROF
     const unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    LOF_CUDA(cudaMemcpyToSymbol(lof_fused_counters_dev, z, 4 * sizeof z[0]));
     LOF_CUDA(cudaMemcpyToSymbol(lof_fused_cycles_dev, z, sizeof z));
+#endif
   }
   return LOF_OK;
 }
@@ -468,9 +510,12 @@ extern "C" int lof_fused_cycles(lof_ctx* c, uint64_t* h_out) {
   if (!c || !h_out) return LOF_E_NULL;
   LOF_CUDA(cudaSetDevice(c->prm.device));
   LOF_CUDA(cudaDeviceSynchronize());
+  for (int i = 0; i < 8; ++i) h_out[i] = 0;
+#ifdef LOF_FUSED_PROF
   unsigned long long v[8];
   LOF_CUDA(cudaMemcpyFromSymbol(v, lof_fused_cycles_dev, sizeof v));
   for (int i = 0; i < 8; ++i) h_out[i] = v[i];
+#endif
   return LOF_OK;
 }
 
@@ -478,5 +523,14 @@ extern "C" int lof_set_path(lof_ctx* c, int path) {
   if (!c) return LOF_E_NULL;
   if (path < 0 || path > 1) return LOF_E_PARAM;
   c->path = path;
+  return LOF_OK;
+}
+
+extern "C" int lof_path_used(const lof_ctx* c) { return c ? c->path_used : LOF_E_NULL; }
+
+extern "C" int lof_set_group(lof_ctx* c, uint32_t max_streams) {
+  if (!c) return LOF_E_NULL;
+  if (max_streams == 0) return LOF_E_PARAM;
+  c->group = max_streams < c->group_alloc ? max_streams : c->group_alloc;
   return LOF_OK;
 }

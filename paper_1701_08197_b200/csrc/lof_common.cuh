@@ -15,6 +15,8 @@ struct LofStreamState {
   double   mean, stddev;
   double   thr_d[LOF_MAX_LEVELS];  // threshold_I, fp64
   float    thr_f[LOF_MAX_LEVELS];  // same rounded to fp32: what the flag kernels compare against
+  float    dead_f[LOF_MAX_LEVELS]; // early-exit levels of the frequency run (lof_dead_level), one per iteration
+  float    dead_t[LOF_MAX_LEVELS]; // ... of the time run
   uint32_t nonfinite;
   uint32_t prefix;                 // radix select: key bits fixed so far
   uint32_t rank;                   // rank still to find among keys matching prefix
@@ -80,6 +82,28 @@ struct InCI16 {
   }
   static constexpr int kBytes = 4;
 };
+
+// Early exit of a SumThreshold run.  A window of 2^k samples is a disjoint union of windows
+// of 2^j samples (j < k), and it fires only if the sum over its unflagged samples of (x - threshold_k) is
+// positive (reading F7) — so at least one of those smaller windows has an unflagged mean above
+// threshold_k.  Hence: if after iteration j NO window of 2^j samples has an unflagged mean above
+// D_j = min over the iterations k still to come of threshold_k, none of them can flag anything and the run
+// stops.  The test is exact; D_j is lowered by 2e-6 relative so that the fp32 rounding of the doubled sums
+// (<= 10 additions, 6e-7 relative) and of the thresholds can never turn a skipped window into a firing one: the
+// result is bit-identical to running every iteration.  A non-positive D_j disables the exit (-huge).
+__device__ __forceinline__ float lof_dead_level(double median, double stddev, const double* factor, double sens,
+                                                uint32_t j, uint32_t n_lev) {
+  double tmin = 1e300;
+  for (uint32_t k = j + 1; k < n_lev; ++k) tmin = fmin(tmin, median + stddev * factor[k] * sens);
+  if (j + 1 >= n_lev) return 3.0e38f;                    // no iteration left: nothing can fire
+  return tmin > 0.0 ? (float)(tmin * (1.0 - 2e-6)) : -1.0e34f;
+}
+
+__device__ __forceinline__ float lof_max3(float a, float b, float c) {
+  float d;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));   // FMNMX3: one issue slot, sm_100+
+  return d;
+}
 
 // Deterministic block reduction of a double (fixed shuffle tree, then warp 0 in warp order).
 __device__ __forceinline__ double lof_warp_sum(double v) {

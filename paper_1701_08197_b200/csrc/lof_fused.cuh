@@ -5,7 +5,7 @@
 // single HBM read of the stream and a single write of its flag words:
 //   load stream -> shared memory                                    (4 B/sample from HBM)
 //   S: statistics: shifted fp32 group sums folded into fp64;
-//      exact median by a 1024-bin value histogram around the estimated centre, then an exact
+//      exact median by a 4096-bin value histogram around the estimated centre, then an exact
 //      rank count among the few samples of the median's bin (radix select as the fallback)
 //   F: SumThreshold along frequency: a thread per time column, the
 //      column's C window sums in registers, doubled in place level by level
@@ -46,7 +46,7 @@ struct LofFusedCfg {
 #endif
   static constexpr size_t smem_bytes =
       (size_t)N * 4 + (size_t)C * W * 4 + LOF_F_NBINS * 4 + LOF_F_CAP * 4 + 64 * 8 + (size_t)3 * C * 8 +
-      64 * 4 + 256 * 4;
+      (48 + 48) * 4 + 256 * 4;
 };
 
 struct LofFusedSmem {
@@ -64,7 +64,7 @@ struct LofFusedSmem {
     s.rowpart = s.red + 64;
     s.rowbar = reinterpret_cast<unsigned long long*>(s.rowpart + 2 * C);
     s.thr = reinterpret_cast<float*>(s.rowbar + C);
-    s.ctl = reinterpret_cast<uint32_t*>(s.thr + 16);
+    s.ctl = reinterpret_cast<uint32_t*>(s.thr + 48);      // thr[0..16) thresholds, [16..32) / [32..48) early-exit levels
     s.part = s.ctl + 48;
     return s;
   }
@@ -72,14 +72,16 @@ struct LofFusedSmem {
 // ctl slots
 enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS, CT_NFLAG, CT_BAD, CT_SELP, CT_SELACC, CT_PREFIX, CT_RANK, CT_FOUND, CT_SROW = 13 };
 
-// how the median of each stream was found: [0] rank count among the samples of the median's bin, [1] radix
-// select among them (a crowded bin), [2] radix select over the whole stream, [3] stream with non-finite samples
-// (diagnostics, lof_fused_counters)
-__device__ unsigned long long lof_fused_counters_dev[4];
-// cycles of thread 0 per phase, summed over CTAs and streams, when built with -DLOF_FUSED_PROF (bench/profiling
-// only): [0] first load + statistics, [1] frequency pass, [2] plan of the next stream, [3] time pass with
-// the next stream's row statistics, [4] end of the next stream's statistics
+// Diagnostics live in a context-owned array `diag` (LOF_DIAG_WORDS words, lof_fused_counters): how the median of
+// each stream was found: [0] rank count among the samples of the median's bin, [1] radix select among them (a
+// crowded bin), [2] radix select over the whole stream, [3] stream with non-finite samples.
+#define LOF_DIAG_WORDS 16
+// cycles of thread 0 per phase, summed over CTAs and streams, when built with -DLOF_FUSED_PROF (profiling builds
+// only; process-global): [0] first load + statistics, [1] frequency pass, [2] plan of the next stream, [3] time
+// pass with the next stream's row statistics, [4] end of the next stream's statistics
+#ifdef LOF_FUSED_PROF
 __device__ unsigned long long lof_fused_cycles_dev[8];
+#endif
 #ifdef LOF_FUSED_PROF
 #define LOF_PROF_T(var) const long long var = clock64()
 #define LOF_PROF_ADD(i, a, b) do { if (threadIdx.x == 0) atomicAdd(&lof_fused_cycles_dev[i], (unsigned long long)((b) - (a))); } while (0)
@@ -257,7 +259,7 @@ __device__ __forceinline__ void lof_stat_row(const LofFusedSmem& sm, int c, cons
 // DESIGN.md S6); `median_out` is valid in every thread.
 template <int C, int L>
 __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& prm, const LofStatPlan& pl,
-                                      lof_stream_stats* out, float& median_out) {
+                                      lof_stream_stats* out, float& median_out, unsigned long long* diag) {
   using Cfg = LofFusedCfg<C, L>;
   constexpr int N = Cfg::N, NT = Cfg::NT;
   const int tid = threadIdx.x, lane = tid & 31;
@@ -369,15 +371,18 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
       if (!(var > 0.0)) var = 0.0;
       mean = (double)pl.K + da / n; stddev = sqrt(var);
     }
-    if ((uint32_t)lane < prm.n_levels)                   // threshold_I, one per lane
+    if ((uint32_t)lane < prm.n_levels) {                 // threshold_I, one per lane
       sm.thr[lane] = (float)((double)median + stddev * prm.factor[lane] * prm.sensitivity);
+      sm.thr[16 + lane] = lof_dead_level((double)median, stddev, prm.factor, prm.sensitivity, lane, prm.n_lev_f);
+      sm.thr[32 + lane] = lof_dead_level((double)median, stddev, prm.factor, prm.sensitivity, lane, prm.n_lev_t);
+    }
     if (lane == 0) {
       lof_stream_stats o;
       o.median = median; o.n_nonfinite = n_bad; o.mean = mean; o.stddev = stddev;
       o.n_flagged = n_bad ? (uint64_t)N : 0;
       *out = o;
       sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_ROW] = 0; sm.ctl[CT_COLGRP] = 0; sm.ctl[CT_SROW] = 0;
-      atomicAdd(&lof_fused_counters_dev[how], 1ull);
+      atomicAdd(&diag[how], 1ull);
     }
   }
   __syncthreads();
@@ -390,14 +395,14 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
 // sample, every row through lof_stat_row, then lof_stat_finalize.
 template <int C, int L>
 __device__ uint32_t lof_stat_whole(const LofFusedSmem& sm, const LofKParams& prm, float sample,
-                                   lof_stream_stats* out, float& median_out) {
+                                   lof_stream_stats* out, float& median_out, unsigned long long* diag) {
   using Cfg = LofFusedCfg<C, L>;
   constexpr int NT = Cfg::NT, NW = NT / 32;
   const LofStatPlan pl = lof_stat_plan<NT>(sample, reinterpret_cast<float*>(sm.red));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int c = warp; c < C; c += NW) lof_stat_row<C, L>(sm, c, pl, lane);
   __syncthreads();
-  return lof_stat_finalize<C, L>(sm, prm, pl, out, median_out);
+  return lof_stat_finalize<C, L>(sm, prm, pl, out, median_out, diag);
 }
 
 __host__ __device__ constexpr int lof_ilog2c(int v) { return v <= 1 ? 0 : 1 + lof_ilog2c(v / 2); }
@@ -475,18 +480,28 @@ __device__ __forceinline__ void lof_col_step(float (&u)[C], __half2 (&e2)[C / 2]
   const float v0 = fmaf(ef_.x, negT, u[2 * (m)]);              \
   const float v1 = fmaf(ef_.y, negT, u[2 * (m) + 1]);
 
+// Test of iteration I = 2^K after its doubling step.  Returns (warp-uniform) whether any flag is new; `dead`
+// (warp-uniform, meaningful when nothing is new) says that no window of I samples of the warp's columns has an
+// unflagged mean above `tdead`: no later iteration can flag anything (lof_dead_level).
 template <int C, int K>
-__device__ __forceinline__ bool lof_col_eval(const float (&u)[C], const __half2 (&e2)[C / 2], float thr, uint64_t& fb) {
+__device__ __forceinline__ bool lof_col_eval(const float (&u)[C], const __half2 (&e2)[C / 2], float thr, float tdead,
+                                             uint64_t& fb, bool& dead) {
   constexpr int I = 1 << K;
-  const float negT = -thr;
-  float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+  const float negT = -thr, negD = -tdead;
+  float tm[2] = {-INFINITY, -INFINITY}, td[2] = {-INFINITY, -INFINITY};
 #pragma unroll
   for (int m = 0; 2 * m + I <= C; ++m) {
     LOF_COL_V(m, v0, v1)
-    tm[(2 * m) & 3] = fmaxf(tm[(2 * m) & 3], v0);                          // u - e*T > 0 <=> window flagged
-    if (2 * m + 1 + I <= C) tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], v1);
+    const float d0 = fmaf(ef_.x, negD, u[2 * m]);
+    if (2 * m + 1 + I <= C) {
+      tm[m & 1] = lof_max3(tm[m & 1], v0, v1);                              // u - e*T > 0 <=> window flagged
+      td[m & 1] = lof_max3(td[m & 1], d0, fmaf(ef_.y, negD, u[2 * m + 1]));
+    } else {
+      tm[m & 1] = fmaxf(tm[m & 1], v0);
+      td[m & 1] = fmaxf(td[m & 1], d0);
+    }
   }
-  const bool fired = fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f;
+  const bool fired = fmaxf(tm[0], tm[1]) > 0.f;
   bool changed = false;
   if (__any_sync(0xffffffffu, fired)) {
     if (fired) {
@@ -507,18 +522,20 @@ __device__ __forceinline__ bool lof_col_eval(const float (&u)[C], const __half2 
     }
     changed = __any_sync(0xffffffffu, changed);
   }
+  dead = __all_sync(0xffffffffu, fmaxf(td[0], td[1]) <= 0.f);
   return changed;
 }
 
 // The frequency run of one column: ld(c) returns the sample of channel c (called again on a restart).
-// Returns the column's flag mask (bit c).  Every lane of the warp must call it (warp-uniform restarts).
+// thr[k]: threshold of iteration k; dead[k]: its early-exit level.  Returns the column's flag mask (bit c).
+// Every lane of the warp must call it (warp-uniform restarts and exits).
 template <int C, class Ld>
-__device__ __forceinline__ uint64_t lof_col_flag(Ld ld, const float* thr, int nlf) {
+__device__ __forceinline__ uint64_t lof_col_flag(Ld ld, const float* thr, const float* dead, int nlf) {
   constexpr int KMAX = lof_ilog2c(C);
   float u[C];
   __half2 e2[C / 2];
   uint64_t fb = 0;
-  const float T0 = thr[0];
+  const float T0 = thr[0], D0 = dead[0];
   int k_next = 1;
 #pragma unroll 1
   for (;;) {
@@ -530,7 +547,8 @@ __device__ __forceinline__ uint64_t lof_col_flag(Ld ld, const float* thr, int nl
       m0 = fmaxf(m0, u[c]); m1 = fmaxf(m1, u[c + 1]);
       e2[c / 2] = lof_h2_bits(LOF_H2_ONES);
     }
-    if (fb != 0 || fmaxf(m0, m1) > T0) {
+    float mu = fmaxf(m0, m1);                             // largest unflagged sample of the column
+    if (fb != 0 || mu > T0) {
       // independent partial masks (one per 32 channels and parity): no serial chain through fb
       uint32_t g[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
@@ -540,14 +558,24 @@ __device__ __forceinline__ uint64_t lof_col_flag(Ld ld, const float* thr, int nl
       for (int c = 0; c < C; ++c) u[c] = ((fb >> c) & 1ull) ? 0.f : u[c];
 #pragma unroll
       for (int m = 0; m < C / 2; ++m) e2[m] = lof_h2_unflagged((uint32_t)(fb >> (2 * m)) & 3u);
+      float a0 = 0.f, a1 = 0.f;                            // flagged samples count as 0 <= D0 (D0 > 0, or no exit)
+#pragma unroll
+      for (int c = 0; c + 1 < C; c += 4) { a0 = lof_max3(a0, u[c], u[c + 1]); if (c + 3 < C) a1 = lof_max3(a1, u[c + 2], u[c + 3]); }
+      mu = fmaxf(a0, a1);
     }
+    // no unflagged sample above every later threshold: no later iteration can flag anything (lof_dead_level)
+    if (__all_sync(0xffffffffu, mu <= D0)) break;
     // one test per level on the way down: past the last level -> done; new flags with levels to go ->
     // back to level 0 under the new mask
 #define LOF_COL_LEVEL(K)                                                             \
     if (K > KMAX || K >= nlf) break;                                                 \
     lof_col_step<C, (K <= KMAX ? K : 1)>(u, e2);                                     \
-    if (K >= k_next && lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e2, thr[K], fb) &&    \
-        K + 1 <= KMAX && K + 1 < nlf) { k_next = K + 1; LOF_PROF_CNT(6); continue; }
+    if (K >= k_next) {                                                               \
+      bool dead_;                                                                    \
+      if (lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e2, thr[K], dead[K], fb, dead_) && \
+          K + 1 <= KMAX && K + 1 < nlf) { k_next = K + 1; LOF_PROF_CNT(6); continue; } \
+      if (dead_) break;                                                              \
+    }
     LOF_COL_LEVEL(1) LOF_COL_LEVEL(2) LOF_COL_LEVEL(3) LOF_COL_LEVEL(4)
     LOF_COL_LEVEL(5) LOF_COL_LEVEL(6) LOF_COL_LEVEL(7) LOF_COL_LEVEL(8)
 #undef LOF_COL_LEVEL
@@ -583,7 +611,7 @@ __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
     if (g >= T / 32) break;
     const int col = g * 32 + lane;
     const float* cp = sm.xs + lof_swz_elem(col);
-    const uint64_t fb = lof_col_flag<C>([cp](int c) { return cp[c * T]; }, sm.thr, (int)n_lev_f);
+    const uint64_t fb = lof_col_flag<C>([cp](int c) { return cp[c * T]; }, sm.thr, sm.thr + 16, (int)n_lev_f);
     // this warp's 32 columns -> one mask word per channel
     const int w = col >> 5;
     uint32_t mine0, mine1;
@@ -627,20 +655,22 @@ __device__ __forceinline__ void lof_pcol_step(float (&u)[32], __half2 (&e2)[16],
   }
 }
 
-// Test of iteration I = 2^K <= 32 after its doubling step.  Returns (warp-uniform) whether any flag is new.
+// Test of iteration I = 2^K <= 32 after its doubling step.  Returns (warp-uniform) whether any flag is new;
+// `dead` as in lof_col_eval.
 template <int K>
 __device__ __forceinline__ bool lof_pcol_eval(const float (&u)[32], const __half2 (&e2)[16], int h, float thr,
-                                              uint32_t& fb) {
+                                              float tdead, uint32_t& fb, bool& dead) {
   constexpr int I = 1 << K;
-  const float negT = -thr;
-  float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+  const float negT = -thr, negD = -tdead;
+  float tm[2] = {-INFINITY, -INFINITY}, td[2] = {-INFINITY, -INFINITY};
 #pragma unroll
   for (int m = 0; m < 16; ++m) {
     const float2 ef = __half22float2(e2[m]);
-    tm[(2 * m) & 3] = fmaxf(tm[(2 * m) & 3], fmaf(ef.x, negT, u[2 * m]));
-    tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], fmaf(ef.y, negT, u[2 * m + 1]));
+    tm[m & 1] = lof_max3(tm[m & 1], fmaf(ef.x, negT, u[2 * m]), fmaf(ef.y, negT, u[2 * m + 1]));
+    td[m & 1] = lof_max3(td[m & 1], fmaf(ef.x, negD, u[2 * m]), fmaf(ef.y, negD, u[2 * m + 1]));
   }
-  const bool fired = fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f;
+  dead = __all_sync(0xffffffffu, fmaxf(td[0], td[1]) <= 0.f);
+  const bool fired = fmaxf(tm[0], tm[1]) > 0.f;
   if (!__any_sync(0xffffffffu, fired)) return false;
   uint32_t tg[4] = {0u, 0u, 0u, 0u};                       // partial masks: no serial chain
   if (fired) {
@@ -666,22 +696,23 @@ __device__ __forceinline__ bool lof_pcol_eval(const float (&u)[32], const __half
 // The frequency run of 16 columns x 64 channels by one warp: ld(j) returns this lane's sample of channel
 // 32h + j (called again on a restart).  Returns the lane's flag mask (bit j = channel 32h + j).
 template <class Ld>
-__device__ __forceinline__ uint32_t lof_pcol_flag(Ld ld, const float* thr, int nlf, int h) {
+__device__ __forceinline__ uint32_t lof_pcol_flag(Ld ld, const float* thr, const float* dead, int nlf, int h) {
   float u[32];
   __half2 e2[16];
   uint32_t fb = 0;
-  const float T0 = thr[0];
+  const float T0 = thr[0], D0 = dead[0];
   int k_next = 1;
 #pragma unroll 1
   for (;;) {
     float m0 = -INFINITY, m1 = -INFINITY;
 #pragma unroll
-    for (int j = 0; j < 32; j += 2) {
-      u[j] = ld(j); u[j + 1] = ld(j + 1);
-      m0 = fmaxf(m0, u[j]); m1 = fmaxf(m1, u[j + 1]);
-      e2[j / 2] = lof_h2_bits(LOF_H2_ONES);
+    for (int j = 0; j < 32; j += 4) {
+      u[j] = ld(j); u[j + 1] = ld(j + 1); u[j + 2] = ld(j + 2); u[j + 3] = ld(j + 3);
+      m0 = lof_max3(m0, u[j], u[j + 1]); m1 = lof_max3(m1, u[j + 2], u[j + 3]);
+      e2[j / 2] = lof_h2_bits(LOF_H2_ONES); e2[j / 2 + 1] = lof_h2_bits(LOF_H2_ONES);
     }
-    if (fb != 0 || fmaxf(m0, m1) > T0) {
+    float mu = fmaxf(m0, m1);                             // largest unflagged sample of this half column
+    if (fb != 0 || mu > T0) {
       uint32_t g[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
       for (int j = 0; j < 32; ++j) g[j & 3] |= (u[j] > T0) ? (1u << j) : 0u;
@@ -690,13 +721,22 @@ __device__ __forceinline__ uint32_t lof_pcol_flag(Ld ld, const float* thr, int n
       for (int j = 0; j < 32; ++j) u[j] = ((fb >> j) & 1u) ? 0.f : u[j];
 #pragma unroll
       for (int m = 0; m < 16; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
+      float a0 = 0.f, a1 = 0.f;                            // flagged samples count as 0 <= D0 (D0 > 0, or no exit)
+#pragma unroll
+      for (int j = 0; j < 32; j += 4) { a0 = lof_max3(a0, u[j], u[j + 1]); a1 = lof_max3(a1, u[j + 2], u[j + 3]); }
+      mu = fmaxf(a0, a1);
     }
+    if (__all_sync(0xffffffffu, mu <= D0)) break;         // lof_dead_level: no later iteration can flag anything
 #define LOF_PCOL_LEVEL(K)                                                          \
     if (K >= nlf) break;                                                           \
     lof_pcol_step<(1 << (K - 1))>(u, e2, h);                                       \
-    if (K >= k_next && lof_pcol_eval<K>(u, e2, h, thr[K], fb) && K + 1 < nlf) {    \
-      k_next = K + 1; LOF_PROF_CNT(6);                                              \
-      continue;                                                                    \
+    if (K >= k_next) {                                                             \
+      bool dead_;                                                                  \
+      if (lof_pcol_eval<K>(u, e2, h, thr[K], dead[K], fb, dead_) && K + 1 < nlf) { \
+        k_next = K + 1; LOF_PROF_CNT(6);                                            \
+        continue;                                                                  \
+      }                                                                            \
+      if (dead_) break;                                                            \
     }
     LOF_PCOL_LEVEL(1) LOF_PCOL_LEVEL(2) LOF_PCOL_LEVEL(3) LOF_PCOL_LEVEL(4) LOF_PCOL_LEVEL(5)
 #undef LOF_PCOL_LEVEL
@@ -727,7 +767,7 @@ __device__ void lof_fused_freq_pair(const LofFusedSmem& sm, uint32_t n_lev_f) {
     if (g >= T / 16) break;
     const int col = g * 16 + p;
     const float* cp = sm.xs + (32 * h) * T + lof_swz_elem(col);
-    const uint32_t fb = lof_pcol_flag([cp](int j) { return cp[j * T]; }, sm.thr, (int)n_lev_f, h);
+    const uint32_t fb = lof_pcol_flag([cp](int j) { return cp[j * T]; }, sm.thr, sm.thr + 16, (int)n_lev_f, h);
     // 16 columns x 64 channels of flags -> half a mask word per channel: the ballot of bit j has channel j
     // of the 16 columns in its low half and channel 32 + j in its high half; lane j keeps it
     uint32_t mine = 0;
@@ -778,20 +818,22 @@ __device__ __forceinline__ void lof_row_step(float (&u)[L], __half2 (&e2)[L / 2]
 }
 
 // Test of iteration I = 2^K on a row after its doubling step: fire windows with u > e*T, dilate the fired
-// starts over I samples across lanes, OR into fb.  Returns (warp-uniform) whether any flag is new.
+// starts over I samples across lanes, OR into fb.  Returns (warp-uniform) whether any flag is new; `dead`
+// (warp-uniform) says that no window of I samples has an unflagged mean above `tdead` (lof_dead_level).
 template <int L, int K>
 __device__ __forceinline__ bool lof_row_eval(const float (&u)[L], const __half2 (&e2)[L / 2], int lane, float thr,
-                                             uint32_t& fb) {
+                                             float tdead, uint32_t& fb, bool& dead) {
   constexpr int I = 1 << K;
-  const float negT = -thr;
-  float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+  const float negT = -thr, negD = -tdead;
+  float tm[2] = {-INFINITY, -INFINITY}, td[2] = {-INFINITY, -INFINITY};
 #pragma unroll
   for (int m = 0; m < L / 2; ++m) {
     const float2 ef = __half22float2(e2[m]);
-    tm[(2 * m) & 3] = fmaxf(tm[(2 * m) & 3], fmaf(ef.x, negT, u[2 * m]));
-    tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], fmaf(ef.y, negT, u[2 * m + 1]));
+    tm[m & 1] = lof_max3(tm[m & 1], fmaf(ef.x, negT, u[2 * m]), fmaf(ef.y, negT, u[2 * m + 1]));
+    td[m & 1] = lof_max3(td[m & 1], fmaf(ef.x, negD, u[2 * m]), fmaf(ef.y, negD, u[2 * m + 1]));
   }
-  if (!__any_sync(0xffffffffu, fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f)) return false;
+  dead = __all_sync(0xffffffffu, fmaxf(td[0], td[1]) <= 0.f);
+  if (!__any_sync(0xffffffffu, fmaxf(tm[0], tm[1]) > 0.f)) return false;
   uint32_t tg[4] = {0u, 0u, 0u, 0u};                       // partial masks: no serial chain
 #pragma unroll
   for (int m = 0; m < L / 2; ++m) {
@@ -828,15 +870,18 @@ __device__ __forceinline__ bool lof_row_eval(const float (&u)[L], const __half2 
 }
 
 // The time run of one row segment held by a warp (lane l: samples [l*L, l*L+L) in x[]): level 0, then the
-// doubling levels with restarts.  fb enters as the mask so far and leaves as the final mask.  `after_level0`
-// is called once, right after the first level 0 has consumed every x[j].  Warp-uniform control flow.
+// doubling levels with restarts and the early exit of lof_dead_level.  fb enters as the mask so far and leaves
+// as the final mask.  `after_level0` is called once, right after the first level 0 has consumed every x[j].
+// Returns true when `lane_sum` holds the sum of the lane's unflagged samples under the final mask (the run
+// ended at a level 0, whose u[] is exactly that: four strided partial sums, then (p0+p1)+(p2+p3)).
+// Warp-uniform control flow.
 template <int L, class Hook>
-__device__ __forceinline__ void lof_row_flag(const float (&x)[L], uint32_t& fb, const float* thr, int nlt, int lane,
-                                             Hook after_level0) {
+__device__ __forceinline__ bool lof_row_flag(const float (&x)[L], uint32_t& fb, const float* thr, const float* dead,
+                                             int nlt, int lane, Hook after_level0, float& lane_sum) {
   const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
   float u[L];
   __half2 e2[L / 2];
-  const float T0 = thr[0];
+  const float T0 = thr[0], D0 = dead[0];
   int k_next = 1;
 #pragma unroll 1
   for (;;) {
@@ -850,24 +895,40 @@ __device__ __forceinline__ void lof_row_flag(const float (&x)[L], uint32_t& fb, 
 #pragma unroll
       for (int j = 0; j < L; ++j) u[j] = ((fb >> j) & 1u) ? 0.f : x[j];
     }
+    if (k_next == 1) after_level0();
+    // the largest unflagged sample (flagged ones count as 0 <= D0: D0 > 0, or there is no exit)
+    float a0 = 0.f, a1 = 0.f;
+#pragma unroll
+    for (int j = 0; j < L; j += 4) { a0 = lof_max3(a0, u[j], u[j + 1]); a1 = lof_max3(a1, u[j + 2], u[j + 3]); }
+    if (__all_sync(0xffffffffu, fmaxf(a0, a1) <= D0 || fb == maskL)) {
+      // nothing left that any later iteration could flag (lof_dead_level), or nothing left to test
+      float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
+#pragma unroll
+      for (int j = 0; j < L; j += 4) { p0 += u[j]; p1 += u[j + 1]; p2 += u[j + 2]; p3 += u[j + 3]; }
+      lane_sum = (p0 + p1) + (p2 + p3);
+      return true;
+    }
 #pragma unroll
     for (int m = 0; m < L / 2; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
-    if (k_next == 1) after_level0();
-    if (__all_sync(0xffffffffu, fb == maskL)) break;     // nothing left to test in this row
     // one test per level on the way down: past the last level -> done; new flags with levels to go ->
     // back to level 0 under the new mask (continue), re-doubling up to k_next without testing
 #define LOF_ROW_LEVEL(K)                                                                 \
     if (K >= nlt) break;                                                                 \
     lof_row_step<L, (1 << (K - 1))>(u, e2, lane);                                        \
-    if (K >= k_next && lof_row_eval<L, K>(u, e2, lane, thr[K], fb) && K + 1 < nlt) {     \
-      k_next = K + 1; LOF_PROF_CNT(7);                                                    \
-      continue;                                                                          \
+    if (K >= k_next) {                                                                   \
+      bool dead_;                                                                        \
+      if (lof_row_eval<L, K>(u, e2, lane, thr[K], dead[K], fb, dead_) && K + 1 < nlt) {  \
+        k_next = K + 1; LOF_PROF_CNT(7);                                                  \
+        continue;                                                                        \
+      }                                                                                  \
+      if (dead_) break;                                                                  \
     }
     LOF_ROW_LEVEL(1) LOF_ROW_LEVEL(2) LOF_ROW_LEVEL(3) LOF_ROW_LEVEL(4) LOF_ROW_LEVEL(5)
     LOF_ROW_LEVEL(6) LOF_ROW_LEVEL(7) LOF_ROW_LEVEL(8) LOF_ROW_LEVEL(9)
 #undef LOF_ROW_LEVEL
     break;
   }
+  return false;
 }
 
 template <int C, int L>
@@ -912,7 +973,9 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
         lof_mbar_arrive_on_copies(sm.rowbar + c);
       }
     };
-    if (nlt > 0) lof_row_flag<L>(x, fb, sm.thr, (int)nlt, lane, prefetch_row);
+    float lane_sum = 0.f;
+    bool have_sum = false;
+    if (nlt > 0) have_sum = lof_row_flag<L>(x, fb, sm.thr, sm.thr + 32, (int)nlt, lane, prefetch_row, lane_sum);
     else prefetch_row();
     // bit-pack: word w of the row = bits [32w, 32w+32) gathered from the lanes' L-bit masks
     {
@@ -930,15 +993,18 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
       if (lane < W) flags[((size_t)s * C + c) * W + lane] = word;
     }
     // row sum of unflagged samples, fp32 within the lane, fp64 across lanes
-    float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
+    if (!have_sum) {
+      float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
 #pragma unroll
-    for (int j = 0; j < L; j += 4) {
-      p0 += ((fb >> j) & 1u) ? 0.f : x[j];
-      p1 += ((fb >> (j + 1)) & 1u) ? 0.f : x[j + 1];
-      p2 += ((fb >> (j + 2)) & 1u) ? 0.f : x[j + 2];
-      p3 += ((fb >> (j + 3)) & 1u) ? 0.f : x[j + 3];
+      for (int j = 0; j < L; j += 4) {
+        p0 += ((fb >> j) & 1u) ? 0.f : x[j];
+        p1 += ((fb >> (j + 1)) & 1u) ? 0.f : x[j + 1];
+        p2 += ((fb >> (j + 2)) & 1u) ? 0.f : x[j + 2];
+        p3 += ((fb >> (j + 3)) & 1u) ? 0.f : x[j + 3];
+      }
+      lane_sum = (p0 + p1) + (p2 + p3);
     }
-    double rs = (double)((p0 + p1) + (p2 + p3));
+    double rs = (double)lane_sum;
     rs = lof_warp_sum(rs);
     uint32_t nf = __popc(fb);
 #pragma unroll
@@ -972,7 +1038,8 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
 template <int C, int L>
 __global__ void __launch_bounds__(LofFusedCfg<C, L>::NT, LofFusedCfg<C, L>::MINB)
 lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_stream_stats* __restrict__ stats,
-            double* __restrict__ rowsum, uint32_t* __restrict__ rowcnt, LofKParams prm) {
+            double* __restrict__ rowsum, uint32_t* __restrict__ rowcnt, LofKParams prm,
+            unsigned long long* __restrict__ diag) {
   using Cfg = LofFusedCfg<C, L>;
   constexpr int N = Cfg::N, NT = Cfg::NT, W = Cfg::W;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -999,14 +1066,14 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
       for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
       lof_cp_async_wait_all();
       __syncthreads();
-      n_bad = lof_stat_whole<C, L>(sm, prm, sample, stats + s, median);
+      n_bad = lof_stat_whole<C, L>(sm, prm, sample, stats + s, median, diag);
     }
     ready = false;
     if (n_bad) {
       // DESIGN.md S6: the whole stream is flagged
       for (int i = tid; i < C * W; i += NT) flags[(size_t)s * C * W + i] = 0xFFFFFFFFu;
       for (int i = tid; i < C; i += NT) { rowsum[(size_t)s * C + i] = 0.0; rowcnt[(size_t)s * C + i] = 0; }
-      if (tid == 0) atomicAdd(&lof_fused_counters_dev[3], 1ull);
+      if (tid == 0) atomicAdd(&diag[3], 1ull);
       __syncthreads();
       continue;
     }
@@ -1034,8 +1101,8 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
     if (tid == 0) stats[s].n_flagged = sm.ctl[CT_NFLAG];
     __syncthreads();
     if (more) {
-      if (Cfg::OVL) n_bad = lof_stat_finalize<C, L>(sm, prm, plan_next, stats + s_next, median);
-      else n_bad = lof_stat_whole<C, L>(sm, prm, sample_next, stats + s_next, median);
+      if (Cfg::OVL) n_bad = lof_stat_finalize<C, L>(sm, prm, plan_next, stats + s_next, median, diag);
+      else n_bad = lof_stat_whole<C, L>(sm, prm, sample_next, stats + s_next, median, diag);
       ready = true;
     }
     LOF_PROF_T(t5);

@@ -1,7 +1,7 @@
 // lof_longrow.cuh — register-resident SumThreshold kernels for streams too long for one SM's shared
 // memory (BASELINE.json configs 4 and 5: rows of 195 312 and 12 208 samples).  Same column / row cores as
-// the fused kernel (lof_col_flag, lof_row_flag in lof_fused.cuh), fed from global memory (L2-resident: the
-// host processes streams in groups that fit L2, after the statistics passes of lof_stats.cuh).
+// the fused kernel (lof_col_flag, lof_row_flag in lof_fused.cuh), fed from global memory after the
+// statistics passes of lof_stats_lr.cuh (one group of streams per launch sequence).
 //   lof_k_freq_reg<C>: a warp per group of 32 time columns, a thread per column.
 //   lof_k_time_seg   : a warp per row segment of 1024 samples = OUT output samples + a halo of H on
 //                      each side, H >= the dependency cone sum_k (2^k - 1) of the time run, so segments
@@ -29,7 +29,7 @@ lof_k_freq_reg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
   const float* thr = state[s].thr_f;
   // a column beyond the row's end holds -inf: it never exceeds a threshold and any window sum with it is -inf
   const uint64_t fb = lof_col_flag<C>(
-      [&](int c) { return valid ? in.ld(base + (uint64_t)c * T) : -INFINITY; }, thr, (int)prm.n_lev_f);
+      [&](int c) { return valid ? in.ld(base + (uint64_t)c * T) : -INFINITY; }, thr, state[s].dead_f, (int)prm.n_lev_f);
   uint32_t mine0, mine1;
   lof_col_words<C>(fb, lane, mine0, mine1);
   if (lane < C) fmask[((uint64_t)s * C + lane) * W + w] = mine0;
@@ -91,21 +91,26 @@ lof_k_time_seg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
   const uint32_t valid = t_w >= T ? 0u : (T - t_w >= 32 ? 0xFFFFFFFFu : ((1u << (T - t_w)) - 1u));
   uint32_t fb = 0;
   if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];   // start from the frequency run's mask (F10)
+  float lane_sum = 0.f;
+  bool have_sum = false;
   if (st.nonfinite) fb = valid;                           // DESIGN.md S6: the whole stream is flagged
-  else if (prm.n_lev_t > 0) lof_row_flag<32>(x, fb, st.thr_f, (int)prm.n_lev_t, lane, [] {});
+  else if (prm.n_lev_t > 0) have_sum = lof_row_flag<32>(x, fb, st.thr_f, st.dead_t, (int)prm.n_lev_t, lane, [] {}, lane_sum);
   fb &= valid;
   const bool mine = t_w >= o_lo && t_w < o_hi;            // this lane's word belongs to the segment's output
   if (mine) flags[row * W + (t_w >> 5)] = fb;
-  float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
-  const uint32_t skip = fb | ~valid;
+  if (!have_sum || valid != 0xFFFFFFFFu) {                // (a word beyond the row's end holds -inf samples)
+    float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
+    const uint32_t skip = fb | ~valid;
 #pragma unroll
-  for (int j = 0; j < 32; j += 4) {
-    p0 += ((skip >> j) & 1u) ? 0.f : x[j];
-    p1 += ((skip >> (j + 1)) & 1u) ? 0.f : x[j + 1];
-    p2 += ((skip >> (j + 2)) & 1u) ? 0.f : x[j + 2];
-    p3 += ((skip >> (j + 3)) & 1u) ? 0.f : x[j + 3];
+    for (int j = 0; j < 32; j += 4) {
+      p0 += ((skip >> j) & 1u) ? 0.f : x[j];
+      p1 += ((skip >> (j + 1)) & 1u) ? 0.f : x[j + 1];
+      p2 += ((skip >> (j + 2)) & 1u) ? 0.f : x[j + 2];
+      p3 += ((skip >> (j + 3)) & 1u) ? 0.f : x[j + 3];
+    }
+    lane_sum = (p0 + p1) + (p2 + p3);
   }
-  double rs = mine ? (double)((p0 + p1) + (p2 + p3)) : 0.0;
+  double rs = mine ? (double)lane_sum : 0.0;
   rs = lof_warp_sum(rs);
   uint32_t nf = mine ? __popc(fb) : 0u, nu = mine ? __popc(valid & ~fb) : 0u;
 #pragma unroll
@@ -173,17 +178,22 @@ __device__ __forceinline__ void lof_row_step_coop(float (&u)[32], __half2 (&e2)[
 // into this one (carry through wmax[]), and "any" is taken over the CTA.  Contains __syncthreads: CTA-uniform.
 template <int K>
 __device__ __forceinline__ bool lof_row_eval_coop(const float (&u)[32], const __half2 (&e2)[16], int lane, int warp,
-                                                  float thr, uint32_t& fb, int* wmax) {
+                                                  float thr, float tdead, uint32_t& fb, int* wmax, bool& dead) {
   constexpr int I = 1 << K;
-  const float negT = -thr;
-  float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+  const float negT = -thr, negD = -tdead;
+  float tm[2] = {-INFINITY, -INFINITY}, td[2] = {-INFINITY, -INFINITY};
 #pragma unroll
   for (int m = 0; m < 16; ++m) {
     const float2 ef = __half22float2(e2[m]);
-    tm[(2 * m) & 3] = fmaxf(tm[(2 * m) & 3], fmaf(ef.x, negT, u[2 * m]));
-    tm[(2 * m + 1) & 3] = fmaxf(tm[(2 * m + 1) & 3], fmaf(ef.y, negT, u[2 * m + 1]));
+    tm[m & 1] = lof_max3(tm[m & 1], fmaf(ef.x, negT, u[2 * m]), fmaf(ef.y, negT, u[2 * m + 1]));
+    td[m & 1] = lof_max3(td[m & 1], fmaf(ef.x, negD, u[2 * m]), fmaf(ef.y, negD, u[2 * m + 1]));
   }
-  if (!__syncthreads_or(fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])) > 0.f)) return false;
+  // one barrier decides the usual case (nothing fired, and no window of I samples has an unflagged mean above
+  // tdead: the tile is done, lof_dead_level); a second one tells the two apart otherwise
+  const bool fired = fmaxf(tm[0], tm[1]) > 0.f, alive = fmaxf(td[0], td[1]) > 0.f;
+  dead = false;
+  if (!__syncthreads_or(fired || alive)) { dead = true; return false; }
+  if (!__syncthreads_or(fired)) return false;
   uint32_t tg[4] = {0u, 0u, 0u, 0u};                       // partial masks: no serial chain
 #pragma unroll
   for (int m = 0; m < 16; ++m) {
@@ -267,7 +277,8 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
   if (st.nonfinite) fb = valid;
   else if (nlt > 0) {
     const float* thr = st.thr_f;
-    const float T0 = thr[0];
+    const float* dead = st.dead_t;
+    const float T0 = thr[0], D0 = dead[0];
     float u[32];
     __half2 e2[16];
     int k_next = 1;
@@ -283,11 +294,19 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
 #pragma unroll
         for (int j = 0; j < 32; ++j) u[j] = ((fb >> j) & 1u) ? 0.f : x[j];
       }
+      {
+        // largest unflagged sample of the tile (flagged ones count as 0): lof_dead_level at level 0
+        float a0 = 0.f, a1 = 0.f;
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) { a0 = lof_max3(a0, u[j], u[j + 1]); a1 = lof_max3(a1, u[j + 2], u[j + 3]); }
+        if (__syncthreads_and(fmaxf(a0, a1) <= D0)) break;
+      }
 #pragma unroll
       for (int m = 0; m < 16; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
       again = false;
+      bool dead_ = false;
 #define LOF_CO_LEVEL(K)                                                                          \
-      if (K < nlt && !again) {                                                                   \
+      if (K < nlt && !again && !dead_) {                                                         \
         constexpr int D = 1 << (K - 1);                                                          \
         float* pbu = sm.bu[K & 1][warp]; uint32_t* pbe = sm.be[K & 1][warp];                     \
         /* publish the first D sums / counts of this strip for the previous warp */             \
@@ -298,7 +317,8 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
         __syncthreads();                                                                         \
         lof_row_step_coop<D>(u, e2, lane, sm.bu[K & 1][has_nb ? warp + 1 : warp],                \
                              sm.be[K & 1][has_nb ? warp + 1 : warp], has_nb);                    \
-        if (K >= k_next && lof_row_eval_coop<K>(u, e2, lane, warp, thr[K], fb, sm.wmax) && K + 1 < nlt) { \
+        if (K >= k_next && lof_row_eval_coop<K>(u, e2, lane, warp, thr[K], dead[K], fb, sm.wmax, dead_) && \
+            K + 1 < nlt) {                                                                       \
           again = true; k_next = K + 1;                                                          \
         }                                                                                        \
       }

@@ -71,6 +71,8 @@ __device__ __forceinline__ void lof_write_thresholds(LofStreamState& st, const L
     const double t = (double)st.median + st.stddev * prm.factor[k] * prm.sensitivity;
     st.thr_d[k] = t;
     st.thr_f[k] = (float)t;
+    st.dead_f[k] = lof_dead_level((double)st.median, st.stddev, prm.factor, prm.sensitivity, k, prm.n_lev_f);
+    st.dead_t[k] = lof_dead_level((double)st.median, st.stddev, prm.factor, prm.sensitivity, k, prm.n_lev_t);
   }
 }
 

@@ -403,6 +403,8 @@ lof_k_lr_select2(In in, LofKParams prm, LofStreamState* __restrict__ state, uint
       const double t = (double)median + sd * prm.factor[k] * prm.sensitivity;
       st.thr_d[k] = t;
       st.thr_f[k] = (float)t;
+      st.dead_f[k] = lof_dead_level((double)median, sd, prm.factor, prm.sensitivity, k, prm.n_lev_f);
+      st.dead_t[k] = lof_dead_level((double)median, sd, prm.factor, prm.sensitivity, k, prm.n_lev_t);
     }
     if (k == 0) {
       st.median = median;

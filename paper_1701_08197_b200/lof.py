@@ -14,10 +14,11 @@ LIB_PATH = os.environ.get("LOF_LIB_PATH") or os.path.join(_DIR, "liblof.so")   #
 DIR_FREQ, DIR_TIME = 1, 2
 MAX_LEVELS = 11
 E_NULL, E_PARAM, E_ALIGN, E_STATE, E_CUDA = -1, -2, -3, -4, -5
+PATH_NONE, PATH_FUSED, PATH_LONGROW_SEG, PATH_LONGROW_COOP, PATH_GENERIC = 0, 1, 2, 3, 4
 
 EXPORTS = ["lof_create", "lof_destroy", "lof_flag_block", "lof_flag_block_ci16", "lof_history_update",
            "lof_reset", "lof_row_sums", "lof_history_export", "lof_flag_block_host", "lof_factor_table",
-           "lof_launch_count", "lof_set_path", "lof_fused_counters", "lof_fused_cycles", "lof_strerror", "lof_last_cuda_error"]
+           "lof_launch_count", "lof_set_path", "lof_path_used", "lof_set_group", "lof_fused_counters", "lof_fused_cycles", "lof_strerror", "lof_last_cuda_error"]
 
 
 class Params(C.Structure):
@@ -56,7 +57,8 @@ def lib():
         L.lof_launch_count.argtypes = [C.c_void_p]
         for name in ("lof_create", "lof_destroy", "lof_flag_block", "lof_flag_block_ci16",
                      "lof_history_update", "lof_reset", "lof_row_sums", "lof_history_export",
-                     "lof_flag_block_host", "lof_factor_table", "lof_set_path", "lof_fused_counters", "lof_fused_cycles"):
+                     "lof_flag_block_host", "lof_factor_table", "lof_set_path", "lof_path_used", "lof_set_group",
+                     "lof_fused_counters", "lof_fused_cycles"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -178,6 +180,12 @@ class Flagger:
 
     def set_path(self, path):
         _check(lib().lof_set_path(self.h, C.c_int(path)))
+
+    def path_used(self):
+        return int(lib().lof_path_used(self.h))
+
+    def set_group(self, max_streams):
+        _check(lib().lof_set_group(self.h, C.c_uint32(max_streams)))
 
     def fused_cycles(self):
         out = (C.c_uint64 * 8)()

@@ -25,16 +25,20 @@ def wl():
     return workloads
 
 
-def run_gpu(lof, power, S, C, T, path=0, **kw):
+def run_gpu(lof, power, S, C, T, path=0, group=None, want_path=None, **kw):
     import torch
     f = lof.Flagger(S, C, T, **kw)
     f.set_path(path)
+    if group:
+        f.set_group(group)
     x = torch.from_numpy(np.ascontiguousarray(power)).cuda()
     flags, stats = f.flag_block(x)
     torch.cuda.synchronize()
     rs, rc = f.row_sums()
     out = dict(flags=lof.flags_to_numpy(flags), stats=lof.stats_to_numpy(stats),
-               rowsum=rs.cpu().numpy(), rowcnt=rc.cpu().numpy().view(np.uint32))
+               rowsum=rs.cpu().numpy(), rowcnt=rc.cpu().numpy().view(np.uint32), path_used=f.path_used())
+    if want_path is not None:
+        assert out["path_used"] == want_path, (out["path_used"], want_path)
     f.close()
     return out
 
@@ -44,13 +48,14 @@ def run_oracle(lofo, power, S, C, T, threads=8, **kw):
     return lofo.flag_block_threads(prm, power, threads, want_margin=True)
 
 
-def check(lof, lofo, power, S, C, T, exact=False, volt=None, paths=(0, 1), **kw):
+def check(lof, lofo, power, S, C, T, exact=False, volt=None, paths=(0, 1), group=None, want_path=None, **kw):
     if volt is not None:
         power = lofo.power_from_ci16(volt)
     ora = run_oracle(lofo, power, S, C, T, **kw)
     res = None
     for path in paths:
-        g = run_gpu(lof, volt if volt is not None else power, S, C, T, path=path, **kw)
+        g = run_gpu(lof, volt if volt is not None else power, S, C, T, path=path, group=group,
+                    want_path=want_path if path == 0 else lof.PATH_GENERIC, **kw)
         assert_stats(g["stats"], ora["stats"])
         res = assert_flags(g["flags"], ora, T, kw.get("max_window", 64), exact=exact)
         if res["n_mismatch"] == 0:
@@ -137,7 +142,12 @@ def test_config5_cut_with_history(lof, lofo, wl):
 @pytest.mark.parametrize("S,C,T,mw,dirs", [
     (3, 5, 77, 8, 3), (2, 1, 100, 16, 3), (2, 7, 1, 4, 3), (1, 3, 33, 64, 3), (2, 16, 256, 32, 1),
     (2, 16, 256, 32, 2), (1, 64, 768, 1, 3), (2, 48, 1000, 1024, 3), (1, 256, 40, 256, 3), (1, 2, 9000, 128, 3),
-    (2, 16, 3000, 128, 3), (1, 32, 5003, 64, 3), (3, 64, 2100, 32, 3), (2, 16, 1025, 64, 2), (1, 32, 4096, 256, 3)])
+    (2, 16, 3000, 128, 3), (1, 32, 5003, 64, 3), (3, 64, 2100, 32, 3), (2, 16, 1025, 64, 2), (1, 32, 4096, 256, 3),
+    # the fused shapes with windows beyond 64 (levels 7-9 of the row core with L = 24 and L = 8)
+    (2, 64, 768, 1024, 3), (3, 16, 768, 256, 3), (2, 16, 256, 128, 3), (2, 32, 768, 512, 2), (3, 16, 768, 128, 2),
+    # long rows with max_window 1024 (the cooperative tiles stop at 512: generic time kernel) and 512 (cross-warp
+    # exchange at distance 256)
+    (1, 16, 9000, 1024, 3), (1, 32, 20011, 512, 3)])
 def test_ragged_shapes(lof, lofo, S, C, T, mw, dirs):
     rng = np.random.default_rng(S * 1000 + C * 10 + T)
     x = rng.standard_exponential((S, C, T)).astype(np.float32)
@@ -316,3 +326,76 @@ def test_repeated_runs_are_bit_identical(lof, wl, shape):
             ref = got
         assert got == ref
     f.close()
+
+
+# ---- paths that only the full-size configurations take (multi-group loop, persistent CTAs past a
+# ---- non-finite stream, many streams on the generic path)
+
+@pytest.mark.parametrize("S,C,T,mw,group,ci16,want", [
+    (5, 16, 12208, 64, 2, False, "seg"),      # three groups (2 + 2 + 1), row segments with halo
+    (3, 32, 20011, 256, 1, True, "coop"),     # three groups of one stream, cooperative tiles, ci16
+    (4, 16, 9001, 256, 3, False, "coop"),     # 3 + 1, float32 through the cooperative tiles
+    (5, 32, 7001, 64, 2, True, "seg")])
+def test_long_rows_several_groups(lof, lofo, wl, S, C, T, mw, group, ci16, want):
+    """kp.s0 > 0: the loop over groups of streams that full config 4 takes (four groups of 26 streams)."""
+    rng = np.random.default_rng(S * 100 + C)
+    want_path = lof.PATH_LONGROW_SEG if want == "seg" else lof.PATH_LONGROW_COOP
+    if ci16:
+        w = wl.config4(7, n_stations=(S + 1) // 2, C=C, T=T)
+        volt = w.volt[:S]
+        check(lof, lofo, None, S, C, T, volt=volt, max_window=mw, group=group, want_path=want_path)
+    else:
+        x = rng.standard_exponential((S, C, T)).astype(np.float32)
+        for s in range(S):
+            x[s, rng.integers(0, C), :] += 3.0 + s
+            t0 = int(rng.integers(0, T - 600)); x[s, :, t0:t0 + 300 + 50 * s] += 1.5
+        check(lof, lofo, x, S, C, T, max_window=mw, group=group, want_path=want_path)
+
+
+def test_generic_path_more_than_1024_streams(lof, lofo):
+    """S > 1024: the generic path splits the block into groups of at most 1024 streams."""
+    rng = np.random.default_rng(21)
+    S, C, T = 1100, 4, 70
+    x = rng.standard_exponential((S, C, T)).astype(np.float32)
+    x[::7, 1, 10:30] += 6.0
+    x[1030:, :, 40] += 12.0                                # events in the second group
+    check(lof, lofo, x, S, C, T, max_window=16, want_path=lof.PATH_GENERIC)
+
+
+@pytest.mark.parametrize("C,T,mw", [(64, 768, 64), (16, 768, 64)])
+def test_fused_nonfinite_streams_inside_persistent_loop(lof, lofo, wl, C, T, mw):
+    """S far above the grid of persistent CTAs: streams with NaN/Inf met as the first stream of a CTA, as a
+    prefetched one, twice in a row in the same CTA and as the last one; the CTA flags them completely (S6) and
+    carries on with clean streams (reload path after the skipped stream)."""
+    import torch
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    grid = n_sm * (1 if C == 64 else 2)
+    S = grid * 3 + 5
+    rng = np.random.default_rng(C)
+    x = rng.standard_exponential((S, C, T)).astype(np.float32)
+    x[:, C // 3, :] += 2.0
+    x[::3, :, 100:103] += 30.0
+    bad = [0, 7, grid + 7, 2 * grid + 7, grid + 11, 2 * grid - 1, S - 1]
+    for i, s in enumerate(bad):
+        x[s, (3 * i) % C, (97 * i) % T] = np.nan if i % 2 == 0 else np.inf
+    g = run_gpu(lof, x, S, C, T, max_window=mw, want_path=lof.PATH_FUSED)
+    ora = run_oracle(lofo, x, S, C, T, threads=16, max_window=mw)
+    assert np.array_equal(g["stats"]["n_nonfinite"] > 0, np.isin(np.arange(S), bad))
+    assert_stats(g["stats"], ora["stats"])
+    assert_flags(g["flags"], ora, T, mw)
+    assert np.array_equal(g["stats"]["n_flagged"], ora["stats"]["n_flagged"])
+    assert np.array_equal(g["rowcnt"], ora["rowcnt"])
+    assert (g["rowcnt"][bad] == 0).all() and (g["flags"][bad] == 0xFFFFFFFF).all()
+
+
+def test_path_used_reports_the_decomposition(lof):
+    import torch
+    for (S, C, T, mw, want) in [(2, 64, 768, 64, "FUSED"), (2, 16, 256, 32, "FUSED"), (2, 64, 704, 64, "GENERIC"),
+                                (1, 16, 12208, 64, "LONGROW_SEG"), (1, 32, 20000, 256, "LONGROW_COOP"),
+                                (1, 32, 20000, 1024, "GENERIC"), (2, 5, 77, 8, "GENERIC")]:
+        f = lof.Flagger(S, C, T, max_window=mw)
+        assert f.path_used() == lof.PATH_NONE
+        f.flag_block(torch.rand((S, C, T), device="cuda"))
+        torch.cuda.synchronize()
+        assert f.path_used() == getattr(lof, "PATH_" + want), (S, C, T, mw, f.path_used())
+        f.close()
