@@ -122,6 +122,50 @@ void lofo_power_from_ci16(const int16_t* volt, uint64_t n, float* power) {
 }
 
 
+// "all ranges of consecutive flagged samples are extended by flagging 20% more samples, before
+// and after the original range".  Runs are those of the input mask (SIR-2); floor(eta * len) samples on each
+// side (SIR-3), clipped at the ends of the line (SIR-4).
+void lofo_sir_1d(uint8_t* mask, uint64_t n, int64_t stride, double eta) {
+  if (!(eta > 0.0) || n == 0) return;
+  std::vector<uint8_t> in(n);
+  for (uint64_t i = 0; i < n; ++i) in[i] = mask[(int64_t)i * stride];
+  uint64_t i = 0;
+  while (i < n) {
+    if (!in[i]) { ++i; continue; }
+    uint64_t b = i;
+    while (b < n && in[b]) ++b;                              // maximal run [i, b)
+    const uint64_t len = b - i;
+    const uint64_t ext = (uint64_t)std::floor(eta * (double)len);
+    const uint64_t lo = ext > i ? 0 : i - ext;               // clipped at the start of the line
+    const uint64_t hi = b + ext > n ? n : b + ext;           // ... and at its end
+    for (uint64_t j = lo; j < i; ++j) mask[(int64_t)j * stride] = 1;
+    for (uint64_t j = b; j < hi; ++j) mask[(int64_t)j * stride] = 1;
+    i = b;
+  }
+}
+
+// The operator on a packed block mask: frequency direction first, then time on the result (SIR-5, the order of
+// the SumThreshold runs).
+void lofo_sir_block(uint32_t* flags, uint64_t S, uint64_t C, uint64_t T, double eta, uint32_t directions) {
+  if (!(eta > 0.0)) return;
+  const uint64_t words = (T + 31) / 32;
+  std::vector<uint8_t> M(C * T);
+  for (uint64_t s = 0; s < S; ++s) {
+    uint32_t* fs = flags + s * C * words;
+    for (uint64_t c = 0; c < C; ++c)
+      for (uint64_t t = 0; t < T; ++t) M[c * T + t] = (fs[c * words + (t >> 5)] >> (t & 31)) & 1u;
+    if (directions & 1u)
+      for (uint64_t t = 0; t < T; ++t) lofo_sir_1d(M.data() + t, C, (int64_t)T, eta);
+    if (directions & 2u)
+      for (uint64_t c = 0; c < C; ++c) lofo_sir_1d(M.data() + c * T, T, 1, eta);
+    for (uint64_t c = 0; c < C; ++c) {
+      for (uint64_t w = 0; w < words; ++w) fs[c * words + w] = 0;
+      for (uint64_t t = 0; t < T; ++t)
+        if (M[c * T + t]) fs[c * words + (t >> 5)] |= (uint32_t)1 << (t & 31);
+    }
+  }
+}
+
 // O1-O9 for a whole block (PAPER.md:37-47 per line; frequency first then time, PAPER.md:83,
 // :180; the time run starts from and substitutes the frequency run's flags, reading F10;
 // statistics over all samples of the stream before any flagging, reading S1).
@@ -170,6 +214,13 @@ int lofo_flag_block(const lofo_params* prm, const float* power, uint32_t* flags,
       }
       if (rowsum) rowsum[s * C + c] = rs;
       if (rowcnt) rowcnt[s * C + c] = rc;
+    }
+    // SIR operator on the packed mask of this stream, after the row sums were taken: it "operates
+    // on the flag masks only, and not on the actual data", reading SIR-6
+    if (prm->sir_eta > 0.0) {
+      lofo_sir_block(flags + s * C * words, 1, C, T, prm->sir_eta, prm->directions);
+      nf = 0;
+      for (uint64_t i = 0; i < C * words; ++i) nf += (uint64_t)__builtin_popcount(flags[s * C * words + i]);
     }
     st.n_flagged = nf;
     if (stats) stats[s] = st;

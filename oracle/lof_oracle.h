@@ -31,6 +31,8 @@ typedef struct {
   uint32_t history_length;      /* H */
   uint32_t history_min_fill;
   double   history_sensitivity; /* <= 0: use sensitivity */
+  double   sir_eta;             /* SIR operator: every run of flagged samples is extended by
+                                   floor(sir_eta * length) samples before and after; 0 = off; typical 0.2 */
 } lofo_params;
 
 typedef struct {
@@ -71,6 +73,17 @@ void lofo_sumthreshold_1d_fast(const float* x, uint64_t n, int64_t stride, uint8
 int lofo_flag_block(const lofo_params* prm, const float* power, uint32_t* flags,
                     lofo_stream_stats* stats, double* rowsum, uint32_t* rowcnt,
                     uint8_t* mask_freq, uint8_t* margin, double margin_rel, int use_literal);
+
+/* Scale-invariant rank operator as PAPER.md:55 states it: "all ranges of consecutive flagged samples are
+ * extended by flagging 20% more samples, before and after the original range".  One line of n mask bytes
+ * (mask[i*stride], 0/1), in place: every maximal run of flagged samples of the INPUT mask, of length len, gets
+ * floor(eta*len) more samples flagged on each side, clipped at the ends of the line; run lengths are those of
+ * the input (extensions do not lengthen one another).  Readings SIR-1..4 of DESIGN.md §3. */
+void lofo_sir_1d(uint8_t* mask, uint64_t n, int64_t stride, double eta);
+
+/* The operator on a packed block mask flags[S][C][ceil(T/32)] in place: along frequency (channels of one time
+ * sample), then along time on the result, for the directions set in `directions` (reading SIR-5). */
+void lofo_sir_block(uint32_t* flags, uint64_t S, uint64_t C, uint64_t T, double eta, uint32_t directions);
 
 /* x = (float)(uint32)(re*re + im*im) for complex int16 volt[n][2] (reading S5). */
 void lofo_power_from_ci16(const int16_t* volt, uint64_t n, float* power);

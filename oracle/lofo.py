@@ -32,7 +32,7 @@ class Params(C.Structure):
                 ("p", C.c_double), ("sensitivity", C.c_double), ("start_threshold", C.c_double),
                 ("max_window", C.c_uint32), ("directions", C.c_uint32),
                 ("history_length", C.c_uint32), ("history_min_fill", C.c_uint32),
-                ("history_sensitivity", C.c_double)]
+                ("history_sensitivity", C.c_double), ("sir_eta", C.c_double)]
 
 
 STATS_DTYPE = np.dtype([("median", np.float32), ("n_nonfinite", np.uint32), ("mean", np.float64),
@@ -56,9 +56,9 @@ def _p(a):
 
 
 def make_params(S, Cn, T, p=1.5, sensitivity=1.0, start_threshold=6.0, max_window=64, directions=3,
-                history_length=0, history_min_fill=2, history_sensitivity=0.0):
+                history_length=0, history_min_fill=2, history_sensitivity=0.0, sir_eta=0.0):
     return Params(S, Cn, T, p, sensitivity, start_threshold, max_window, directions,
-                  history_length, history_min_fill, history_sensitivity)
+                  history_length, history_min_fill, history_sensitivity, float(np.float32(sir_eta)))
 
 
 def factor_table(n, start_threshold=6.0, p=1.5):
@@ -133,6 +133,23 @@ def flag_block_threads(prm, power, n_threads, **kw):
     with ThreadPoolExecutor(len(parts)) as ex:
         outs = list(ex.map(work, parts))
     return {k: np.concatenate([o[k] for o in outs], axis=0) for k in outs[0]}
+
+
+def sir_1d(mask, eta):
+    """SIR operator on one line (uint8 0/1).  Returns the extended mask."""
+    m = np.ascontiguousarray(mask, np.uint8).copy()
+    lib().lofo_sir_1d(_p(m), C.c_uint64(m.size), C.c_int64(1), C.c_double(float(np.float32(eta))))
+    return m
+
+
+def sir_block(flags, T, eta, directions=3):
+    """SIR operator on packed flags uint32[S][C][ceil(T/32)] (frequency, then time).  Returns a new array."""
+    f = np.ascontiguousarray(flags, np.uint32).copy()
+    S, Cn, W = f.shape
+    assert W == (T + 31) // 32
+    lib().lofo_sir_block(_p(f), C.c_uint64(S), C.c_uint64(Cn), C.c_uint64(T), C.c_double(float(np.float32(eta))),
+                         C.c_uint32(directions))
+    return f
 
 
 def power_from_ci16(volt):

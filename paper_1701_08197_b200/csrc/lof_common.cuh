@@ -83,6 +83,22 @@ struct InCI16 {
   static constexpr int kBytes = 4;
 };
 
+// cycles of thread 0 per phase, summed over CTAs and streams, when built with -DLOF_FUSED_PROF (profiling builds
+// only; process-global): [0] first load + statistics, [1] frequency pass, [2] plan of the next stream, [3] time
+// pass with the next stream's row statistics, [4] end of the next stream's statistics
+#ifdef LOF_FUSED_PROF
+__device__ unsigned long long lof_fused_cycles_dev[8];
+#endif
+#ifdef LOF_FUSED_PROF
+#define LOF_PROF_T(var) const long long var = clock64()
+#define LOF_PROF_ADD(i, a, b) do { if (threadIdx.x == 0) atomicAdd(&lof_fused_cycles_dev[i], (unsigned long long)((b) - (a))); } while (0)
+#define LOF_PROF_CNT(i) do { if ((threadIdx.x & 31) == 0) atomicAdd(&lof_fused_cycles_dev[i], 1ull); } while (0)
+#else
+#define LOF_PROF_T(var)
+#define LOF_PROF_ADD(i, a, b)
+#define LOF_PROF_CNT(i)
+#endif
+
 // Early exit of a SumThreshold run.  A window of 2^k samples is a disjoint union of windows
 // of 2^j samples (j < k), and it fires only if the sum over its unflagged samples of (x - threshold_k) is
 // positive (reading F7) — so at least one of those smaller windows has an unflagged mean above

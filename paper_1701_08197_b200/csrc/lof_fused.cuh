@@ -21,6 +21,7 @@
 #include <cuda_fp16.h>
 
 #include "lof_common.cuh"
+#include "lof_core.cuh"
 
 #define LOF_F_NBINS 4096
 #define LOF_F_CAP 1024
@@ -45,26 +46,25 @@ struct LofFusedCfg {
   static constexpr bool OVL = MINB == 1;
 #endif
   static constexpr size_t smem_bytes =
-      (size_t)N * 4 + (size_t)C * W * 4 + LOF_F_NBINS * 4 + LOF_F_CAP * 4 + 64 * 8 + (size_t)3 * C * 8 +
-      (48 + 48) * 4 + 256 * 4;
+      (size_t)N * 4 + LOF_F_NBINS * 4 + LOF_F_CAP * 4 + 64 * 8 + (size_t)3 * C * 8 + (64 + 48) * 4 + 256 * 4;
 };
 
 struct LofFusedSmem {
-  float* xs; uint32_t* fm; uint32_t* hist; float* cand; double* red; double* rowpart; unsigned long long* rowbar; float* thr;
+  float* xs; uint32_t* hist; float* cand; double* red; double* rowpart; unsigned long long* rowbar; float* thr;
   uint32_t* ctl; uint32_t* part;
   template <int C, int L>
   __device__ static LofFusedSmem make(unsigned char* base) {
     LofFusedSmem s;
     constexpr int N = C * 32 * L;
     s.xs = reinterpret_cast<float*>(base);
-    s.fm = reinterpret_cast<uint32_t*>(s.xs + N);
-    s.hist = s.fm + C * L;
+    s.hist = reinterpret_cast<uint32_t*>(s.xs + N);
     s.cand = reinterpret_cast<float*>(s.hist + LOF_F_NBINS);
     s.red = reinterpret_cast<double*>(s.cand + LOF_F_CAP);
     s.rowpart = s.red + 64;
     s.rowbar = reinterpret_cast<unsigned long long*>(s.rowpart + 2 * C);
     s.thr = reinterpret_cast<float*>(s.rowbar + C);
-    s.ctl = reinterpret_cast<uint32_t*>(s.thr + 48);      // thr[0..16) thresholds, [16..32) / [32..48) early-exit levels
+    // thr[0..16) thresholds, [16..32) / [32..48) early-exit levels of the two runs, [48] = FLT_MAX (time run off)
+    s.ctl = reinterpret_cast<uint32_t*>(s.thr + 64);
     s.part = s.ctl + 48;
     return s;
   }
@@ -76,22 +76,6 @@ enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS,
 // each stream was found: [0] rank count among the samples of the median's bin, [1] radix select among them (a
 // crowded bin), [2] radix select over the whole stream, [3] stream with non-finite samples.
 #define LOF_DIAG_WORDS 16
-// cycles of thread 0 per phase, summed over CTAs and streams, when built with -DLOF_FUSED_PROF (profiling builds
-// only; process-global): [0] first load + statistics, [1] frequency pass, [2] plan of the next stream, [3] time
-// pass with the next stream's row statistics, [4] end of the next stream's statistics
-#ifdef LOF_FUSED_PROF
-__device__ unsigned long long lof_fused_cycles_dev[8];
-#endif
-#ifdef LOF_FUSED_PROF
-#define LOF_PROF_T(var) const long long var = clock64()
-#define LOF_PROF_ADD(i, a, b) do { if (threadIdx.x == 0) atomicAdd(&lof_fused_cycles_dev[i], (unsigned long long)((b) - (a))); } while (0)
-#define LOF_PROF_CNT(i) do { if ((threadIdx.x & 31) == 0) atomicAdd(&lof_fused_cycles_dev[i], 1ull); } while (0)
-#else
-#define LOF_PROF_T(var)
-#define LOF_PROF_ADD(i, a, b)
-#define LOF_PROF_CNT(i)
-#endif
-
 // Find the bin holding `rank` in hist[NB] (NB a multiple of 1024, any blockDim that is a multiple of 32).
 // Results in ctl[CT_BIN] (bin) and ctl[CT_BEFORE] (number of entries in lower bins); rank beyond the total
 // gives the last bin.  Groups of 32 bins are summed by warps (one bin per lane: no bank conflicts), warp 0
@@ -376,6 +360,7 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
       sm.thr[16 + lane] = lof_dead_level((double)median, stddev, prm.factor, prm.sensitivity, lane, prm.n_lev_f);
       sm.thr[32 + lane] = lof_dead_level((double)median, stddev, prm.factor, prm.sensitivity, lane, prm.n_lev_t);
     }
+    if (lane == 0) sm.thr[48] = LOF_BELOW_MARK;            // "threshold" of a run that is switched off
     if (lane == 0) {
       lof_stream_stats o;
       o.median = median; o.n_nonfinite = n_bad; o.mean = mean; o.stddev = stddev;
@@ -404,8 +389,6 @@ __device__ uint32_t lof_stat_whole(const LofFusedSmem& sm, const LofKParams& prm
   __syncthreads();
   return lof_stat_finalize<C, L>(sm, prm, pl, out, median_out, diag);
 }
-
-__host__ __device__ constexpr int lof_ilog2c(int v) { return v <= 1 ? 0 : 1 + lof_ilog2c(v / 2); }
 
 // Shared-memory layout of a row: float4 chunk g is stored at g ^ ((g >> 3) & 1): adjacent float4 pairs swapped in
 // every odd group of 32 floats.  Column access (32 consecutive t) stays conflict-free, and the time pass's
@@ -438,327 +421,35 @@ __device__ __forceinline__ void lof_mbar_wait(unsigned long long* bar, unsigned 
       "@!p bra LOF_MBAR_WAIT_%=;\n}" ::"r"(a), "r"(parity) : "memory");
 }
 
-// ---- F: SumThreshold along frequency.  One thread per time column; u[c], e[c] in registers.
-// Levels run in order; u, e are doubled in place (ascending c, so u[c + d] is still the previous level).
-// When an iteration sets a new flag anywhere in the warp, the warp restarts from level 0 under the new
-// mask and re-doubles up to that level without testing (k_next), then carries on: every step and every
-// test exists once in the code, which keeps the kernel inside the instruction cache.
-// e (number of unflagged samples of a window, an integer <= 1024) is kept as packed halves, two window
-// positions per register: exact, half the registers of fp32 (the 64-channel column then fits 128 registers
-// per thread, i.e. 16 warps per SM), and one HADD2 doubles two positions.
-#define LOF_H2_ONES 0x3C003C00u
-__device__ __forceinline__ __half2 lof_h2_bits(uint32_t b) { return *reinterpret_cast<__half2*>(&b); }
-__device__ __forceinline__ uint32_t lof_bits_h2(__half2 h) { return *reinterpret_cast<uint32_t*>(&h); }
-// (a.hi, b.lo): the pair starting one position later
-__device__ __forceinline__ __half2 lof_h2_shift1(__half2 a, __half2 b) {
-  return lof_h2_bits(__byte_perm(lof_bits_h2(a), lof_bits_h2(b), 0x5432));
-}
-// e of two consecutive positions from their flag bits (bit 0 = first): 1.0 where unflagged, 0.0 where flagged
-__device__ __forceinline__ __half2 lof_h2_unflagged(uint32_t two_flag_bits) {
-  const uint32_t keep = ((two_flag_bits & 1u) ? 0u : 0x0000FFFFu) | ((two_flag_bits & 2u) ? 0u : 0xFFFF0000u);
-  return lof_h2_bits(LOF_H2_ONES & keep);
-}
-
-template <int C, int K>
-__device__ __forceinline__ void lof_col_step(float (&u)[C], __half2 (&e2)[C / 2]) {
-  constexpr int d = 1 << (K - 1), I = 1 << K;
-#pragma unroll
-  for (int c = 0; c + I <= C; ++c) u[c] += u[c + d];
-  if constexpr (K == 1) {
-#pragma unroll
-    for (int m = 0; m < C / 2; ++m)
-      e2[m] = __hadd2(e2[m], lof_h2_shift1(e2[m], e2[m + 1 < C / 2 ? m + 1 : m]));
-  } else {
-#pragma unroll
-    for (int m = 0; 2 * m + I <= C; ++m) e2[m] = __hadd2(e2[m], e2[m + d / 2]);
-  }
-}
-
-// v[c] = u[c] - e[c]*T for the two positions of pair m
-#define LOF_COL_V(m, v0, v1)                                   \
-  const float2 ef_ = __half22float2(e2[m]);                    \
-  const float v0 = fmaf(ef_.x, negT, u[2 * (m)]);              \
-  const float v1 = fmaf(ef_.y, negT, u[2 * (m) + 1]);
-
-// Test of iteration I = 2^K after its doubling step.  Returns (warp-uniform) whether any flag is new; `dead`
-// (warp-uniform, meaningful when nothing is new) says that no window of I samples of the warp's columns has an
-// unflagged mean above `tdead`: no later iteration can flag anything (lof_dead_level).
-template <int C, int K>
-__device__ __forceinline__ bool lof_col_eval(const float (&u)[C], const __half2 (&e2)[C / 2], float thr, float tdead,
-                                             uint64_t& fb, bool& dead) {
-  constexpr int I = 1 << K;
-  const float negT = -thr, negD = -tdead;
-  float tm[2] = {-INFINITY, -INFINITY}, td[2] = {-INFINITY, -INFINITY};
-#pragma unroll
-  for (int m = 0; 2 * m + I <= C; ++m) {
-    LOF_COL_V(m, v0, v1)
-    const float d0 = fmaf(ef_.x, negD, u[2 * m]);
-    if (2 * m + 1 + I <= C) {
-      tm[m & 1] = lof_max3(tm[m & 1], v0, v1);                              // u - e*T > 0 <=> window flagged
-      td[m & 1] = lof_max3(td[m & 1], d0, fmaf(ef_.y, negD, u[2 * m + 1]));
-    } else {
-      tm[m & 1] = fmaxf(tm[m & 1], v0);
-      td[m & 1] = fmaxf(td[m & 1], d0);
-    }
-  }
-  const bool fired = fmaxf(tm[0], tm[1]) > 0.f;
-  bool changed = false;
-  if (__any_sync(0xffffffffu, fired)) {
-    if (fired) {
-      uint32_t tg[4] = {0u, 0u, 0u, 0u};                   // partial masks: no serial chain
-#pragma unroll
-      for (int m = 0; 2 * m + I <= C; ++m) {
-        LOF_COL_V(m, v0, v1)
-        tg[(2 * m) >> 5] |= (v0 > 0.f) ? (1u << ((2 * m) & 31)) : 0u;
-        if (2 * m + 1 + I <= C) tg[2 + ((2 * m) >> 5)] |= (v1 > 0.f) ? (2u << ((2 * m) & 31)) : 0u;
-      }
-      const uint64_t trig = (uint64_t)(tg[0] | tg[2]) | ((uint64_t)(tg[1] | tg[3]) << 32);
-      uint64_t dil = trig;
-#pragma unroll
-      for (int s = 1; s < I; s <<= 1) dil |= dil << s;
-      const uint64_t nf = fb | dil;
-      changed = nf != fb;
-      fb = nf;
-    }
-    changed = __any_sync(0xffffffffu, changed);
-  }
-  dead = __all_sync(0xffffffffu, fmaxf(td[0], td[1]) <= 0.f);
-  return changed;
-}
-
-// The frequency run of one column: ld(c) returns the sample of channel c (called again on a restart).
-// thr[k]: threshold of iteration k; dead[k]: its early-exit level.  Returns the column's flag mask (bit c).
-// Every lane of the warp must call it (warp-uniform restarts and exits).
-template <int C, class Ld>
-__device__ __forceinline__ uint64_t lof_col_flag(Ld ld, const float* thr, const float* dead, int nlf) {
-  constexpr int KMAX = lof_ilog2c(C);
-  float u[C];
-  __half2 e2[C / 2];
-  uint64_t fb = 0;
-  const float T0 = thr[0], D0 = dead[0];
-  int k_next = 1;
-#pragma unroll 1
-  for (;;) {
-    // level 0 under the current mask: I = 1 is the simple thresholder x > threshold_1
-    float m0 = -INFINITY, m1 = -INFINITY;
-#pragma unroll
-    for (int c = 0; c < C; c += 2) {
-      u[c] = ld(c); u[c + 1] = ld(c + 1);
-      m0 = fmaxf(m0, u[c]); m1 = fmaxf(m1, u[c + 1]);
-      e2[c / 2] = lof_h2_bits(LOF_H2_ONES);
-    }
-    float mu = fmaxf(m0, m1);                             // largest unflagged sample of the column
-    if (fb != 0 || mu > T0) {
-      // independent partial masks (one per 32 channels and parity): no serial chain through fb
-      uint32_t g[4] = {0u, 0u, 0u, 0u};
-#pragma unroll
-      for (int c = 0; c < C; ++c) g[((c >> 5) << 1) | (c & 1)] |= (u[c] > T0) ? (1u << (c & 31)) : 0u;
-      fb |= (uint64_t)(g[0] | g[1]) | ((uint64_t)(g[2] | g[3]) << 32);
-#pragma unroll
-      for (int c = 0; c < C; ++c) u[c] = ((fb >> c) & 1ull) ? 0.f : u[c];
-#pragma unroll
-      for (int m = 0; m < C / 2; ++m) e2[m] = lof_h2_unflagged((uint32_t)(fb >> (2 * m)) & 3u);
-      float a0 = 0.f, a1 = 0.f;                            // flagged samples count as 0 <= D0 (D0 > 0, or no exit)
-#pragma unroll
-      for (int c = 0; c + 1 < C; c += 4) { a0 = lof_max3(a0, u[c], u[c + 1]); if (c + 3 < C) a1 = lof_max3(a1, u[c + 2], u[c + 3]); }
-      mu = fmaxf(a0, a1);
-    }
-    // no unflagged sample above every later threshold: no later iteration can flag anything (lof_dead_level)
-    if (__all_sync(0xffffffffu, mu <= D0)) break;
-    // one test per level on the way down: past the last level -> done; new flags with levels to go ->
-    // back to level 0 under the new mask
-#define LOF_COL_LEVEL(K)                                                             \
-    if (K > KMAX || K >= nlf) break;                                                 \
-    lof_col_step<C, (K <= KMAX ? K : 1)>(u, e2);                                     \
-    if (K >= k_next) {                                                               \
-      bool dead_;                                                                    \
-      if (lof_col_eval<C, (K <= KMAX ? K : 1)>(u, e2, thr[K], dead[K], fb, dead_) && \
-          K + 1 <= KMAX && K + 1 < nlf) { k_next = K + 1; LOF_PROF_CNT(6); continue; } \
-      if (dead_) break;                                                              \
-    }
-    LOF_COL_LEVEL(1) LOF_COL_LEVEL(2) LOF_COL_LEVEL(3) LOF_COL_LEVEL(4)
-    LOF_COL_LEVEL(5) LOF_COL_LEVEL(6) LOF_COL_LEVEL(7) LOF_COL_LEVEL(8)
-#undef LOF_COL_LEVEL
-    break;
-  }
-  return fb;
-}
-
-// A warp's 32 column masks -> one word per channel (lane c & 31 ends up holding channel c's word).
-template <int C>
-__device__ __forceinline__ void lof_col_words(uint64_t fb, int lane, uint32_t& mine0, uint32_t& mine1) {
-  mine0 = 0; mine1 = 0;
-  if (__any_sync(0xffffffffu, fb != 0)) {
-#pragma unroll
-    for (int c = 0; c < C; ++c) {
-      const uint32_t word = __ballot_sync(0xffffffffu, (fb >> c) & 1ull);
-      if ((c & 31) == lane) { if (c < 32) mine0 = word; else mine1 = word; }
-    }
-  }
-}
-
+// ---- F: SumThreshold along frequency ("We first flag in the frequency direction"): the column
+// cores of lof_core.cuh on the stream in shared memory.  A flagged sample is marked IN the shared-memory copy
+// of the stream (LOF_MARK): that is how the time run, which starts from this run's mask (reading F10), sees it.
 template <int C, int L>
 __device__ void lof_fused_freq(const LofFusedSmem& sm, uint32_t n_lev_f) {
   using Cfg = LofFusedCfg<C, L>;
-  constexpr int T = Cfg::T, W = Cfg::W;
+  constexpr int T = Cfg::T;
   const int lane = threadIdx.x & 31;
 #pragma unroll 1
   for (;;) {
-    // groups of 32 columns are handed out dynamically (restarts make their cost uneven)
+    // groups of 32 columns are handed out dynamically (restarts and early exits make their cost uneven)
     int g = 0;
     if (lane == 0) g = (int)atomicAdd(&sm.ctl[CT_COLGRP], 1u);
     g = __shfl_sync(0xffffffffu, g, 0);
     if (g >= T / 32) break;
     const int col = g * 32 + lane;
-    const float* cp = sm.xs + lof_swz_elem(col);
-    const uint64_t fb = lof_col_flag<C>([cp](int c) { return cp[c * T]; }, sm.thr, sm.thr + 16, (int)n_lev_f);
-    // this warp's 32 columns -> one mask word per channel
-    const int w = col >> 5;
-    uint32_t mine0, mine1;
-    lof_col_words<C>(fb, lane, mine0, mine1);
-    if (lane < C) sm.fm[lane * W + w] = mine0;
-    if (C > 32 && lane + 32 < C) sm.fm[(lane + 32) * W + w] = mine1;
+    float* cp = sm.xs + lof_swz_elem(col);
+    uint64_t fb = lof_col_flag<C>([cp](int c) { return cp[c * T]; }, sm.thr, sm.thr + 16, (int)n_lev_f);
+    while (fb) { const int c = __ffsll((long long)fb) - 1; cp[c * T] = LOF_MARK; fb &= fb - 1; }
   }
 }
 
-// ---- F, 64 channels: two lanes per time column.  Lane l of the warp holds column p = l & 15 of the warp's 16
-// columns, channels [32h, 32h+32) with h = l >> 4; the lane holding the other half is l ^ 16.  Same doubling
-// as lof_col_flag with half the registers per thread (16 warps per SM instead of 12) and half the columns per
-// task (48 tasks per stream instead of 24: a shorter wait at the barrier that ends the pass).  Windows that
-// start in the lower half reach into the upper half through shuffles of the upper half's first D sums; a
-// window that would leave the column gets -inf and never fires.
-template <int D>
-__device__ __forceinline__ void lof_pcol_step(float (&u)[32], __half2 (&e2)[16], int h) {
-  if constexpr (D == 1) {
-    float pu = __shfl_xor_sync(0xffffffffu, u[0], 16);
-    const uint32_t pe = __shfl_xor_sync(0xffffffffu, lof_bits_h2(e2[0]), 16);
-    if (h) pu = -INFINITY;
-#pragma unroll
-    for (int j = 0; j < 32; ++j) u[j] += (j + 1 < 32) ? u[j + 1] : pu;
-#pragma unroll
-    for (int m = 0; m < 16; ++m)
-      e2[m] = __hadd2(e2[m], lof_h2_shift1(e2[m], (m + 1 < 16) ? e2[m + 1] : lof_h2_bits(pe)));
-  } else {
-    float pu[D];
-    uint32_t pe[D / 2];
-#pragma unroll
-    for (int jj = 0; jj < D; ++jj) {
-      pu[jj] = __shfl_xor_sync(0xffffffffu, u[jj], 16);
-      if (h) pu[jj] = -INFINITY;
-      if ((jj & 1) == 0) pe[jj / 2] = __shfl_xor_sync(0xffffffffu, lof_bits_h2(e2[jj / 2]), 16);
-    }
-#pragma unroll
-    for (int j = 0; j < 32; ++j) u[j] += (j + D < 32) ? u[j + D] : pu[j + D - 32];
-#pragma unroll
-    for (int m = 0; m < 16; ++m)
-      e2[m] = __hadd2(e2[m], (2 * m + D < 32) ? e2[m + D / 2] : lof_h2_bits(pe[(2 * m + D - 32) / 2]));
-  }
-}
-
-// Test of iteration I = 2^K <= 32 after its doubling step.  Returns (warp-uniform) whether any flag is new;
-// `dead` as in lof_col_eval.
-template <int K>
-__device__ __forceinline__ bool lof_pcol_eval(const float (&u)[32], const __half2 (&e2)[16], int h, float thr,
-                                              float tdead, uint32_t& fb, bool& dead) {
-  constexpr int I = 1 << K;
-  const float negT = -thr, negD = -tdead;
-  float tm[2] = {-INFINITY, -INFINITY}, td[2] = {-INFINITY, -INFINITY};
-#pragma unroll
-  for (int m = 0; m < 16; ++m) {
-    const float2 ef = __half22float2(e2[m]);
-    tm[m & 1] = lof_max3(tm[m & 1], fmaf(ef.x, negT, u[2 * m]), fmaf(ef.y, negT, u[2 * m + 1]));
-    td[m & 1] = lof_max3(td[m & 1], fmaf(ef.x, negD, u[2 * m]), fmaf(ef.y, negD, u[2 * m + 1]));
-  }
-  dead = __all_sync(0xffffffffu, fmaxf(td[0], td[1]) <= 0.f);
-  const bool fired = fmaxf(tm[0], tm[1]) > 0.f;
-  if (!__any_sync(0xffffffffu, fired)) return false;
-  uint32_t tg[4] = {0u, 0u, 0u, 0u};                       // partial masks: no serial chain
-  if (fired) {
-#pragma unroll
-    for (int m = 0; m < 16; ++m) {
-      const float2 ef = __half22float2(e2[m]);
-      tg[m & 1] |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
-      tg[2 + (m & 1)] |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
-    }
-  }
-  const uint32_t trig = (tg[0] | tg[1]) | (tg[2] | tg[3]);
-  uint64_t dil = trig;
-#pragma unroll
-  for (int s = 1; s < I; s <<= 1) dil |= dil << s;
-  // windows started in the lower half reach into the upper half
-  const uint32_t spill = __shfl_xor_sync(0xffffffffu, (uint32_t)(dil >> 32), 16);
-  const uint32_t nf = fb | (uint32_t)dil | (h ? spill : 0u);
-  const bool changed = nf != fb;
-  fb = nf;
-  return __any_sync(0xffffffffu, changed);
-}
-
-// The frequency run of 16 columns x 64 channels by one warp: ld(j) returns this lane's sample of channel
-// 32h + j (called again on a restart).  Returns the lane's flag mask (bit j = channel 32h + j).
-template <class Ld>
-__device__ __forceinline__ uint32_t lof_pcol_flag(Ld ld, const float* thr, const float* dead, int nlf, int h) {
-  float u[32];
-  __half2 e2[16];
-  uint32_t fb = 0;
-  const float T0 = thr[0], D0 = dead[0];
-  int k_next = 1;
-#pragma unroll 1
-  for (;;) {
-    float m0 = -INFINITY, m1 = -INFINITY;
-#pragma unroll
-    for (int j = 0; j < 32; j += 4) {
-      u[j] = ld(j); u[j + 1] = ld(j + 1); u[j + 2] = ld(j + 2); u[j + 3] = ld(j + 3);
-      m0 = lof_max3(m0, u[j], u[j + 1]); m1 = lof_max3(m1, u[j + 2], u[j + 3]);
-      e2[j / 2] = lof_h2_bits(LOF_H2_ONES); e2[j / 2 + 1] = lof_h2_bits(LOF_H2_ONES);
-    }
-    float mu = fmaxf(m0, m1);                             // largest unflagged sample of this half column
-    if (fb != 0 || mu > T0) {
-      uint32_t g[4] = {0u, 0u, 0u, 0u};
-#pragma unroll
-      for (int j = 0; j < 32; ++j) g[j & 3] |= (u[j] > T0) ? (1u << j) : 0u;
-      fb |= (g[0] | g[1]) | (g[2] | g[3]);
-#pragma unroll
-      for (int j = 0; j < 32; ++j) u[j] = ((fb >> j) & 1u) ? 0.f : u[j];
-#pragma unroll
-      for (int m = 0; m < 16; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
-      float a0 = 0.f, a1 = 0.f;                            // flagged samples count as 0 <= D0 (D0 > 0, or no exit)
-#pragma unroll
-      for (int j = 0; j < 32; j += 4) { a0 = lof_max3(a0, u[j], u[j + 1]); a1 = lof_max3(a1, u[j + 2], u[j + 3]); }
-      mu = fmaxf(a0, a1);
-    }
-    if (__all_sync(0xffffffffu, mu <= D0)) break;         // lof_dead_level: no later iteration can flag anything
-#define LOF_PCOL_LEVEL(K)                                                          \
-    if (K >= nlf) break;                                                           \
-    lof_pcol_step<(1 << (K - 1))>(u, e2, h);                                       \
-    if (K >= k_next) {                                                             \
-      bool dead_;                                                                  \
-      if (lof_pcol_eval<K>(u, e2, h, thr[K], dead[K], fb, dead_) && K + 1 < nlf) { \
-        k_next = K + 1; LOF_PROF_CNT(6);                                            \
-        continue;                                                                  \
-      }                                                                            \
-      if (dead_) break;                                                            \
-    }
-    LOF_PCOL_LEVEL(1) LOF_PCOL_LEVEL(2) LOF_PCOL_LEVEL(3) LOF_PCOL_LEVEL(4) LOF_PCOL_LEVEL(5)
-#undef LOF_PCOL_LEVEL
-    if (6 < nlf) {
-      // I = 64: the one window that is the whole column
-      const float ub = __shfl_xor_sync(0xffffffffu, u[0], 16);
-      const float eb = __shfl_xor_sync(0xffffffffu, __low2float(e2[0]), 16);
-      const float v = (u[0] + ub) - (__low2float(e2[0]) + eb) * thr[6];
-      if (v > 0.f) fb = 0xFFFFFFFFu;             // both lanes of the pair see the same v
-    }
-    break;
-  }
-  return fb;
-}
-
+// 64 channels: two lanes per column (lof_pcol_flag), 16 columns per task.
 template <int C, int L>
 __device__ void lof_fused_freq_pair(const LofFusedSmem& sm, uint32_t n_lev_f) {
   static_assert(C == 64, "two lanes per column: 64 channels");
   using Cfg = LofFusedCfg<C, L>;
-  constexpr int T = Cfg::T, W = Cfg::W;
+  constexpr int T = Cfg::T;
   const int lane = threadIdx.x & 31, h = lane >> 4, p = lane & 15;
-  uint16_t* fm16 = reinterpret_cast<uint16_t*>(sm.fm);
 #pragma unroll 1
   for (;;) {
     int g = 0;
@@ -766,175 +457,18 @@ __device__ void lof_fused_freq_pair(const LofFusedSmem& sm, uint32_t n_lev_f) {
     g = __shfl_sync(0xffffffffu, g, 0);
     if (g >= T / 16) break;
     const int col = g * 16 + p;
-    const float* cp = sm.xs + (32 * h) * T + lof_swz_elem(col);
-    const uint32_t fb = lof_pcol_flag([cp](int j) { return cp[j * T]; }, sm.thr, sm.thr + 16, (int)n_lev_f, h);
-    // 16 columns x 64 channels of flags -> half a mask word per channel: the ballot of bit j has channel j
-    // of the 16 columns in its low half and channel 32 + j in its high half; lane j keeps it
-    uint32_t mine = 0;
-    if (__any_sync(0xffffffffu, fb != 0)) {
-#pragma unroll
-      for (int j = 0; j < 32; ++j) {
-        const uint32_t word = __ballot_sync(0xffffffffu, (fb >> j) & 1u);
-        if (j == lane) mine = word;
-      }
-    }
-    const int w = g >> 1, half = g & 1;
-    fm16[(lane * W + w) * 2 + half] = (uint16_t)(mine & 0xFFFFu);
-    fm16[((lane + 32) * W + w) * 2 + half] = (uint16_t)(mine >> 16);
+    float* cp = sm.xs + (32 * h) * T + lof_swz_elem(col);
+    uint32_t fb = lof_pcol_flag([cp](int j) { return cp[j * T]; }, sm.thr, sm.thr + 16, (int)n_lev_f, h);
+    while (fb) { const int j = __ffs((int)fb) - 1; cp[j * T] = LOF_MARK; fb &= fb - 1; }
   }
 }
 
-// ---- T: SumThreshold along time.  One warp per channel row; lane l holds samples [l*L, l*L+L).
-// One doubling step of distance D (window 2D): partners beyond the lane's own L samples come from the
-// following lanes by shuffle.  A window that leaves the row picks up some lane's own sums instead (the shuffle
-// wraps): a harmless finite value, because a valid window only ever adds valid windows, and lof_row_eval drops
-// the window starts beyond T - I before they can flag anything.
-template <int L, int D>
-__device__ __forceinline__ void lof_row_step(float (&u)[L], __half2 (&e2)[L / 2], int lane) {
-  if constexpr (D == 1) {
-    const float pu = __shfl_down_sync(0xffffffffu, u[0], 1);
-    const uint32_t pe = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[0]), 1);
-#pragma unroll
-    for (int j = 0; j < L; ++j) u[j] += (j + 1 < L) ? u[j + 1] : pu;
-#pragma unroll
-    for (int m = 0; m < L / 2; ++m)
-      e2[m] = __hadd2(e2[m], lof_h2_shift1(e2[m], (m + 1 < L / 2) ? e2[m + 1] : lof_h2_bits(pe)));
-  } else {
-    constexpr int NP = D < L ? D : L;                   // elements whose partner lives in a following lane
-    float pu[NP];
-    uint32_t pe[NP / 2];
-#pragma unroll
-    for (int jj = 0; jj < NP; ++jj) {
-      const int j = L - NP + jj, src = (j + D) % L, off = (j + D) / L;
-      pu[jj] = __shfl_down_sync(0xffffffffu, u[src], off);
-      if ((jj & 1) == 0) pe[jj / 2] = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[src / 2]), off);
-    }
-#pragma unroll
-    for (int j = 0; j < L; ++j) u[j] += (j + D < L) ? u[j + D] : pu[j - (L - NP)];
-#pragma unroll
-    for (int m = 0; m < L / 2; ++m)
-      e2[m] = __hadd2(e2[m], (2 * m + D < L) ? e2[m + D / 2] : lof_h2_bits(pe[(2 * m - (L - NP)) / 2]));
-  }
-}
-
-// Test of iteration I = 2^K on a row after its doubling step: fire windows with u > e*T, dilate the fired
-// starts over I samples across lanes, OR into fb.  Returns (warp-uniform) whether any flag is new; `dead`
-// (warp-uniform) says that no window of I samples has an unflagged mean above `tdead` (lof_dead_level).
-template <int L, int K>
-__device__ __forceinline__ bool lof_row_eval(const float (&u)[L], const __half2 (&e2)[L / 2], int lane, float thr,
-                                             float tdead, uint32_t& fb, bool& dead) {
-  constexpr int I = 1 << K;
-  const float negT = -thr, negD = -tdead;
-  float tm[2] = {-INFINITY, -INFINITY}, td[2] = {-INFINITY, -INFINITY};
-#pragma unroll
-  for (int m = 0; m < L / 2; ++m) {
-    const float2 ef = __half22float2(e2[m]);
-    tm[m & 1] = lof_max3(tm[m & 1], fmaf(ef.x, negT, u[2 * m]), fmaf(ef.y, negT, u[2 * m + 1]));
-    td[m & 1] = lof_max3(td[m & 1], fmaf(ef.x, negD, u[2 * m]), fmaf(ef.y, negD, u[2 * m + 1]));
-  }
-  dead = __all_sync(0xffffffffu, fmaxf(td[0], td[1]) <= 0.f);
-  if (!__any_sync(0xffffffffu, fmaxf(tm[0], tm[1]) > 0.f)) return false;
-  uint32_t tg[4] = {0u, 0u, 0u, 0u};                       // partial masks: no serial chain
-#pragma unroll
-  for (int m = 0; m < L / 2; ++m) {
-    const float2 ef = __half22float2(e2[m]);
-    tg[m & 1] |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
-    tg[2 + (m & 1)] |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
-  }
-  uint32_t trig = (tg[0] | tg[1]) | (tg[2] | tg[3]);
-  {
-    // only windows that lie inside the row: starts t = lane*L + j <= 32*L - I
-    int nv = 32 * L - I + 1 - lane * L;
-    nv = nv < 0 ? 0 : (nv > L ? L : nv);
-    trig &= nv >= 32 ? 0xFFFFFFFFu : ((1u << nv) - 1u);
-  }
-  // own windows, inside the lane's L bits
-  uint32_t own = trig;
-#pragma unroll
-  for (int s = 1; s < I && s < 32; s <<= 1) own |= own << s;
-  // windows started in earlier lanes: sample p is covered iff p < (last start before this lane) + I
-  const int hi = trig ? (lane * L + 31 - __clz(trig)) : -(1 << 20);
-  int pm = hi;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pm, o); if (lane >= o) pm = max(pm, v); }
-  int prev = __shfl_up_sync(0xffffffffu, pm, 1);
-  if (lane == 0) prev = -(1 << 20);
-  int cnt = prev + I - lane * L;
-  cnt = cnt < 0 ? 0 : (cnt > L ? L : cnt);
-  const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
-  const uint32_t pre = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
-  const uint32_t nf = (fb | own | pre) & maskL;
-  const bool changed = nf != fb;
-  fb = nf;
-  return __any_sync(0xffffffffu, changed);
-}
-
-// The time run of one row segment held by a warp (lane l: samples [l*L, l*L+L) in x[]): level 0, then the
-// doubling levels with restarts and the early exit of lof_dead_level.  fb enters as the mask so far and leaves
-// as the final mask.  `after_level0` is called once, right after the first level 0 has consumed every x[j].
-// Returns true when `lane_sum` holds the sum of the lane's unflagged samples under the final mask (the run
-// ended at a level 0, whose u[] is exactly that: four strided partial sums, then (p0+p1)+(p2+p3)).
-// Warp-uniform control flow.
-template <int L, class Hook>
-__device__ __forceinline__ bool lof_row_flag(const float (&x)[L], uint32_t& fb, const float* thr, const float* dead,
-                                             int nlt, int lane, Hook after_level0, float& lane_sum) {
-  const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
-  float u[L];
-  __half2 e2[L / 2];
-  const float T0 = thr[0], D0 = dead[0];
-  int k_next = 1;
-#pragma unroll 1
-  for (;;) {
-    // level 0 (I = 1) under the current mask: x > threshold_1 on samples not yet flagged
-    {
-      // four independent partial masks: no serial chain through fb
-      uint32_t g[4] = {0u, 0u, 0u, 0u};
-#pragma unroll
-      for (int j = 0; j < L; ++j) g[j & 3] |= (x[j] > T0) ? (1u << j) : 0u;
-      fb |= (g[0] | g[1]) | (g[2] | g[3]);
-#pragma unroll
-      for (int j = 0; j < L; ++j) u[j] = ((fb >> j) & 1u) ? 0.f : x[j];
-    }
-    if (k_next == 1) after_level0();
-    // the largest unflagged sample (flagged ones count as 0 <= D0: D0 > 0, or there is no exit)
-    float a0 = 0.f, a1 = 0.f;
-#pragma unroll
-    for (int j = 0; j < L; j += 4) { a0 = lof_max3(a0, u[j], u[j + 1]); a1 = lof_max3(a1, u[j + 2], u[j + 3]); }
-    if (__all_sync(0xffffffffu, fmaxf(a0, a1) <= D0 || fb == maskL)) {
-      // nothing left that any later iteration could flag (lof_dead_level), or nothing left to test
-      float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
-#pragma unroll
-      for (int j = 0; j < L; j += 4) { p0 += u[j]; p1 += u[j + 1]; p2 += u[j + 2]; p3 += u[j + 3]; }
-      lane_sum = (p0 + p1) + (p2 + p3);
-      return true;
-    }
-#pragma unroll
-    for (int m = 0; m < L / 2; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
-    // one test per level on the way down: past the last level -> done; new flags with levels to go ->
-    // back to level 0 under the new mask (continue), re-doubling up to k_next without testing
-#define LOF_ROW_LEVEL(K)                                                                 \
-    if (K >= nlt) break;                                                                 \
-    lof_row_step<L, (1 << (K - 1))>(u, e2, lane);                                        \
-    if (K >= k_next) {                                                                   \
-      bool dead_;                                                                        \
-      if (lof_row_eval<L, K>(u, e2, lane, thr[K], dead[K], fb, dead_) && K + 1 < nlt) {  \
-        k_next = K + 1; LOF_PROF_CNT(7);                                                  \
-        continue;                                                                        \
-      }                                                                                  \
-      if (dead_) break;                                                                  \
-    }
-    LOF_ROW_LEVEL(1) LOF_ROW_LEVEL(2) LOF_ROW_LEVEL(3) LOF_ROW_LEVEL(4) LOF_ROW_LEVEL(5)
-    LOF_ROW_LEVEL(6) LOF_ROW_LEVEL(7) LOF_ROW_LEVEL(8) LOF_ROW_LEVEL(9)
-#undef LOF_ROW_LEVEL
-    break;
-  }
-  return false;
-}
-
+// ---- T: SumThreshold along time (lof_row_flag): one warp per channel row, then bit-pack and row sums.
 template <int C, int L>
-__device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, uint32_t s, bool have_f,
+__device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, uint32_t s,
                                uint32_t* __restrict__ flags, double* __restrict__ rowsum,
-                               uint32_t* __restrict__ rowcnt, const float* __restrict__ next_stream,
+                               uint32_t* __restrict__ rowcnt, const float* __restrict__ this_stream,
+                               const float* __restrict__ next_stream,
                                const LofStatPlan& plan_next, unsigned bar_parity) {
   using Cfg = LofFusedCfg<C, L>;
   constexpr int T = Cfg::T, NT = Cfg::NT, W = Cfg::W, NW = NT / 32;
@@ -950,22 +484,18 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
     if (lane == 0) c = (int)atomicAdd(&sm.ctl[CT_ROW], 1u);
     c = __shfl_sync(0xffffffffu, c, 0);
     if (c >= C) break;
-    float x[L];
+    // the row from shared memory (samples the frequency run flagged hold LOF_MARK there: the run starts from its
+    // mask, F10); as soon as it is in registers its slot takes the next stream's row.  A restart re-reads the raw
+    // row from global memory (every flag so far, the frequency run's included, is then in fb).
     const float4* rp = reinterpret_cast<const float4*>(sm.xs + c * T);
+    const float4* gp = reinterpret_cast<const float4*>(this_stream + c * T);
+    auto load = [&](float2 (&x2)[L / 2], bool again) {
 #pragma unroll
-    for (int q = 0; q < L / 4; ++q) {
-      const float4 v = rp[lof_swz_chunk(lane * (L / 4) + q)];
-      x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
-    }
-    uint32_t fb = 0;
-    if (have_f) {                                       // start from the frequency run's mask (F10)
-      const int b0 = lane * L, q = b0 >> 5, r = b0 & 31;
-      const uint32_t lo = sm.fm[c * W + q], hi = (q + 1 < W) ? sm.fm[c * W + q + 1] : 0u;
-      fb = __funnelshift_r(lo, hi, r) & maskL;
-    }
-    // as soon as level 0 has moved the row into registers its shared-memory slot takes the next stream's row
-    auto prefetch_row = [&]() {
-      if (next_stream) {
+      for (int q = 0; q < L / 4; ++q) {
+        const float4 v = again ? __ldg(gp + lane * (L / 4) + q) : rp[lof_swz_chunk(lane * (L / 4) + q)];
+        x2[2 * q] = make_float2(v.x, v.y); x2[2 * q + 1] = make_float2(v.z, v.w);
+      }
+      if (!again && next_stream) {
         float4* dst = reinterpret_cast<float4*>(sm.xs + c * T);
         const float4* src = reinterpret_cast<const float4*>(next_stream + c * T);
 #pragma unroll
@@ -973,10 +503,11 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
         lof_mbar_arrive_on_copies(sm.rowbar + c);
       }
     };
+    // With the time direction off (n_lev_t = 0) level 0 alone runs, with a threshold only the marks exceed: it
+    // turns them into the mask and sums the rest.
+    uint32_t fb = 0;
     float lane_sum = 0.f;
-    bool have_sum = false;
-    if (nlt > 0) have_sum = lof_row_flag<L>(x, fb, sm.thr, sm.thr + 32, (int)nlt, lane, prefetch_row, lane_sum);
-    else prefetch_row();
+    lof_row_flag<L>(load, fb, nlt > 0 ? sm.thr : sm.thr + 48, sm.thr + 32, nlt > 0 ? (int)nlt : 1, lane, lane_sum);
     // bit-pack: word w of the row = bits [32w, 32w+32) gathered from the lanes' L-bit masks
     {
       const int q0 = (32 * lane) / L, r0 = 32 * lane - L * q0;
@@ -992,18 +523,7 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
       }
       if (lane < W) flags[((size_t)s * C + c) * W + lane] = word;
     }
-    // row sum of unflagged samples, fp32 within the lane, fp64 across lanes
-    if (!have_sum) {
-      float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
-#pragma unroll
-      for (int j = 0; j < L; j += 4) {
-        p0 += ((fb >> j) & 1u) ? 0.f : x[j];
-        p1 += ((fb >> (j + 1)) & 1u) ? 0.f : x[j + 1];
-        p2 += ((fb >> (j + 2)) & 1u) ? 0.f : x[j + 2];
-        p3 += ((fb >> (j + 3)) & 1u) ? 0.f : x[j + 3];
-      }
-      lane_sum = (p0 + p1) + (p2 + p3);
-    }
+    // row sum of unflagged samples: fp32 within the lane (lof_row_flag), fp64 across lanes
     double rs = (double)lane_sum;
     rs = lof_warp_sum(rs);
     uint32_t nf = __popc(fb);
@@ -1093,7 +613,7 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
     LofStatPlan plan_next;
     if (Cfg::OVL) plan_next = lof_stat_plan<NT>(sample_next, reinterpret_cast<float*>(sm.red));
     LOF_PROF_T(t3);
-    lof_fused_time<C, L>(sm, prm, s, have_f, flags, rowsum, rowcnt, next, plan_next, bar_parity);
+    lof_fused_time<C, L>(sm, prm, s, flags, rowsum, rowcnt, power + (size_t)s * N, next, plan_next, bar_parity);
     if (more) bar_parity ^= 1u;
     lof_cp_async_wait_all();
     __syncthreads();

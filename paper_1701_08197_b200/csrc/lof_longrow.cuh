@@ -8,7 +8,7 @@
 //                      are independent; lane l holds samples [32 l, 32 l + 32).
 #pragma once
 #include "lof_common.cuh"
-#include "lof_fused.cuh"
+#include "lof_core.cuh"
 
 #define LOF_LR_THREADS 256
 #define LOF_LR_WARPS (LOF_LR_THREADS / 32)
@@ -41,6 +41,19 @@ lof_k_freq_reg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
 __device__ __forceinline__ int lof_lr_swz(int i) {
   const int g = i >> 2;
   return ((g ^ ((g >> 3) & 7)) << 2) | (i & 3);
+}
+
+// sum of the samples of a lane's word that are not in `skip` (the lane's share of PAPER.md:102's row mean)
+__device__ __forceinline__ float lof_sum_unflagged(const float2 (&x2)[16], uint32_t skip) {
+  float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
+#pragma unroll
+  for (int m = 0; m < 16; m += 2) {
+    p0 += ((skip >> (2 * m)) & 1u) ? 0.f : x2[m].x;
+    p1 += ((skip >> (2 * m + 1)) & 1u) ? 0.f : x2[m].y;
+    p2 += ((skip >> (2 * m + 2)) & 1u) ? 0.f : x2[m + 1].x;
+    p3 += ((skip >> (2 * m + 3)) & 1u) ? 0.f : x2[m + 1].y;
+  }
+  return (p0 + p1) + (p2 + p3);
 }
 
 template <class In>
@@ -81,34 +94,33 @@ lof_k_time_seg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
     }
   }
   __syncwarp();
-  float x[32];
+  // the lane's 32 samples from the staging strip (again on a restart: the strip keeps the raw samples)
+  auto load = [&](float2 (&x2)[16], bool) {
 #pragma unroll
-  for (int q = 0; q < 8; ++q) {
-    const float4 v = reinterpret_cast<const float4*>(sg)[(8 * lane + q) ^ (lane & 7)];
-    x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
-  }
+    for (int q = 0; q < 8; ++q) {
+      const float4 v = reinterpret_cast<const float4*>(sg)[(8 * lane + q) ^ (lane & 7)];
+      x2[2 * q] = make_float2(v.x, v.y); x2[2 * q + 1] = make_float2(v.z, v.w);
+    }
+  };
   const uint32_t t_w = t_lo + 32 * lane;                  // first sample of this lane's word
   const uint32_t valid = t_w >= T ? 0u : (T - t_w >= 32 ? 0xFFFFFFFFu : ((1u << (T - t_w)) - 1u));
+  // start from the frequency run's mask (F10): its flagged samples enter the row core as LOF_MARK
   uint32_t fb = 0;
-  if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];   // start from the frequency run's mask (F10)
+  if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];
   float lane_sum = 0.f;
   bool have_sum = false;
   if (st.nonfinite) fb = valid;                           // DESIGN.md S6: the whole stream is flagged
-  else if (prm.n_lev_t > 0) have_sum = lof_row_flag<32>(x, fb, st.thr_f, st.dead_t, (int)prm.n_lev_t, lane, [] {}, lane_sum);
+  else if (prm.n_lev_t > 0) {
+    lof_row_flag<32>(load, fb, st.thr_f, st.dead_t, (int)prm.n_lev_t, lane, lane_sum);
+    have_sum = true;
+  }
   fb &= valid;
   const bool mine = t_w >= o_lo && t_w < o_hi;            // this lane's word belongs to the segment's output
   if (mine) flags[row * W + (t_w >> 5)] = fb;
-  if (!have_sum || valid != 0xFFFFFFFFu) {                // (a word beyond the row's end holds -inf samples)
-    float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
-    const uint32_t skip = fb | ~valid;
-#pragma unroll
-    for (int j = 0; j < 32; j += 4) {
-      p0 += ((skip >> j) & 1u) ? 0.f : x[j];
-      p1 += ((skip >> (j + 1)) & 1u) ? 0.f : x[j + 1];
-      p2 += ((skip >> (j + 2)) & 1u) ? 0.f : x[j + 2];
-      p3 += ((skip >> (j + 3)) & 1u) ? 0.f : x[j + 3];
-    }
-    lane_sum = (p0 + p1) + (p2 + p3);
+  if (!have_sum || valid != 0xFFFFFFFFu) {                // (-inf beyond the row's end)
+    float2 x2[16];
+    load(x2, true);
+    lane_sum = lof_sum_unflagged(x2, fb | ~valid);
   }
   double rs = mine ? (double)lane_sum : 0.0;
   rs = lof_warp_sum(rs);
@@ -135,58 +147,60 @@ lof_k_time_seg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
 struct LofCoopSmem {
   float stage[LOF_CO_WARPS][LOF_LR_TILE];               // load staging, one 1024-sample strip per warp
   float bu[2][LOF_CO_WARPS][256];                       // published window sums (double-buffered by level)
-  uint32_t be[2][LOF_CO_WARPS][128];                    // published counts (packed halves)
+  float be[2][LOF_CO_WARPS][256];                       // published counts
   int wmax[LOF_CO_WARPS];                               // last fired window start per warp
 };
 
+// One doubling step of distance D on a strip of 1024 samples (lane l: 32 samples as 16 pairs); partners beyond
+// the strip come from the next warp's published sums nb_u / nb_e (its first D positions), or do not exist.
 template <int D>
-__device__ __forceinline__ void lof_row_step_coop(float (&u)[32], __half2 (&e2)[16], int lane, const float* nb_u,
-                                                  const uint32_t* nb_e, bool has_nb) {
+__device__ __forceinline__ void lof_row_step_coop(float2 (&u2)[16], float2 (&e2)[16], int lane, const float* nb_u,
+                                                  const float* nb_e, bool has_nb) {
   if constexpr (D == 1) {
-    float pu = __shfl_down_sync(0xffffffffu, u[0], 1);
-    uint32_t pe = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[0]), 1);
-    if (lane == 31) { pu = has_nb ? nb_u[0] : -INFINITY; pe = has_nb ? nb_e[0] : 0u; }
+    float pu = __shfl_down_sync(0xffffffffu, u2[0].x, 1);
+    float pe = __shfl_down_sync(0xffffffffu, e2[0].x, 1);
+    if (lane == 31) { pu = has_nb ? nb_u[0] : -INFINITY; pe = has_nb ? nb_e[0] : 0.f; }
 #pragma unroll
-    for (int j = 0; j < 32; ++j) u[j] += (j + 1 < 32) ? u[j + 1] : pu;
-#pragma unroll
-    for (int m = 0; m < 16; ++m)
-      e2[m] = __hadd2(e2[m], lof_h2_shift1(e2[m], (m + 1 < 16) ? e2[m + 1] : lof_h2_bits(pe)));
-  } else {
-    constexpr int NP = D < 32 ? D : 32;
-    float pu[NP];
-    uint32_t pe[NP / 2];
-#pragma unroll
-    for (int jj = 0; jj < NP; ++jj) {
-      const int j = 32 - NP + jj, src = (j + D) % 32, off = (j + D) / 32;
-      pu[jj] = __shfl_down_sync(0xffffffffu, u[src], off);
-      if ((jj & 1) == 0) pe[jj / 2] = __shfl_down_sync(0xffffffffu, lof_bits_h2(e2[src / 2]), off);
-      if (lane + off > 31) {                            // the partner lives in the next warp's strip
-        const int p = (lane + off - 32) * 32 + src;     // its position there, < D
-        pu[jj] = has_nb ? nb_u[p] : -INFINITY;
-        if ((jj & 1) == 0) pe[jj / 2] = has_nb ? nb_e[p >> 1] : 0u;
-      }
+    for (int m = 0; m < 16; ++m) {
+      u2[m].x += u2[m].y; e2[m].x += e2[m].y;
+      u2[m].y += (m + 1 < 16) ? u2[m + 1].x : pu; e2[m].y += (m + 1 < 16) ? e2[m + 1].x : pe;
     }
+  } else {
+    constexpr int H = D / 2;                              // distance in pairs
+    constexpr int NQ = H < 16 ? H : 16;
+    // one tree at a time (the partners fetched from other lanes are live for one of them only)
+    auto one = [&](float2 (&a2)[16], const float* nb, float none) {
+      float2 pa[NQ];
 #pragma unroll
-    for (int j = 0; j < 32; ++j) u[j] += (j + D < 32) ? u[j + D] : pu[j - (32 - NP)];
+      for (int q = 0; q < NQ; ++q) {
+        const int m = 16 - NQ + q, src = (m + H) % 16, off = (m + H) / 16;
+        pa[q].x = __shfl_down_sync(0xffffffffu, a2[src].x, off); pa[q].y = __shfl_down_sync(0xffffffffu, a2[src].y, off);
+        if (lane + off > 31) {                            // the partner lives in the next warp's strip
+          const int p = (lane + off - 32) * 32 + 2 * src; // its position there, < D (even)
+          pa[q] = has_nb ? *reinterpret_cast<const float2*>(nb + p) : make_float2(none, none);
+        }
+      }
 #pragma unroll
-    for (int m = 0; m < 16; ++m)
-      e2[m] = __hadd2(e2[m], (2 * m + D < 32) ? e2[m + D / 2] : lof_h2_bits(pe[(2 * m - (32 - NP)) / 2]));
+      for (int m = 0; m < 16; ++m) a2[m] = __fadd2_rn(a2[m], (m + H < 16) ? a2[m + H] : pa[m - (16 - NQ)]);
+    };
+    one(u2, nb_u, -INFINITY);
+    one(e2, nb_e, 0.f);
   }
 }
 
 // Test of iteration I = 2^K on a strip; like lof_row_eval, but windows fired in previous warps' strips dilate
 // into this one (carry through wmax[]), and "any" is taken over the CTA.  Contains __syncthreads: CTA-uniform.
 template <int K>
-__device__ __forceinline__ bool lof_row_eval_coop(const float (&u)[32], const __half2 (&e2)[16], int lane, int warp,
+__device__ __forceinline__ bool lof_row_eval_coop(const float2 (&u2)[16], const float2 (&e2)[16], int lane, int warp,
                                                   float thr, float tdead, uint32_t& fb, int* wmax, bool& dead) {
   constexpr int I = 1 << K;
-  const float negT = -thr, negD = -tdead;
+  const float2 negT = make_float2(-thr, -thr), negD = make_float2(-tdead, -tdead);
   float tm[2] = {-INFINITY, -INFINITY}, td[2] = {-INFINITY, -INFINITY};
 #pragma unroll
   for (int m = 0; m < 16; ++m) {
-    const float2 ef = __half22float2(e2[m]);
-    tm[m & 1] = lof_max3(tm[m & 1], fmaf(ef.x, negT, u[2 * m]), fmaf(ef.y, negT, u[2 * m + 1]));
-    td[m & 1] = lof_max3(td[m & 1], fmaf(ef.x, negD, u[2 * m]), fmaf(ef.y, negD, u[2 * m + 1]));
+    const float2 v = __ffma2_rn(e2[m], negT, u2[m]), w = __ffma2_rn(e2[m], negD, u2[m]);
+    tm[m & 1] = lof_max3(tm[m & 1], v.x, v.y);
+    td[m & 1] = lof_max3(td[m & 1], w.x, w.y);
   }
   // one barrier decides the usual case (nothing fired, and no window of I samples has an unflagged mean above
   // tdead: the tile is done, lof_dead_level); a second one tells the two apart otherwise
@@ -197,9 +211,8 @@ __device__ __forceinline__ bool lof_row_eval_coop(const float (&u)[32], const __
   uint32_t tg[4] = {0u, 0u, 0u, 0u};                       // partial masks: no serial chain
 #pragma unroll
   for (int m = 0; m < 16; ++m) {
-    const float2 ef = __half22float2(e2[m]);
-    tg[m & 1] |= (fmaf(ef.x, negT, u[2 * m]) > 0.f) ? (1u << (2 * m)) : 0u;
-    tg[2 + (m & 1)] |= (fmaf(ef.y, negT, u[2 * m + 1]) > 0.f) ? (2u << (2 * m)) : 0u;
+    tg[m & 1] |= (fmaf(e2[m].x, -thr, u2[m].x) > 0.f) ? (1u << (2 * m)) : 0u;
+    tg[2 + (m & 1)] |= (fmaf(e2[m].y, -thr, u2[m].y) > 0.f) ? (2u << (2 * m)) : 0u;
   }
   const uint32_t trig = (tg[0] | tg[1]) | (tg[2] | tg[3]);
   uint32_t own = trig;
@@ -263,63 +276,61 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
     }
   }
   __syncwarp();
-  float x[32];
+  auto load = [&](float2 (&x2)[16]) {
 #pragma unroll
-  for (int q = 0; q < 8; ++q) {
-    const float4 v = reinterpret_cast<const float4*>(sg)[(8 * lane + q) ^ (lane & 7)];
-    x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
-  }
+    for (int q = 0; q < 8; ++q) {
+      const float4 v = reinterpret_cast<const float4*>(sg)[(8 * lane + q) ^ (lane & 7)];
+      x2[2 * q] = make_float2(v.x, v.y); x2[2 * q + 1] = make_float2(v.z, v.w);
+    }
+  };
   const uint32_t t_w = t_lo + 32 * lane;
   const uint32_t valid = t_w >= T ? 0u : (T - t_w >= 32 ? 0xFFFFFFFFu : ((1u << (T - t_w)) - 1u));
   uint32_t fb = 0;
-  if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];
+  if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];   // the frequency run's flags (F10)
   const int nlt = (int)prm.n_lev_t;
+  float lane_sum = 0.f;
+  bool have_sum = false;
   if (st.nonfinite) fb = valid;
   else if (nlt > 0) {
     const float* thr = st.thr_f;
     const float* dead = st.dead_t;
     const float T0 = thr[0], D0 = dead[0];
-    float u[32];
-    __half2 e2[16];
+    float2 u2[16], e2[16];
     int k_next = 1;
     bool again = true;
     const bool has_nb = warp + 1 < LOF_CO_WARPS;
+    have_sum = true;
 #pragma unroll 1
     while (again) {
+      float mu = 0.f;
       {
-        uint32_t g[4] = {0u, 0u, 0u, 0u};                  // partial masks: no serial chain through fb
-#pragma unroll
-        for (int j = 0; j < 32; ++j) g[j & 3] |= (x[j] > T0) ? (1u << j) : 0u;
-        fb |= (g[0] | g[1]) | (g[2] | g[3]);
-#pragma unroll
-        for (int j = 0; j < 32; ++j) u[j] = ((fb >> j) & 1u) ? 0.f : x[j];
+        float2 x2[16];
+        load(x2);
+        if (fb) lof_mark<16>(x2, fb);                     // flags of the frequency run and of earlier restarts
+        fb = ~lof_level0<16>(x2, T0, u2, e2, mu);
       }
-      {
-        // largest unflagged sample of the tile (flagged ones count as 0): lof_dead_level at level 0
-        float a0 = 0.f, a1 = 0.f;
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) { a0 = lof_max3(a0, u[j], u[j + 1]); a1 = lof_max3(a1, u[j + 2], u[j + 3]); }
-        if (__syncthreads_and(fmaxf(a0, a1) <= D0)) break;
-      }
-#pragma unroll
-      for (int m = 0; m < 16; ++m) e2[m] = lof_h2_unflagged((fb >> (2 * m)) & 3u);
+      lane_sum = lof_lane_sum<16>(u2);
+      // no iteration left, or no unflagged sample of the tile above every later threshold (lof_dead_level)
+      if (k_next >= nlt || __syncthreads_and(mu <= D0)) break;
       again = false;
       bool dead_ = false;
 #define LOF_CO_LEVEL(K)                                                                          \
       if (K < nlt && !again && !dead_) {                                                         \
         constexpr int D = 1 << (K - 1);                                                          \
-        float* pbu = sm.bu[K & 1][warp]; uint32_t* pbe = sm.be[K & 1][warp];                     \
+        float* pbu = sm.bu[K & 1][warp]; float* pbe = sm.be[K & 1][warp];                        \
         /* publish the first D sums / counts of this strip for the previous warp */             \
         if (lane * 32 < D) {                                                                     \
-          _Pragma("unroll") for (int j = 0; j < 32; ++j) if (lane * 32 + j < D) pbu[lane * 32 + j] = u[j];        \
-          _Pragma("unroll") for (int m = 0; m < 16; ++m) if (lane * 32 + 2 * m < D) pbe[lane * 16 + m] = lof_bits_h2(e2[m]); \
+          _Pragma("unroll") for (int m = 0; m < 16; ++m) if (lane * 32 + 2 * m < D) {            \
+            if (D == 1) { pbu[0] = u2[0].x; pbe[0] = e2[0].x; }                                  \
+            else { *reinterpret_cast<float2*>(pbu + lane * 32 + 2 * m) = u2[m];                  \
+                   *reinterpret_cast<float2*>(pbe + lane * 32 + 2 * m) = e2[m]; }                \
+          }                                                                                      \
         }                                                                                        \
         __syncthreads();                                                                         \
-        lof_row_step_coop<D>(u, e2, lane, sm.bu[K & 1][has_nb ? warp + 1 : warp],                \
+        lof_row_step_coop<D>(u2, e2, lane, sm.bu[K & 1][has_nb ? warp + 1 : warp],               \
                              sm.be[K & 1][has_nb ? warp + 1 : warp], has_nb);                    \
-        if (K >= k_next && lof_row_eval_coop<K>(u, e2, lane, warp, thr[K], dead[K], fb, sm.wmax, dead_) && \
-            K + 1 < nlt) {                                                                       \
-          again = true; k_next = K + 1;                                                          \
+        if (K >= k_next && lof_row_eval_coop<K>(u2, e2, lane, warp, thr[K], dead[K], fb, sm.wmax, dead_)) { \
+          again = true; k_next = K + 1 < nlt ? K + 1 : 99;                                       \
         }                                                                                        \
       }
       LOF_CO_LEVEL(1) LOF_CO_LEVEL(2) LOF_CO_LEVEL(3) LOF_CO_LEVEL(4) LOF_CO_LEVEL(5)
@@ -331,16 +342,12 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
   fb &= valid;
   const bool mine = t_w >= o_lo && t_w < o_hi;
   if (mine) flags[row * W + (t_w >> 5)] = fb;
-  float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
-  const uint32_t skip = fb | ~valid;
-#pragma unroll
-  for (int j = 0; j < 32; j += 4) {
-    p0 += ((skip >> j) & 1u) ? 0.f : x[j];
-    p1 += ((skip >> (j + 1)) & 1u) ? 0.f : x[j + 1];
-    p2 += ((skip >> (j + 2)) & 1u) ? 0.f : x[j + 2];
-    p3 += ((skip >> (j + 3)) & 1u) ? 0.f : x[j + 3];
+  if (!have_sum || valid != 0xFFFFFFFFu) {
+    float2 x2[16];
+    load(x2);
+    lane_sum = lof_sum_unflagged(x2, fb | ~valid);
   }
-  double rs = mine ? (double)((p0 + p1) + (p2 + p3)) : 0.0;
+  double rs = mine ? (double)lane_sum : 0.0;
   rs = lof_warp_sum(rs);
   uint32_t nf = mine ? __popc(fb) : 0u, nu = mine ? __popc(valid & ~fb) : 0u;
 #pragma unroll

@@ -390,7 +390,7 @@ def test_fused_nonfinite_streams_inside_persistent_loop(lof, lofo, wl, C, T, mw)
 
 def test_path_used_reports_the_decomposition(lof):
     import torch
-    for (S, C, T, mw, want) in [(2, 64, 768, 64, "FUSED"), (2, 16, 256, 32, "FUSED"), (2, 64, 704, 64, "GENERIC"),
+    for (S, C, T, mw, want) in [(2, 64, 768, 64, "FUSED"), (2, 16, 256, 32, "FUSED"), (2, 64, 704, 64, "LONGROW_SEG"), (2, 48, 768, 64, "GENERIC"),
                                 (1, 16, 12208, 64, "LONGROW_SEG"), (1, 32, 20000, 256, "LONGROW_COOP"),
                                 (1, 32, 20000, 1024, "GENERIC"), (2, 5, 77, 8, "GENERIC")]:
         f = lof.Flagger(S, C, T, max_window=mw)

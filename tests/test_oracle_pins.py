@@ -407,3 +407,108 @@ def test_history_sensitivity_fallback_is_sensitivity(lofo):
     assert run(2.0, 1.0, 3.5)[0] == 1                               # explicit 1.0: threshold 2.8165
     assert run(0.5, 0.0, 2.5)[0] == 1                               # fallback to 0.5: threshold 2.408
     assert run(0.5, 0.0, 2.3)[0] == 0
+
+
+# ---------------------------------------------------------------- NEXT-1: SIR operator
+def _runs_to_mask(n, runs):
+    m = np.zeros(n, np.uint8)
+    for lo, hi in runs:
+        m[lo:hi] = 1
+    return m
+
+
+@pytest.mark.parametrize("case", HV["SIR"]["cases"], ids=lambda c: c["name"])
+def test_sir_hand_vectors(lofo, case):
+    got = lofo.sir_1d(_runs_to_mask(case["n"], case["in"]), HV["SIR"]["eta"])
+    assert list(got) == list(_runs_to_mask(case["n"], case["out"])), case["why"]
+
+
+def _sir_python(mask, eta):
+    """From-scratch transcription of PAPER.md:55: every run of the INPUT mask, floor(eta*len) on each side."""
+    m = [int(v) for v in mask]
+    n = len(m)
+    out = list(m)
+    i = 0
+    while i < n:
+        if not m[i]:
+            i += 1
+            continue
+        j = i
+        while j < n and m[j]:
+            j += 1
+        e = int(math.floor(float(np.float32(eta)) * (j - i)))
+        for k in range(max(0, i - e), i):
+            out[k] = 1
+        for k in range(j, min(n, j + e)):
+            out[k] = 1
+        i = j
+    return out
+
+
+def test_sir_equals_python_bruteforce_and_invariants(lofo):
+    rng = np.random.default_rng(55)
+    for trial in range(200):
+        n = int(rng.integers(1, 200))
+        dens = rng.choice([0.05, 0.3, 0.6, 0.9])
+        m = (rng.random(n) < dens).astype(np.uint8)
+        if trial % 3 == 0 and n > 20:                      # a few long runs
+            a = int(rng.integers(0, n - 10)); m[a:a + int(rng.integers(5, 60))] = 1
+        eta = float(rng.choice([0.2, 0.1, 0.5, 0.33, 1.0]))
+        got = lofo.sir_1d(m, eta)
+        assert list(got) == _sir_python(m, eta), (trial, eta)
+        assert (got >= m).all()                            # flags are only ever added
+        assert np.array_equal(lofo.sir_1d(m, 0.0), m)      # eta = 0 is the identity
+    # closed form: an isolated run of len samples far from the ends flags len + 2*floor(eta*len) samples
+    for ln in (1, 4, 5, 9, 10, 37, 100):
+        m = np.zeros(400, np.uint8); m[150:150 + ln] = 1
+        assert int(lofo.sir_1d(m, 0.2).sum()) == ln + 2 * (ln // 5)
+
+
+def test_sir_block_is_frequency_then_time(lofo):
+    v = HV["SIR"]["order_2d"]
+    M = np.array(v["in"], np.uint8)
+    Cn, T = M.shape
+    packed = np.zeros((1, Cn, 1), np.uint32)
+    for c in range(Cn):
+        for t in range(T):
+            packed[0, c, 0] |= np.uint32(int(M[c, t]) << t)
+    got = lofo.unpack_flags(lofo.sir_block(packed, T, 0.2), T)[0]
+    assert got.tolist() == v["out_freq_then_time"], v["why"]
+    assert np.array_equal(lofo.unpack_flags(lofo.sir_block(packed, T, 0.2, directions=2), T)[0], M)
+    # the block form is the 1-D form applied to every column, then to every row of the result (SIR-5), and the two
+    # orders differ on a random mask
+    rng = np.random.default_rng(57)
+    Cn, T = 24, 75
+    M = (rng.random((Cn, T)) < 0.55).astype(np.uint8)
+    W_ = (T + 31) // 32
+    packed = np.zeros((1, Cn, W_), np.uint32)
+    for c in range(Cn):
+        for t in range(T):
+            if M[c, t]:
+                packed[0, c, t >> 5] |= np.uint32(1 << (t & 31))
+    ft = M.copy()
+    for t in range(T):
+        ft[:, t] = lofo.sir_1d(ft[:, t], 0.2)
+    for c in range(Cn):
+        ft[c] = lofo.sir_1d(ft[c], 0.2)
+    tf = M.copy()
+    for c in range(Cn):
+        tf[c] = lofo.sir_1d(tf[c], 0.2)
+    for t in range(T):
+        tf[:, t] = lofo.sir_1d(tf[:, t], 0.2)
+    got = lofo.unpack_flags(lofo.sir_block(packed, T, 0.2), T)[0]
+    assert np.array_equal(got, ft) and not np.array_equal(ft, tf)
+    assert (lofo.sir_block(packed, T, 0.2)[0, :, -1] >> np.uint32(T % 32)).max() == 0     # padding bits stay 0
+
+
+def test_sir_inside_flag_block(lofo):
+    """sir_eta in lofo_flag_block: the SumThreshold mask, then the SIR operator on it; statistics and row sums are
+    those of the SumThreshold mask (the operator works on masks only; reading SIR-6)."""
+    w = W.config2(n_stations=2)
+    base = lofo.flag_block(lofo.make_params(w.S, w.C, w.T, max_window=64), w.power)
+    sir = lofo.flag_block(lofo.make_params(w.S, w.C, w.T, max_window=64, sir_eta=0.2), w.power)
+    assert np.array_equal(sir["flags"], lofo.sir_block(base["flags"], w.T, 0.2))
+    assert np.array_equal(sir["rowsum"], base["rowsum"]) and np.array_equal(sir["rowcnt"], base["rowcnt"])
+    pop = np.unpackbits(sir["flags"].view(np.uint8), axis=-1).reshape(w.S, -1).sum(axis=1)
+    assert np.array_equal(pop.astype(np.uint64), sir["stats"]["n_flagged"])
+    assert (sir["stats"]["n_flagged"] > base["stats"]["n_flagged"]).any()
