@@ -64,7 +64,17 @@ typedef struct {
                                    flagger; the paper's example is 300            */
   uint32_t history_min_fill;    /* below this many entries a ring only records (H3')   */
   float    history_sensitivity; /* <= 0: use `sensitivity`, the literal text of PAPER.md:106     */
+  float    sir_eta;             /* scale-invariant rank operator: every run of flagged
+                                   samples grows by floor(sir_eta * length) samples on each side, along
+                                   frequency and then along time (the directions set in `directions`);
+                                   0 = off, the paper's typical value is 0.2; in [0, 1]               */
+  uint32_t stats_mode;          /* LOF_STATS_PLAIN (0): stddev of all samples, as PAPER.md:41 is written;
+                                   LOF_STATS_MAD (1): 1.4826 * median absolute deviation in its place,
+                                   one of the robust statistics PAPER.md:120 lists (R1)     */
 } lof_params;
+
+#define LOF_STATS_PLAIN 0u
+#define LOF_STATS_MAD   1u
 
 /* Per-stream results of lof_flag_block (32 bytes, no padding surprises: 4+4+8+8+8). */
 typedef struct {
@@ -79,7 +89,7 @@ typedef struct {
 /* Validate params (LOF_E_PARAM when: struct_size mismatch; S, C or T zero; C > 256; max_window
  * zero, not a power of two or > 1024; directions zero or with unknown bits; p, sensitivity or
  * start_threshold not > 0 and finite; history_length > 0 with history_min_fill == 0 — an empty ring has no
- * mean; history_sensitivity not finite), select the device, allocate scratch and history rings
+ * mean; history_sensitivity not finite; sir_eta not in [0, 1]; stats_mode unknown), select the device, allocate scratch and history rings
  * (zero-filled, all rings empty).  *out receives the handle; on failure *out = NULL. */
 int lof_create(const lof_params* params, lof_ctx** out);
 
@@ -88,7 +98,9 @@ int lof_destroy(lof_ctx* ctx);
 
 /* One pass of the hot path over one block:
  *   statistics -> thresholds -> SumThreshold(frequency) -> SumThreshold(time) -> bit-pack,
- *   per-row sums of unflagged samples (kept inside the context for lof_history_update).
+ *   per-row sums of unflagged samples (kept inside the context for lof_history_update),
+ *   then, if sir_eta > 0, the SIR operator on the packed mask (it works on the mask only,
+ *   the row sums are those of the SumThreshold mask; n_flagged counts the final mask).
  * d_power [S][C][T] float32 (in), d_flags [S][C][ceil(T/32)] uint32 (out, fully overwritten),
  * d_stats [S] (out, may be NULL).  Asynchronous on cuda_stream. */
 int lof_flag_block(lof_ctx* ctx, const float* d_power, uint32_t* d_flags,

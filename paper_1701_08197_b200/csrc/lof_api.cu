@@ -13,6 +13,7 @@
 #include "lof_history.cuh"
 #include "lof_fused.cuh"
 #include "lof_longrow.cuh"
+#include "lof_sir.cuh"
 
 static thread_local char g_cuda_err[256] = "";
 
@@ -82,6 +83,8 @@ static int validate(const lof_params* p) {
   // an empty ring has no mean: with min_fill = 0 the first threshold would be 0/0 and every later one NaN
   if (p->history_length > 0 && p->history_min_fill == 0) return LOF_E_PARAM;
   if (!std::isfinite(p->history_sensitivity)) return LOF_E_PARAM;
+  if (!(p->sir_eta >= 0.f && p->sir_eta <= 1.f)) return LOF_E_PARAM;
+  if (p->stats_mode > LOF_STATS_MAD) return LOF_E_PARAM;
   return LOF_OK;
 }
 
@@ -379,6 +382,50 @@ static int flag_block_fused(lof_ctx* c, const float* d_power, uint32_t* d_flags,
 }
 static int flag_block_fused(lof_ctx*, const int16_t*, uint32_t*, cudaStream_t) { return 0; }
 
+// ---- SIR operator on the packed mask (lof_sir.cuh): frequency, then time; ping-pong between the caller's
+// flags and the context's mask buffer
+template <int G>
+static void sir_time_launch(const uint32_t* in, uint32_t* out, lof_ctx* c, cudaStream_t st) {
+  const uint64_t rows = (uint64_t)c->prm.n_streams * c->prm.n_channels;
+  const uint64_t threads = rows * G;
+  lof_k_sir_time<G><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(in, out, c->d_stats, rows, c->prm.n_channels,
+                                                                      c->kp.W, c->prm.n_time, c->prm.sir_eta);
+}
+
+static int sir_apply(lof_ctx* c, uint32_t* d_flags, cudaStream_t st) {
+  const float eta = c->prm.sir_eta;
+  if (!(eta > 0.f)) return LOF_OK;
+  const uint32_t C = c->prm.n_channels, W = c->kp.W;
+  const size_t words = (size_t)c->prm.n_streams * C * W;
+  uint32_t* cur = d_flags;
+  uint32_t* other = c->d_fmask;
+  if (c->prm.directions & LOF_DIR_FREQ) {
+    uint32_t m_min = 1;                                  // shortest run that grows at all
+    while (m_min <= C && (uint32_t)std::floor((double)eta * (double)m_min) == 0) ++m_min;
+    const uint64_t n_cols = (uint64_t)c->prm.n_streams * W;
+    lof_k_sir_freq<<<(unsigned)((n_cols + 255) / 256), 256, 0, st>>>(cur, other, c->d_stats, n_cols, C, W, eta, m_min);
+    c->launches += 1;
+    uint32_t* t = cur; cur = other; other = t;
+  }
+  if (c->prm.directions & LOF_DIR_TIME) {
+    uint32_t G = 1;
+    while (G < 32 && G * 8 < W) G <<= 1;                  // about eight words per lane
+    switch (G) {
+      case 1: sir_time_launch<1>(cur, other, c, st); break;
+      case 2: sir_time_launch<2>(cur, other, c, st); break;
+      case 4: sir_time_launch<4>(cur, other, c, st); break;
+      case 8: sir_time_launch<8>(cur, other, c, st); break;
+      case 16: sir_time_launch<16>(cur, other, c, st); break;
+      default: sir_time_launch<32>(cur, other, c, st); break;
+    }
+    c->launches += 1;
+    uint32_t* t = cur; cur = other; other = t;
+  }
+  LOF_CUDA(cudaGetLastError());
+  if (cur != d_flags) LOF_CUDA(cudaMemcpyAsync(d_flags, cur, words * 4, cudaMemcpyDeviceToDevice, st));
+  return LOF_OK;
+}
+
 template <class In>
 static int flag_block_any(lof_ctx* c, In in, uint32_t* d_flags, lof_stream_stats* d_stats, void* cuda_stream) {
   if (!c || !in.p || !d_flags) return LOF_E_NULL;
@@ -389,6 +436,8 @@ static int flag_block_any(lof_ctx* c, In in, uint32_t* d_flags, lof_stream_stats
   if (rc < 0) return rc;
   if (rc == 1) c->path_used = LOF_PATH_FUSED;
   if (rc == 0) { rc = flag_block_generic(c, in, d_flags, st); if (rc) return rc; }
+  rc = sir_apply(c, d_flags, st);
+  if (rc) return rc;
   if (d_stats)
     LOF_CUDA(cudaMemcpyAsync(d_stats, c->d_stats, (size_t)c->prm.n_streams * sizeof(lof_stream_stats),
                              cudaMemcpyDeviceToDevice, st));

@@ -474,7 +474,6 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
   constexpr int T = Cfg::T, NT = Cfg::NT, W = Cfg::W, NW = NT / 32;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t nlt = prm.n_lev_t;
-  const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
   uint32_t n_flag_acc = 0;
   (void)warp; (void)NW;
 #pragma unroll 1

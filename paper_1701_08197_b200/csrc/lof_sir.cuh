@@ -1,0 +1,179 @@
+// lof_sir.cuh — the scale-invariant rank operator as PAPER.md:49-57 states it: "all ranges of consecutive
+// flagged samples are extended by flagging 20% more samples, before and after the original range".  It "operates
+// on the flag masks only, and not on the actual data": two kernels on the bit-packed mask
+// uint32[S][C][W], frequency direction first, then time on the result (readings SIR-1..6):
+//   every maximal run of flagged samples of the INPUT mask of a pass, of length n, gets floor(eta * n) more
+//   samples flagged on each side, clipped at the ends of the line; run lengths are those of the input.
+// Both kernels read `in` and write `out` (different buffers), and add the bits they set to the stream's n_flagged.
+#pragma once
+#include "lof_common.cuh"
+
+__device__ __forceinline__ uint32_t lof_sir_ext(float eta, uint32_t n) {
+  return (uint32_t)floor((double)eta * (double)n);       // the oracle's expression, same IEEE operations
+}
+
+// first position q in [p, pend) whose bit equals `want` (pend if none); w = the row's words
+__device__ __forceinline__ uint32_t lof_sir_next(const uint32_t* __restrict__ w, uint32_t p, uint32_t pend, bool want) {
+  while (p < pend) {
+    uint32_t word = w[p >> 5];
+    if (!want) word = ~word;
+    word &= 0xFFFFFFFFu << (p & 31);
+    if (word) { const uint32_t q = (p & ~31u) + (uint32_t)__ffs((int)word) - 1u; return q < pend ? q : pend; }
+    p = (p & ~31u) + 32u;
+  }
+  return pend;
+}
+// number of consecutive set bits ending just before pend, looking back no further than p0
+__device__ __forceinline__ uint32_t lof_sir_trail(const uint32_t* __restrict__ w, uint32_t p0, uint32_t pend) {
+  uint32_t p = pend;
+  while (p > p0) {
+    const uint32_t wi = (p - 1) >> 5, hi = ((p - 1) & 31) + 1;            // bits [0, hi) of word wi are in range
+    uint32_t word = ~w[wi];
+    if (hi < 32) word &= (1u << hi) - 1u;
+    const uint32_t lo_pos = wi << 5;
+    if (lo_pos < p0) word &= 0xFFFFFFFFu << (p0 - lo_pos);
+    if (word) { const uint32_t z = lo_pos + 31u - (uint32_t)__clz((int)word); return pend - (z + 1u); }
+    if (lo_pos <= p0) break;
+    p = lo_pos;
+  }
+  return pend - p0;
+}
+// set bits [lo, hi) of the row's words
+__device__ __forceinline__ void lof_sir_set(uint32_t* __restrict__ w, uint32_t lo, uint32_t hi) {
+  while (lo < hi) {
+    const uint32_t wi = lo >> 5, b = lo & 31, e = min(hi - (wi << 5), 32u);
+    const uint32_t m = (e >= 32 ? 0xFFFFFFFFu : ((1u << e) - 1u)) & (0xFFFFFFFFu << b);
+    w[wi] |= m;
+    lo = (wi << 5) + 32u;
+  }
+}
+
+// Time direction.  G lanes (a power of two <= 32) share one row of T bits; lane j owns the words [j*B, j*B+B).
+// 1. per lane: is the block all ones, how many ones lead / trail it; scans across the G lanes give the length of
+//    the run that ends just left of the block (carry_in) and of the one that starts just right of it (carry_out);
+// 2. per lane: every run of the block with its full length (carries added); the lane in which a run really ends
+//    emits the right reach end + floor(eta n), the lane in which it really starts the left reach start - floor(..);
+//    an exclusive prefix maximum / suffix minimum over the lanes carries the reaches into the other blocks;
+// 3. per lane: out = in | own extensions | [block start, reach from the left) | [reach from the right, block end).
+template <int G>
+__global__ void __launch_bounds__(256)
+lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_stream_stats* __restrict__ stats,
+               uint64_t n_rows, uint32_t C, uint32_t W, uint32_t T, float eta) {
+  const uint64_t gid = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / G;
+  const int j = threadIdx.x % G;
+  const bool live = gid < n_rows;
+  const uint64_t row = live ? gid : n_rows - 1;           // idle groups shadow the last row and write nothing
+  const uint32_t* wi = in + row * W;
+  uint32_t* wo = out + row * W;
+  const uint32_t B = (W + G - 1) / G;
+  const uint32_t p0 = min((uint32_t)j * B * 32u, T), p1 = min(((uint32_t)j + 1u) * B * 32u, T), len = p1 - p0;
+  const unsigned gmask = (G == 32) ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
+  // 1. block summary and the carries
+  const uint32_t lead = lof_sir_next(wi, p0, p1, false) - p0;
+  const bool all = lead == len;
+  const uint32_t trail = all ? len : lof_sir_trail(wi, p0, p1);
+  uint32_t cin = 0, cout = 0;
+  if (G > 1) {
+    // inclusive scan of (all, trailing ones) from the left, then shifted by one lane; mirrored from the right
+    uint32_t t = trail; bool a = all;
+    uint32_t l = lead; bool b = all;
+#pragma unroll
+    for (int o = 1; o < G; o <<= 1) {
+      const uint32_t tl = __shfl_up_sync(gmask, t, o, G); const bool al = __shfl_up_sync(gmask, (int)a, o, G);
+      if (j >= o) { if (a) t += tl; a = a && al; }
+      const uint32_t lr = __shfl_down_sync(gmask, l, o, G); const bool br = __shfl_down_sync(gmask, (int)b, o, G);
+      if (j + o < G) { if (b) l += lr; b = b && br; }
+    }
+    cin = __shfl_up_sync(gmask, t, 1, G); if (j == 0) cin = 0;
+    cout = __shfl_down_sync(gmask, l, 1, G); if (j == G - 1) cout = 0;
+  }
+  // 2. runs of the block, reaches
+  int rmax = -1;                                          // exclusive end of the farthest right extension emitted here
+  int lmin = 0x7FFFFFFF;                                  // start of the farthest left extension emitted here
+  for (uint32_t p = p0; p < p1;) {
+    const uint32_t a = lof_sir_next(wi, p, p1, true);
+    if (a >= p1) break;
+    const uint32_t b = lof_sir_next(wi, a, p1, false);
+    const bool starts = a > p0 || cin == 0, ends = b < p1 || cout == 0;
+    const uint32_t n = (b - a) + (a == p0 ? cin : 0u) + (b == p1 ? cout : 0u);
+    const uint32_t e = lof_sir_ext(eta, n);
+    if (ends) rmax = max(rmax, (int)min(b + e, T));
+    if (starts) lmin = min(lmin, (int)(a > e ? a - e : 0u));
+    p = b;
+  }
+  int rin = -1, lin = 0x7FFFFFFF;
+  if (G > 1) {
+    int r = rmax, l = lmin;
+#pragma unroll
+    for (int o = 1; o < G; o <<= 1) {
+      const int rl = __shfl_up_sync(gmask, r, o, G); if (j >= o) r = max(r, rl);
+      const int lr = __shfl_down_sync(gmask, l, o, G); if (j + o < G) l = min(l, lr);
+    }
+    rin = __shfl_up_sync(gmask, r, 1, G); if (j == 0) rin = -1;
+    lin = __shfl_down_sync(gmask, l, 1, G); if (j == G - 1) lin = 0x7FFFFFFF;
+  }
+  if (!live) return;
+  // 3. output words of the block
+  const uint32_t w0 = (uint32_t)j * B, w1 = min(w0 + B, W);
+  uint32_t before = 0, after = 0;
+  for (uint32_t w = w0; w < w1; ++w) { const uint32_t v = wi[w]; wo[w] = v; before += __popc(v); }
+  for (uint32_t p = p0; p < p1;) {
+    const uint32_t a = lof_sir_next(wi, p, p1, true);
+    if (a >= p1) break;
+    const uint32_t b = lof_sir_next(wi, a, p1, false);
+    const bool starts = a > p0 || cin == 0, ends = b < p1 || cout == 0;
+    const uint32_t n = (b - a) + (a == p0 ? cin : 0u) + (b == p1 ? cout : 0u);
+    const uint32_t e = lof_sir_ext(eta, n);
+    if (ends && e) lof_sir_set(wo, b, min(b + e, p1));
+    if (starts && e) lof_sir_set(wo, max(a > e ? a - e : 0u, p0), a);
+    p = b;
+  }
+  if (rin > (int)p0) lof_sir_set(wo, p0, min((uint32_t)rin, p1));
+  if (lin < (int)p1) lof_sir_set(wo, max((uint32_t)max(lin, 0), p0), p1);
+  for (uint32_t w = w0; w < w1; ++w) after += __popc(wo[w]);
+  if (after != before)
+    atomicAdd(reinterpret_cast<unsigned long long*>(&stats[row / C].n_flagged), (unsigned long long)(after - before));
+}
+
+// Frequency direction.  One thread per (stream, word column): the C words in[c][w] carry 32 time samples each.
+// A run can only grow if it is at least m = ceil(1/eta) channels long: a bit-parallel screen (AND of m consecutive
+// words, OR over c) names the time samples that have such a run; only those columns are walked channel by channel.
+__global__ void __launch_bounds__(256)
+lof_k_sir_freq(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_stream_stats* __restrict__ stats,
+               uint64_t n_cols /* S*W */, uint32_t C, uint32_t W, float eta, uint32_t m_min) {
+  const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= n_cols) return;
+  const uint64_t s = gid / W;
+  const uint32_t w = (uint32_t)(gid - s * W);
+  const uint32_t* ci = in + s * C * W + w;
+  uint32_t* co = out + s * C * W + w;
+  // copy, and screen: longrun = OR over c of the AND of the m_min words ending at channel c
+  uint32_t longrun = 0;
+  for (uint32_t c = 0; c < C; ++c) {
+    const uint32_t v = ci[(uint64_t)c * W];
+    co[(uint64_t)c * W] = v;
+    if (c + 1 >= m_min) {
+      uint32_t a = v;
+      for (uint32_t k = 1; k < m_min && a; ++k) a &= ci[(uint64_t)(c - k) * W];
+      longrun |= a;
+    }
+  }
+  if (m_min > C) longrun = 0;
+  uint32_t added = 0;
+  while (longrun) {
+    const uint32_t b = (uint32_t)__ffs((int)longrun) - 1u;
+    longrun &= longrun - 1u;
+    const uint32_t bit = 1u << b;
+    for (uint32_t c = 0; c < C;) {
+      if (!(ci[(uint64_t)c * W] & bit)) { ++c; continue; }
+      uint32_t e_ = c;
+      while (e_ < C && (ci[(uint64_t)e_ * W] & bit)) ++e_;                 // run [c, e_)
+      const uint32_t ext = lof_sir_ext(eta, e_ - c);
+      const uint32_t lo = c > ext ? c - ext : 0u, hi = min(e_ + ext, C);
+      for (uint32_t q = lo; q < c; ++q) { const uint32_t o = co[(uint64_t)q * W]; if (!(o & bit)) { co[(uint64_t)q * W] = o | bit; ++added; } }
+      for (uint32_t q = e_; q < hi; ++q) { const uint32_t o = co[(uint64_t)q * W]; if (!(o & bit)) { co[(uint64_t)q * W] = o | bit; ++added; } }
+      c = e_;
+    }
+  }
+  if (added) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[s].n_flagged), (unsigned long long)added);
+}

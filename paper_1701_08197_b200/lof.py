@@ -12,6 +12,7 @@ _DIR = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("LOF_LIB_PATH") or os.path.join(_DIR, "liblof.so")   # override: kernel experiments
 
 DIR_FREQ, DIR_TIME = 1, 2
+STATS_PLAIN, STATS_MAD = 0, 1
 MAX_LEVELS = 11
 E_NULL, E_PARAM, E_ALIGN, E_STATE, E_CUDA = -1, -2, -3, -4, -5
 PATH_NONE, PATH_FUSED, PATH_LONGROW_SEG, PATH_LONGROW_COOP, PATH_GENERIC = 0, 1, 2, 3, 4
@@ -27,7 +28,7 @@ class Params(C.Structure):
                 ("p", C.c_float), ("sensitivity", C.c_float), ("start_threshold", C.c_float),
                 ("max_window", C.c_uint32), ("directions", C.c_uint32),
                 ("history_length", C.c_uint32), ("history_min_fill", C.c_uint32),
-                ("history_sensitivity", C.c_float)]
+                ("history_sensitivity", C.c_float), ("sir_eta", C.c_float), ("stats_mode", C.c_uint32)]
 
 
 STATS_DTYPE = np.dtype([("median", np.float32), ("n_nonfinite", np.uint32), ("mean", np.float64),
@@ -74,9 +75,9 @@ def _check(rc):
 
 
 def make_params(S, Cn, T, p=1.5, sensitivity=1.0, start_threshold=6.0, max_window=64, directions=3,
-                history_length=0, history_min_fill=2, history_sensitivity=0.0, device=0):
+                history_length=0, history_min_fill=2, history_sensitivity=0.0, sir_eta=0.0, stats_mode=0, device=0):
     return Params(C.sizeof(Params), device, S, Cn, T, p, sensitivity, start_threshold, max_window,
-                  directions, history_length, history_min_fill, history_sensitivity)
+                  directions, history_length, history_min_fill, history_sensitivity, sir_eta, stats_mode)
 
 
 def factor_table(n, start_threshold=6.0, p=1.5):

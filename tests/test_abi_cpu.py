@@ -33,7 +33,7 @@ def test_exports_match_header(lof):
 
 
 def test_struct_layout(lof):
-    assert C.sizeof(lof.Params) == 52
+    assert C.sizeof(lof.Params) == 60
     assert lof.STATS_DTYPE.itemsize == 32
     assert lof.STATS_DTYPE.fields["mean"][1] == 8 and lof.STATS_DTYPE.fields["n_flagged"][1] == 24
 
@@ -47,7 +47,9 @@ def test_factor_table_host(lof):
 
 @pytest.mark.parametrize("kw", [dict(S=0), dict(Cn=0), dict(T=0), dict(max_window=3), dict(max_window=2048),
                                 dict(max_window=0), dict(directions=0), dict(directions=4), dict(p=0.0),
-                                dict(sensitivity=-1.0), dict(start_threshold=float("nan")), dict(Cn=257)])
+                                dict(sensitivity=-1.0), dict(start_threshold=float("nan")), dict(Cn=257),
+                                dict(history_length=4, history_min_fill=0), dict(history_sensitivity=float("inf")),
+                                dict(sir_eta=-0.1), dict(sir_eta=1.5), dict(sir_eta=float("nan")), dict(stats_mode=2)])
 def test_bad_params_rejected_before_device(lof, kw):
     a = dict(S=1, Cn=4, T=64)
     a.update({k: v for k, v in kw.items() if k in a})

@@ -399,3 +399,54 @@ def test_path_used_reports_the_decomposition(lof):
         torch.cuda.synchronize()
         assert f.path_used() == getattr(lof, "PATH_" + want), (S, C, T, mw, f.path_used())
         f.close()
+
+
+# ---- NEXT-1: SIR operator on the packed mask
+
+@pytest.mark.parametrize("cfg,eta,dirs", [("cfg1", 0.2, 3), ("cfg2", 0.2, 3), ("cfg3", 0.2, 3), ("cfg2", 0.5, 1),
+                                          ("cfg2", 0.2, 2), ("cfg3", 1.0, 3), ("cfg1", 0.05, 3)])
+def test_sir_fused_shapes(lof, lofo, wl, cfg, eta, dirs):
+    if cfg == "cfg1":
+        w = wl.config1(0); mw = 32
+    elif cfg == "cfg2":
+        w = wl.config2(0, n_stations=6); mw = 64
+    else:
+        w = wl.config3(0, max_baselines=12); mw = 64
+    res, ora = check(lof, lofo, w.power, w.S, w.C, w.T, exact=True, max_window=mw, sir_eta=eta, directions=dirs)
+    base = run_oracle(lofo, w.power, w.S, w.C, w.T, max_window=mw, directions=dirs)
+    assert ora["stats"]["n_flagged"].sum() > base["stats"]["n_flagged"].sum()      # the operator did add flags
+
+
+@pytest.mark.parametrize("S,C,T,mw,eta", [(3, 16, 12208, 64, 0.2), (2, 32, 20011, 256, 0.2), (2, 5, 77, 8, 0.3),
+                                          (1, 64, 2100, 32, 0.2), (2, 16, 1025, 64, 0.5), (1, 1, 5000, 16, 0.2),
+                                          (2, 200, 40, 8, 0.2)])
+def test_sir_long_rows_and_ragged(lof, lofo, S, C, T, mw, eta):
+    rng = np.random.default_rng(S + C + T)
+    x = rng.standard_exponential((S, C, T)).astype(np.float32)
+    x[0, C // 2, :] += 4.0
+    for _ in range(6):                                     # bursts of many lengths: runs that cross word and lane blocks
+        d = int(rng.integers(3, max(4, min(T, 3000)))); t0 = int(rng.integers(0, max(1, T - d)))
+        c0 = int(rng.integers(0, C)); h = int(rng.integers(1, max(2, C // 2 + 1)))
+        x[rng.integers(0, S), c0:c0 + h, t0:t0 + d] += 12.0
+    x[:, :, T - 7:] += 20.0                                # a run that ends at the end of the row
+    x[S - 1, :, :9] += 20.0                                # and one that starts at its start
+    check(lof, lofo, x, S, C, T, exact=True, max_window=mw, sir_eta=eta)
+
+
+def test_sir_mask_kernels_on_random_masks(lof, lofo):
+    """The two SIR kernels alone, on dense random masks (runs of every length, merging extensions), through
+    lof_flag_block with a threshold nothing exceeds except planted samples: max_window 1, so the SumThreshold
+    mask is exactly the planted pattern."""
+    rng = np.random.default_rng(77)
+    for (S, C, T, dens) in [(2, 24, 75, 0.45), (1, 70, 333, 0.3), (3, 16, 768, 0.48), (1, 8, 9000, 0.4)]:
+        pat = rng.random((S, C, T)) < dens
+        x = np.where(pat, 1000.0, rng.random((S, C, T))).astype(np.float32)
+        # fewer than half of the samples are planted, so the median is a noise value (< 1) and, with sensitivity
+        # 0.1, median + 0.6 sigma (sigma <= 500) lies between the two populations
+        kw = dict(max_window=1, directions=3, sir_eta=0.2, sensitivity=0.1)
+        ora = run_oracle(lofo, x, S, C, T, **kw)
+        base = run_oracle(lofo, x, S, C, T, **dict(kw, sir_eta=0.0))
+        assert np.array_equal(unpack(base["flags"], T).astype(bool), pat)
+        g = run_gpu(lof, x, S, C, T, **kw)
+        assert np.array_equal(g["flags"], ora["flags"])
+        assert np.array_equal(g["stats"]["n_flagged"], ora["stats"]["n_flagged"])
