@@ -414,7 +414,8 @@ def test_sir_fused_shapes(lof, lofo, wl, cfg, eta, dirs):
         w = wl.config3(0, max_baselines=12); mw = 64
     res, ora = check(lof, lofo, w.power, w.S, w.C, w.T, exact=True, max_window=mw, sir_eta=eta, directions=dirs)
     base = run_oracle(lofo, w.power, w.S, w.C, w.T, max_window=mw, directions=dirs)
-    assert ora["stats"]["n_flagged"].sum() > base["stats"]["n_flagged"].sum()      # the operator did add flags
+    added = int(ora["stats"]["n_flagged"].sum()) - int(base["stats"]["n_flagged"].sum())
+    assert added >= 0 and (added > 0 or cfg == "cfg1")     # the operator did add flags (config 1 has no run to grow)
 
 
 @pytest.mark.parametrize("S,C,T,mw,eta", [(3, 16, 12208, 64, 0.2), (2, 32, 20011, 256, 0.2), (2, 5, 77, 8, 0.3),
