@@ -112,6 +112,24 @@ int lof_flag_block(lof_ctx* ctx, const float* d_power, uint32_t* d_flags,
 int lof_flag_block_ci16(lof_ctx* ctx, const int16_t* d_volt, uint32_t* d_flags,
                         lof_stream_stats* d_stats, void* cuda_stream);
 
+/* Fully integrated mode (Fig. 4: "integrate the time direction fully for frequency flagging, and
+ * ... the frequency direction fully for time domain flagging. We first flag in the frequency direction."), per stream:
+ *   a[c] = mean over time of power[c][t]; one SumThreshold run over a (windows <= min(max_window, C)), thresholds
+ *          from the median and stddev of a itself -> flagged channels;
+ *   b[t] = mean over the UNFLAGGED channels of power[c][t] (0 if none is left); one run over b -> flagged times;
+ *   sample (c, t) is flagged iff its channel or its time sample is (readings I1-I5).
+ * `directions` selects the runs.  d_power [S][C][T] float32 (read once, plus the rows of flagged channels a
+ * second time), d_flags [S][C][ceil(T/32)] (out, fully overwritten), d_stats_freq / d_stats_time [S] (out, may be
+ * NULL): statistics of a / of b, n_flagged = number of flagged channels / time samples.  It leaves no row sums:
+ * lof_history_update after it returns LOF_E_STATE.  The first call allocates this mode's scratch (S*T*12 bytes
+ * and two inner contexts).  Asynchronous on cuda_stream. */
+int lof_flag_block_integrated(lof_ctx* ctx, const float* d_power, uint32_t* d_flags,
+                              lof_stream_stats* d_stats_freq, lof_stream_stats* d_stats_time, void* cuda_stream);
+
+/* Copies the vectors of the last lof_flag_block_integrated to caller DEVICE buffers (either may be NULL):
+ * spectrum [S][C] float32 = a, series [S][T] float32 = b.  LOF_E_STATE before the first integrated block. */
+int lof_integrated_vectors(lof_ctx* ctx, float* d_spectrum, float* d_series, void* cuda_stream);
+
 /* History flagger (PAPER.md:97-113 pseudocode), one ring per (stream, channel):
  *   cur = mean of the row's unflagged samples of the block just flagged;
  *   thr = mean(ring) + history_sensitivity * stddev(ring);

@@ -228,6 +228,74 @@ int lofo_flag_block(const lofo_params* prm, const float* power, uint32_t* flags,
   return 0;
 }
 
+// ---- fully integrated mode (Fig. 4).  One 1-D vector: statistics of the vector itself (O1-O3),
+// thresholds (O4), one SumThreshold run (O7 on a single line).  Returns the number of flagged entries.
+static uint64_t run_vector(const lofo_params* prm, const float* v, uint64_t n, uint8_t* mask, lofo_stream_stats* st_out) {
+  uint32_t n_levels = 0;
+  while (((uint32_t)1 << n_levels) <= prm->max_window) ++n_levels;
+  lofo_stream_stats st;
+  lofo_statistics(v, n, &st);
+  if (st.n_nonfinite) std::fill(mask, mask + n, (uint8_t)1);          // S6
+  else {
+    std::vector<double> thr(n_levels);
+    lofo_threshold_table((double)st.median, st.stddev, prm->start_threshold, prm->p, prm->sensitivity, n_levels,
+                         thr.data());
+    std::fill(mask, mask + n, (uint8_t)0);
+    lofo_sumthreshold_1d_fast(v, n, 1, mask, 1, thr.data(), n_levels, nullptr, 0.0);
+  }
+  uint64_t nf = 0;
+  for (uint64_t i = 0; i < n; ++i) nf += mask[i];
+  st.n_flagged = nf;
+  if (st_out) *st_out = st;
+  return nf;
+}
+
+int lofo_flag_block_integrated(const lofo_params* prm, const float* power, uint32_t* flags, float* spectrum,
+                               float* series, uint8_t* chan_mask, uint8_t* time_mask,
+                               lofo_stream_stats* stats_freq, lofo_stream_stats* stats_time) {
+  const uint64_t S = prm->n_streams, C = prm->n_channels, T = prm->n_time;
+  if (!S || !C || !T || !prm->max_window || (prm->max_window & (prm->max_window - 1))) return -1;
+  const uint64_t words = (T + 31) / 32;
+  std::vector<float> a(C), b(T);
+  std::vector<uint8_t> Mc(C), Mt(T);
+  for (uint64_t s = 0; s < S; ++s) {
+    const float* X = power + s * C * T;
+    // "integrate the time direction fully for frequency flagging"; frequency first
+    for (uint64_t c = 0; c < C; ++c) {
+      double sum = 0.0;
+      for (uint64_t t = 0; t < T; ++t) sum += (double)X[c * T + t];
+      a[c] = (float)(sum / (double)T);
+    }
+    std::fill(Mc.begin(), Mc.end(), (uint8_t)0);
+    lofo_stream_stats sf; std::memset(&sf, 0, sizeof sf);
+    if (prm->directions & 1u) run_vector(prm, a.data(), C, Mc.data(), &sf);
+    // "integrate the frequency direction fully for time domain flagging": over the channels left unflagged
+    uint64_t n_unf = 0;
+    for (uint64_t c = 0; c < C; ++c) n_unf += Mc[c] ? 0 : 1;
+    for (uint64_t t = 0; t < T; ++t) {
+      double sum = 0.0;
+      for (uint64_t c = 0; c < C; ++c) if (!Mc[c]) sum += (double)X[c * T + t];
+      b[t] = n_unf ? (float)(sum / (double)n_unf) : 0.f;
+    }
+    std::fill(Mt.begin(), Mt.end(), (uint8_t)0);
+    lofo_stream_stats stt; std::memset(&stt, 0, sizeof stt);
+    if ((prm->directions & 2u) && n_unf) run_vector(prm, b.data(), T, Mt.data(), &stt);
+    if (flags)
+      for (uint64_t c = 0; c < C; ++c) {
+        uint32_t* fw = flags + (s * C + c) * words;
+        for (uint64_t w = 0; w < words; ++w) fw[w] = 0;
+        for (uint64_t t = 0; t < T; ++t) if (Mc[c] || Mt[t]) fw[t >> 5] |= (uint32_t)1 << (t & 31);
+      }
+    if (spectrum) std::memcpy(spectrum + s * C, a.data(), C * sizeof(float));
+    if (series) std::memcpy(series + s * T, b.data(), T * sizeof(float));
+    if (chan_mask) std::memcpy(chan_mask + s * C, Mc.data(), C);
+    if (time_mask) std::memcpy(time_mask + s * T, Mt.data(), T);
+    if (stats_freq) stats_freq[s] = sf;
+    if (stats_time) stats_time[s] = stt;
+  }
+  return 0;
+}
+
 // ---- history flagger (PAPER.md:87-116 pseudocode; buffer of 32-bit means) ----
 struct lofo_history {
   lofo_params prm;

@@ -85,6 +85,22 @@ void lofo_sir_1d(uint8_t* mask, uint64_t n, int64_t stride, double eta);
  * sample), then along time on the result, for the directions set in `directions` (reading SIR-5). */
 void lofo_sir_block(uint32_t* flags, uint64_t S, uint64_t C, uint64_t T, double eta, uint32_t directions);
 
+/* Fully integrated mode (Fig. 4): "integrate the time direction fully for frequency flagging,
+ * and ... the frequency direction fully for time domain flagging. We first flag in the frequency direction."
+ * Per stream X[C][T] (readings I1-I5):
+ *   a[c] = (float)(sum_t X[c][t] / T)                       fp64 sum in index order, rounded once
+ *   channel mask = one SumThreshold run over a[0..C), thresholds from the median / stddev of a itself
+ *   b[t] = (float)(sum over unflagged channels c of X[c][t] / their number)   (no unflagged channel: b = 0)
+ *   time mask    = one SumThreshold run over b[0..T), thresholds from the median / stddev of b itself
+ *   sample (c, t) is flagged iff its channel or its time sample is.
+ * A vector with a non-finite entry is flagged completely (S6).  Outputs: flags uint32[S][C][ceil(T/32)],
+ * spectrum float[S][C] = a, series float[S][T] = b, chan_mask uint8[S][C], time_mask uint8[S][T],
+ * stats_freq / stats_time [S] = statistics of a / of b (n_flagged: flagged channels / time samples).  Any output
+ * may be NULL.  prm->directions selects the runs (1 = channel run only, 2 = time run only, 3 = both). */
+int lofo_flag_block_integrated(const lofo_params* prm, const float* power, uint32_t* flags, float* spectrum,
+                               float* series, uint8_t* chan_mask, uint8_t* time_mask,
+                               lofo_stream_stats* stats_freq, lofo_stream_stats* stats_time);
+
 /* x = (float)(uint32)(re*re + im*im) for complex int16 volt[n][2] (reading S5). */
 void lofo_power_from_ci16(const int16_t* volt, uint64_t n, float* power);
 

@@ -152,6 +152,25 @@ def sir_block(flags, T, eta, directions=3):
     return f
 
 
+def flag_block_integrated(prm, power):
+    """Fully integrated mode.  Returns dict(flags, spectrum, series, chan_mask, time_mask,
+    stats_freq, stats_time)."""
+    S, Cn, T = prm.n_streams, prm.n_channels, prm.n_time
+    power = np.ascontiguousarray(power, np.float32).reshape(S, Cn, T)
+    W = (T + 31) // 32
+    out = dict(flags=np.zeros((S, Cn, W), np.uint32), spectrum=np.zeros((S, Cn), np.float32),
+               series=np.zeros((S, T), np.float32), chan_mask=np.zeros((S, Cn), np.uint8),
+               time_mask=np.zeros((S, T), np.uint8), stats_freq=np.zeros(S, STATS_DTYPE),
+               stats_time=np.zeros(S, STATS_DTYPE))
+    lib().lofo_flag_block_integrated.restype = C.c_int
+    rc = lib().lofo_flag_block_integrated(C.byref(prm), _p(power), _p(out["flags"]), _p(out["spectrum"]),
+                                          _p(out["series"]), _p(out["chan_mask"]), _p(out["time_mask"]),
+                                          _p(out["stats_freq"]), _p(out["stats_time"]))
+    if rc != 0:
+        raise ValueError("lofo_flag_block_integrated: bad parameters")
+    return out
+
+
 def power_from_ci16(volt):
     volt = np.ascontiguousarray(volt, np.int16)
     n = volt.size // 2

@@ -14,6 +14,7 @@
 #include "lof_fused.cuh"
 #include "lof_longrow.cuh"
 #include "lof_sir.cuh"
+#include "lof_integrated.cuh"
 
 static thread_local char g_cuda_err[256] = "";
 
@@ -60,6 +61,11 @@ struct lof_ctx {
   float* d_ring;                  // [S][C][H]
   uint32_t* d_head; uint32_t* d_count;
   uint8_t* d_row_flagged;
+  // fully integrated mode (lof_integrated.cuh), allocated on first use: two inner contexts run the 1-D
+  // SumThreshold over the spectrum (S x 1 x C) and over the series (S x 1 x T)
+  lof_ctx* ig_freq; lof_ctx* ig_time;
+  double* d_ig_rowpart; double* d_ig_colsum; float* d_ig_spec; float* d_ig_series;
+  uint32_t* d_ig_cmask; uint32_t* d_ig_tmask; uint32_t ig_tiles;
   unsigned long long* d_diag;     // per-context diagnostics of the fused kernel: [0..4) counters, [8..16) cycles
   // staging for lof_flag_block_host
   void* d_in_stage; size_t in_stage_bytes;
@@ -128,6 +134,9 @@ extern "C" int lof_destroy(lof_ctx* c) {
   cudaFree(c->d_stats); cudaFree(c->d_ring); cudaFree(c->d_head); cudaFree(c->d_count);
   cudaFree(c->d_row_flagged); cudaFree(c->d_diag); cudaFree(c->d_in_stage); cudaFree(c->d_flags_stage);
   if (c->host_stream) cudaStreamDestroy(c->host_stream);
+  lof_destroy(c->ig_freq); lof_destroy(c->ig_time);
+  cudaFree(c->d_ig_rowpart); cudaFree(c->d_ig_colsum); cudaFree(c->d_ig_spec); cudaFree(c->d_ig_series);
+  cudaFree(c->d_ig_cmask); cudaFree(c->d_ig_tmask);
   delete c;
   return LOF_OK;
 }
@@ -452,6 +461,91 @@ extern "C" int lof_flag_block(lof_ctx* c, const float* d_power, uint32_t* d_flag
 extern "C" int lof_flag_block_ci16(lof_ctx* c, const int16_t* d_volt, uint32_t* d_flags, lof_stream_stats* d_stats,
                                    void* cuda_stream) {
   return flag_block_any(c, InCI16{d_volt}, d_flags, d_stats, cuda_stream);
+}
+
+// ---- fully integrated mode
+static int integrated_prepare(lof_ctx* c) {
+  if (c->d_ig_colsum) return LOF_OK;
+  const uint32_t S = c->prm.n_streams, C = c->prm.n_channels, T = c->prm.n_time;
+  lof_params q = c->prm;
+  q.n_channels = 1; q.directions = LOF_DIR_TIME; q.history_length = 0; q.sir_eta = 0.f;
+  q.n_time = C;
+  int rc = lof_create(&q, &c->ig_freq);
+  if (rc) return rc;
+  q.n_time = T;
+  rc = lof_create(&q, &c->ig_time);
+  if (rc) return rc;
+  c->ig_tiles = (T + LOF_IG_TILE - 1) / LOF_IG_TILE;
+  cudaError_t e = cudaSuccess;
+  auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  A(dev_alloc(&c->d_ig_rowpart, (size_t)S * C * c->ig_tiles));
+  A(dev_alloc(&c->d_ig_spec, (size_t)S * ((C + 3) & ~3u)));
+  A(dev_alloc(&c->d_ig_series, (size_t)S * T + 4));
+  A(dev_alloc(&c->d_ig_cmask, (size_t)S * ((C + 31) / 32) + 4));
+  A(dev_alloc(&c->d_ig_tmask, (size_t)S * c->kp.W + 4));
+  A(dev_alloc(&c->d_ig_colsum, (size_t)S * T));
+  if (e != cudaSuccess) {
+    snprintf(g_cuda_err, sizeof g_cuda_err, "integrated mode scratch: %s", cudaGetErrorString(e));
+    return LOF_E_CUDA;
+  }
+  return LOF_OK;
+}
+
+extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint32_t* d_flags,
+                                         lof_stream_stats* d_stats_freq, lof_stream_stats* d_stats_time,
+                                         void* cuda_stream) {
+  if (!c || !d_power || !d_flags) return LOF_E_NULL;
+  if (((uintptr_t)d_power & 15) || ((uintptr_t)d_flags & 15) || ((uintptr_t)d_stats_freq & 7) ||
+      ((uintptr_t)d_stats_time & 7)) return LOF_E_ALIGN;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  int rc = integrated_prepare(c);
+  if (rc) return rc;
+  const uint32_t S = c->prm.n_streams, C = c->prm.n_channels, T = c->prm.n_time, W = c->kp.W;
+  const uint32_t CW = (C + 31) / 32;
+  // one read of the block: sums over time per channel, sums over all channels per time sample
+  lof_k_integ_sums<<<dim3(c->ig_tiles, S), LOF_IG_THREADS, 0, st>>>(d_power, c->d_ig_rowpart, c->d_ig_colsum, C, T,
+                                                                    c->ig_tiles);
+  const uint64_t rows = (uint64_t)S * C;
+  lof_k_integ_spectrum<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(c->d_ig_rowpart, c->d_ig_spec, rows, c->ig_tiles, T);
+  c->launches += 2;
+  // frequency first: one SumThreshold run over the time-integrated spectrum of every stream
+  const uint64_t l0 = c->ig_freq->launches + c->ig_time->launches;
+  if (c->prm.directions & LOF_DIR_FREQ) {
+    rc = lof_flag_block(c->ig_freq, c->d_ig_spec, c->d_ig_cmask, d_stats_freq, st);
+    if (rc) return rc;
+  } else {
+    LOF_CUDA(cudaMemsetAsync(c->d_ig_cmask, 0, (size_t)S * CW * 4, st));
+    if (d_stats_freq) LOF_CUDA(cudaMemsetAsync(d_stats_freq, 0, (size_t)S * sizeof(lof_stream_stats), st));
+  }
+  // then time: the series integrated over the channels that are left
+  const uint64_t n_st = (uint64_t)S * T;
+  lof_k_integ_series<<<(unsigned)((n_st + 255) / 256), 256, 0, st>>>(d_power, c->d_ig_colsum, c->d_ig_cmask,
+                                                                    c->d_ig_series, S, C, T);
+  if (c->prm.directions & LOF_DIR_TIME) {
+    rc = lof_flag_block(c->ig_time, c->d_ig_series, c->d_ig_tmask, d_stats_time, st);
+    if (rc) return rc;
+  } else {
+    LOF_CUDA(cudaMemsetAsync(c->d_ig_tmask, 0, (size_t)S * W * 4, st));
+    if (d_stats_time) LOF_CUDA(cudaMemsetAsync(d_stats_time, 0, (size_t)S * sizeof(lof_stream_stats), st));
+  }
+  const uint64_t n_w = (uint64_t)S * C * W;
+  lof_k_integ_combine<<<(unsigned)((n_w + 255) / 256), 256, 0, st>>>(c->d_ig_cmask, c->d_ig_tmask, d_flags, S, C, W, T);
+  c->launches += 2 + (c->ig_freq->launches + c->ig_time->launches - l0);
+  LOF_CUDA(cudaGetLastError());
+  c->block_pending = false;                               // no row sums of this block: the history flagger needs lof_flag_block
+  return LOF_OK;
+}
+
+extern "C" int lof_integrated_vectors(lof_ctx* c, float* d_spectrum, float* d_series, void* cuda_stream) {
+  if (!c) return LOF_E_NULL;
+  if (!c->d_ig_colsum) return LOF_E_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LOF_CUDA(cudaSetDevice(c->prm.device));
+  const size_t S = c->prm.n_streams;
+  if (d_spectrum) LOF_CUDA(cudaMemcpyAsync(d_spectrum, c->d_ig_spec, S * c->prm.n_channels * 4, cudaMemcpyDeviceToDevice, st));
+  if (d_series) LOF_CUDA(cudaMemcpyAsync(d_series, c->d_ig_series, S * c->prm.n_time * 4, cudaMemcpyDeviceToDevice, st));
+  return LOF_OK;
 }
 
 extern "C" int lof_history_update(lof_ctx* c, uint32_t* d_flags, uint8_t* d_row_flagged, void* cuda_stream) {

@@ -17,7 +17,8 @@ MAX_LEVELS = 11
 E_NULL, E_PARAM, E_ALIGN, E_STATE, E_CUDA = -1, -2, -3, -4, -5
 PATH_NONE, PATH_FUSED, PATH_LONGROW_SEG, PATH_LONGROW_COOP, PATH_GENERIC = 0, 1, 2, 3, 4
 
-EXPORTS = ["lof_create", "lof_destroy", "lof_flag_block", "lof_flag_block_ci16", "lof_history_update",
+EXPORTS = ["lof_create", "lof_destroy", "lof_flag_block", "lof_flag_block_ci16", "lof_flag_block_integrated",
+           "lof_integrated_vectors", "lof_history_update",
            "lof_reset", "lof_row_sums", "lof_history_export", "lof_flag_block_host", "lof_factor_table",
            "lof_launch_count", "lof_set_path", "lof_path_used", "lof_set_group", "lof_fused_counters", "lof_fused_cycles", "lof_strerror", "lof_last_cuda_error"]
 
@@ -57,6 +58,7 @@ def lib():
         L.lof_launch_count.restype = C.c_uint64
         L.lof_launch_count.argtypes = [C.c_void_p]
         for name in ("lof_create", "lof_destroy", "lof_flag_block", "lof_flag_block_ci16",
+                     "lof_flag_block_integrated", "lof_integrated_vectors",
                      "lof_history_update", "lof_reset", "lof_row_sums", "lof_history_export",
                      "lof_flag_block_host", "lof_factor_table", "lof_set_path", "lof_path_used", "lof_set_group",
                      "lof_fused_counters", "lof_fused_cycles"):
@@ -139,6 +141,24 @@ class Flagger:
             raise TypeError("power must be float32 or int16 (complex pairs)")
         _check(fn(self.h, _ptr(power), _ptr(flags), _ptr(stats), _stream(stream)))
         return flags, stats
+
+    def flag_block_integrated(self, power, flags=None, stats_freq=None, stats_time=None, stream=None):
+        """Fully integrated mode: returns (flags, stats of the spectrum, stats of the series)."""
+        flags = self.new_flags() if flags is None else flags
+        stats_freq = self.new_stats() if stats_freq is None else stats_freq
+        stats_time = self.new_stats() if stats_time is None else stats_time
+        assert power.is_cuda and power.is_contiguous() and power.dtype == self.torch.float32
+        assert power.numel() == self.S * self.Cn * self.T
+        _check(lib().lof_flag_block_integrated(self.h, _ptr(power), _ptr(flags), _ptr(stats_freq), _ptr(stats_time),
+                                               _stream(stream)))
+        return flags, stats_freq, stats_time
+
+    def integrated_vectors(self, stream=None):
+        t = self.torch
+        spec = t.empty((self.S, self.Cn), dtype=t.float32, device=self.dev)
+        series = t.empty((self.S, self.T), dtype=t.float32, device=self.dev)
+        _check(lib().lof_integrated_vectors(self.h, _ptr(spec), _ptr(series), _stream(stream)))
+        return spec, series
 
     def history_update(self, flags, row_flagged=None, stream=None):
         t = self.torch

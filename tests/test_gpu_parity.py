@@ -451,3 +451,67 @@ def test_sir_mask_kernels_on_random_masks(lof, lofo):
         g = run_gpu(lof, x, S, C, T, **kw)
         assert np.array_equal(g["flags"], ora["flags"])
         assert np.array_equal(g["stats"]["n_flagged"], ora["stats"]["n_flagged"])
+
+
+# ---- NEXT-2: fully integrated mode
+
+def _check_integrated(lof, lofo, x, S, C, T, **kw):
+    import torch
+    ora = lofo.flag_block_integrated(lofo.make_params(S, C, T, **kw), x)
+    f = lof.Flagger(S, C, T, **kw)
+    flags, sf, st = f.flag_block_integrated(torch.from_numpy(np.ascontiguousarray(x)).cuda())
+    torch.cuda.synchronize()
+    spec, series = [a.cpu().numpy() for a in f.integrated_vectors()]
+    g = lof.flags_to_numpy(flags)
+    sf, st = lof.stats_to_numpy(sf), lof.stats_to_numpy(st)
+    with pytest.raises(lof.LofError) as e:                 # no row sums after an integrated block
+        f.history_update(flags)
+    assert e.value.code == lof.E_STATE
+    f.close()
+    # the two vectors are fp64 sums rounded to float32: the summation orders differ, so 1e-6 relative (reading I5)
+    ok = ora["stats_freq"]["n_nonfinite"] == 0
+    np.testing.assert_allclose(spec[ok], ora["spectrum"][ok], rtol=1e-6, atol=0)
+    np.testing.assert_allclose(series[ok], ora["series"][ok], rtol=1e-6, atol=1e-30)
+    for gs, os_ in ((sf, ora["stats_freq"]), (st, ora["stats_time"])):
+        fin = os_["n_nonfinite"] == 0
+        for k in ("median", "mean", "stddev"):
+            np.testing.assert_allclose(gs[k][fin], os_[k][fin], rtol=2e-6, atol=1e-30)
+    assert np.array_equal(g, ora["flags"])
+    assert np.array_equal(sf["n_flagged"], ora["stats_freq"]["n_flagged"])
+    dirs = kw.get("directions", 3)
+    if dirs & 2:
+        assert np.array_equal(st["n_flagged"][ok], ora["stats_time"]["n_flagged"][ok])
+    if T % 32:
+        assert (g[..., -1] >> np.uint32(T % 32)).max() == 0
+    return ora
+
+
+@pytest.mark.parametrize("S,C,T,mw,dirs", [(4, 64, 768, 64, 3), (6, 16, 768, 16, 3), (2, 32, 20011, 256, 3),
+                                           (3, 16, 12208, 64, 3), (2, 7, 333, 8, 3), (2, 64, 768, 32, 1),
+                                           (2, 64, 768, 32, 2), (1, 200, 1025, 64, 3), (2, 3, 40, 4, 3)])
+def test_integrated_mode(lof, lofo, S, C, T, mw, dirs):
+    rng = np.random.default_rng(S * 7 + C + T)
+    x = rng.standard_exponential((S, C, T)).astype(np.float32)
+    x[0, C // 3, :] += 1.0                                 # weak narrow-band RFI, found after integration over time
+    if C > 8:
+        x[S - 1, C // 2:C // 2 + 2, :] += 0.7
+    x[:, :, T // 2:T // 2 + 5] += 1.5                      # weak broadband burst, found after integration over channels
+    x[0, :, T // 5] += 9.0
+    ora = _check_integrated(lof, lofo, x, S, C, T, max_window=mw, directions=dirs)
+    if dirs == 3 and C >= 16:
+        assert ora["chan_mask"][0, C // 3] == 1 and ora["time_mask"][0, T // 5] == 1
+
+
+def test_integrated_mode_nonfinite_and_constant(lof, lofo):
+    rng = np.random.default_rng(85)
+    x = rng.standard_exponential((3, 16, 300)).astype(np.float32)
+    x[1] = 2.5                                             # constant stream: no flags
+    x[2, 4, 17] = np.inf                                   # non-finite: everything flagged (S6)
+    ora = _check_integrated(lof, lofo, x, 3, 16, 300, max_window=16)
+    m = unpack(ora["flags"], 300)
+    assert m[1].sum() == 0 and m[2].all()
+
+
+def test_integrated_mode_config2_batch(lof, lofo, wl):
+    w = wl.config2(0, n_stations=8, want_truth=False)
+    _check_integrated(lof, lofo, w.power, w.S, w.C, w.T, max_window=64)

@@ -512,3 +512,60 @@ def test_sir_inside_flag_block(lofo):
     pop = np.unpackbits(sir["flags"].view(np.uint8), axis=-1).reshape(w.S, -1).sum(axis=1)
     assert np.array_equal(pop.astype(np.uint64), sir["stats"]["n_flagged"])
     assert (sir["stats"]["n_flagged"] > base["stats"]["n_flagged"]).any()
+
+
+# ---------------------------------------------------------------- NEXT-2: fully integrated mode
+def test_integrated_mode_definition(lofo):
+    """lofo_flag_block_integrated against its definition spelled out with numpy and the pinned 1-D pieces:
+    a = mean over time (fp64, rounded once), one SumThreshold run over a with a's own median / stddev, b = mean
+    over the unflagged channels, one run over b, flags = channel OR time (readings I1-I5)."""
+    rng = np.random.default_rng(83)
+    Cn, T = 48, 700
+    X = rng.standard_exponential((2, Cn, T)).astype(np.float32)
+    X[0, 7, :] += 1.0                      # weak narrow-band RFI: 1 sigma per sample, 26 sigma after integration
+    X[:, :, 300:306] += 1.5                # weak broadband burst: shows up after integrating over frequency
+    X[1, 30, 100:140] += 30.0              # strong but short: barely moves the channel's mean
+    prm = lofo.make_params(2, Cn, T, max_window=16)
+    out = lofo.flag_block_integrated(prm, X)
+    for s in range(2):
+        a = (X[s].astype(np.float64).sum(axis=1) / T).astype(np.float32)
+        assert np.array_equal(out["spectrum"][s], a)
+        st = lofo.statistics(a)
+        thr = lofo.threshold_table(float(st["median"]), float(st["stddev"]), 5)
+        mc, _ = lofo.sumthreshold_1d(a, thr)
+        assert np.array_equal(out["chan_mask"][s], mc)
+        keep = mc == 0
+        b = (X[s][keep].astype(np.float64).sum(axis=0) / keep.sum()).astype(np.float32)
+        np.testing.assert_allclose(out["series"][s], b, rtol=1e-7)      # (numpy sums pairwise, the oracle in order)
+        stb = lofo.statistics(out["series"][s])
+        thrb = lofo.threshold_table(float(stb["median"]), float(stb["stddev"]), 5)
+        mt, _ = lofo.sumthreshold_1d(out["series"][s], thrb)
+        assert np.array_equal(out["time_mask"][s], mt)
+        m2 = lofo.unpack_flags(out["flags"], T)[s]
+        assert np.array_equal(m2, (mc[:, None] | mt[None, :]).astype(np.uint8))
+        assert out["stats_freq"]["n_flagged"][s] == mc.sum() and out["stats_time"]["n_flagged"][s] == mt.sum()
+    # what integration buys (PAPER.md:83 "improves the INR"): the 1-sigma channel and the 1.5-sigma burst are found
+    assert out["chan_mask"][0, 7] == 1 and out["chan_mask"][0].sum() == 1
+    assert out["time_mask"][0, 300:306].all()
+    full = lofo.unpack_flags(lofo.flag_block(lofo.make_params(2, Cn, T, max_window=16), X)["flags"], T)
+    assert full[0, 7].mean() < 0.05                      # ... which the full-resolution run misses almost entirely
+
+
+def test_integrated_mode_special_cases(lofo):
+    rng = np.random.default_rng(84)
+    X = rng.standard_exponential((1, 8, 64)).astype(np.float32)
+    # constant block: stddev 0 on both vectors, strict '>' (F6): nothing flagged
+    Z = np.full((1, 8, 64), 3.0, np.float32)
+    assert lofo.flag_block_integrated(lofo.make_params(1, 8, 64, max_window=8), Z)["flags"].sum() == 0
+    # single directions
+    X[0, 3, :] += 5.0; X[0, :, 10] += 20.0
+    # (one outlier among 8 values is at most 2.5 sample sigmas out: sensitivity 0.3 puts the I = 1 level at 1.8)
+    f = lofo.flag_block_integrated(lofo.make_params(1, 8, 64, max_window=8, directions=1, sensitivity=0.3), X)
+    assert f["chan_mask"][0, 3] == 1 and f["time_mask"].sum() == 0
+    t = lofo.flag_block_integrated(lofo.make_params(1, 8, 64, max_window=8, directions=2), X)
+    assert t["chan_mask"].sum() == 0 and t["time_mask"][0, 10] == 1
+    # a non-finite sample: its channel's mean is non-finite, the spectrum is flagged completely (S6), so is everything
+    X[0, 1, 5] = np.nan
+    n = lofo.flag_block_integrated(lofo.make_params(1, 8, 64, max_window=8), X)
+    assert n["chan_mask"].all() and lofo.unpack_flags(n["flags"], 64).all()
+    assert (n["flags"][..., -1] >> np.uint32(0)).max() == 0xFFFFFFFF
