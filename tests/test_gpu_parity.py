@@ -498,7 +498,7 @@ def test_integrated_mode(lof, lofo, S, C, T, mw, dirs):
     x[:, :, T // 2:T // 2 + 5] += 1.5                      # weak broadband burst, found after integration over channels
     x[0, :, T // 5] += 9.0
     ora = _check_integrated(lof, lofo, x, S, C, T, max_window=mw, directions=dirs)
-    if dirs == 3 and C >= 16:
+    if dirs == 3 and C >= 64:                              # (one outlier among n values is at most (n-1)/sqrt(n) sigmas out)
         assert ora["chan_mask"][0, C // 3] == 1 and ora["time_mask"][0, T // 5] == 1
 
 
