@@ -49,6 +49,15 @@ void lofo_statistics(const float* x, uint64_t n, lofo_stream_stats* out) {
   out->median = v[n / 2];                            // rank floor(N/2), 0-based (S3)
 }
 
+// PAPER.md:120 "the MAD (Median Absolute Deviation)": median of |x - median|, same rank convention as the median (S3).
+float lofo_mad(const float* x, uint64_t n, float median) {
+  if (n == 0) return 0.f;
+  std::vector<float> d(n);
+  for (uint64_t i = 0; i < n; ++i) d[i] = (float)std::fabs((double)x[i] - (double)median);
+  std::nth_element(d.begin(), d.begin() + n / 2, d.end());
+  return d[n / 2];
+}
+
 static inline void mark_margin(uint8_t* margin, int64_t ms, uint64_t t0, uint64_t I, double S,
                                double lim, double rel) {
   if (!margin) return;
@@ -186,6 +195,9 @@ int lofo_flag_block(const lofo_params* prm, const float* power, uint32_t* flags,
     lofo_statistics(X, C * T, &st);                                     // O1-O3
     uint8_t* mg = margin ? margin + s * C * T : nullptr;
     if (mg) std::memset(mg, 0, C * T);
+    // robust scale (reading R1): 1.4826 * MAD takes the place of the standard deviation in threshold_I; the
+    // factor makes it an estimate of sigma for Gaussian data.  The stats record reports the scale that was used.
+    if (!st.n_nonfinite && prm->stats_mode == 1) st.stddev = 1.4826 * (double)lofo_mad(X, C * T, st.median);
     if (st.n_nonfinite) {                                               // reading S6
       std::fill(M.begin(), M.end(), (uint8_t)1);
     } else {

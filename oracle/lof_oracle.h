@@ -33,6 +33,8 @@ typedef struct {
   double   history_sensitivity; /* <= 0: use sensitivity */
   double   sir_eta;             /* SIR operator: every run of flagged samples is extended by
                                    floor(sir_eta * length) samples before and after; 0 = off; typical 0.2 */
+  uint32_t stats_mode;          /* 0: stddev as PAPER.md:41 is written; 1: 1.4826 * MAD in its place (PAPER.md:120
+                                   lists the MAD among the statistics used; reading R1) */
 } lofo_params;
 
 typedef struct {
@@ -51,6 +53,10 @@ void lofo_threshold_table(double median, double stddev, double start_threshold, 
 
 /* O1-O3: mean (index order), population stddev (two-pass), median = rank floor(N/2) element. */
 void lofo_statistics(const float* x, uint64_t n, lofo_stream_stats* out);
+
+/* Median absolute deviation: the rank floor(N/2) element of d_i = (float)|x_i - median|, the
+ * difference taken exactly and rounded once to float32 (which is what a float32 subtraction does). */
+float lofo_mad(const float* x, uint64_t n, float median);
 
 /* One SumThreshold run along one line of n samples x[i*stride]; mask[i*mask_stride] is
  * uint8 0/1, updated in place.  thresholds[k] is T_I for I = 2^k; levels k = 0..n_levels-1

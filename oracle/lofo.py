@@ -32,7 +32,7 @@ class Params(C.Structure):
                 ("p", C.c_double), ("sensitivity", C.c_double), ("start_threshold", C.c_double),
                 ("max_window", C.c_uint32), ("directions", C.c_uint32),
                 ("history_length", C.c_uint32), ("history_min_fill", C.c_uint32),
-                ("history_sensitivity", C.c_double), ("sir_eta", C.c_double)]
+                ("history_sensitivity", C.c_double), ("sir_eta", C.c_double), ("stats_mode", C.c_uint32)]
 
 
 STATS_DTYPE = np.dtype([("median", np.float32), ("n_nonfinite", np.uint32), ("mean", np.float64),
@@ -56,9 +56,9 @@ def _p(a):
 
 
 def make_params(S, Cn, T, p=1.5, sensitivity=1.0, start_threshold=6.0, max_window=64, directions=3,
-                history_length=0, history_min_fill=2, history_sensitivity=0.0, sir_eta=0.0):
+                history_length=0, history_min_fill=2, history_sensitivity=0.0, sir_eta=0.0, stats_mode=0):
     return Params(S, Cn, T, p, sensitivity, start_threshold, max_window, directions,
-                  history_length, history_min_fill, history_sensitivity, float(np.float32(sir_eta)))
+                  history_length, history_min_fill, history_sensitivity, float(np.float32(sir_eta)), stats_mode)
 
 
 def factor_table(n, start_threshold=6.0, p=1.5):
@@ -79,6 +79,12 @@ def statistics(x):
     st = np.zeros(1, STATS_DTYPE)
     lib().lofo_statistics(_p(x), C.c_uint64(x.size), _p(st))
     return st[0]
+
+
+def mad(x, median):
+    x = np.ascontiguousarray(x, np.float32).ravel()
+    lib().lofo_mad.restype = C.c_float
+    return float(lib().lofo_mad(_p(x), C.c_uint64(x.size), C.c_float(median)))
 
 
 def sumthreshold_1d(x, thresholds, mask=None, literal=False, margin_rel=MARGIN_REL):

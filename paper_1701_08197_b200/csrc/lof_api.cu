@@ -48,6 +48,8 @@ struct lof_ctx {
   size_t smem_freq, smem_time;
   // device memory owned by the context
   LofStreamState* d_state;
+  LofStreamState* d_state2;       // MAD mode: state of the selection over |x - median|
+  lof_stream_stats* d_stats2;
   uint32_t* d_hist;               // [group][4096] (the radix passes use 2048 of them)
   float* d_cand;                  // [group][LOF_LR_CAND] samples of the median's bin (lof_stats_lr.cuh)
   uint32_t* d_ctr;                // [group][2] non-finite samples, candidates gathered (lof_stats_lr.cuh)
@@ -129,7 +131,7 @@ extern "C" int lof_destroy(lof_ctx* c) {
   if (!c) return LOF_OK;
   cudaSetDevice(c->prm.device);
   cudaDeviceSynchronize();
-  cudaFree(c->d_state); cudaFree(c->d_hist); cudaFree(c->d_cand); cudaFree(c->d_ctr); cudaFree(c->d_partial); cudaFree(c->d_fmask);
+  cudaFree(c->d_state); cudaFree(c->d_state2); cudaFree(c->d_stats2); cudaFree(c->d_hist); cudaFree(c->d_cand); cudaFree(c->d_ctr); cudaFree(c->d_partial); cudaFree(c->d_fmask);
   cudaFree(c->d_part_sum); cudaFree(c->d_part_cnt); cudaFree(c->d_rowsum); cudaFree(c->d_rowcnt);
   cudaFree(c->d_stats); cudaFree(c->d_ring); cudaFree(c->d_head); cudaFree(c->d_count);
   cudaFree(c->d_row_flagged); cudaFree(c->d_diag); cudaFree(c->d_in_stage); cudaFree(c->d_flags_stage);
@@ -226,6 +228,7 @@ extern "C" int lof_create(const lof_params* p, lof_ctx** out) {
   cudaError_t e = cudaSuccess;
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   A(dev_alloc(&c->d_state, S));
+  if (p->stats_mode == LOF_STATS_MAD) { A(dev_alloc(&c->d_state2, S)); A(dev_alloc(&c->d_stats2, S)); }
   A(dev_alloc(&c->d_hist, (size_t)c->group * LOF_LR_NBINS));
   A(dev_alloc(&c->d_cand, (size_t)c->group * LOF_LR_CAND));
   A(dev_alloc(&c->d_ctr, (size_t)c->group * 2));
@@ -294,6 +297,22 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
       lof_k_hist<In, 2><<<nb, LOF_STATS_THREADS, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks);
       lof_k_scan<In, 2><<<G, 256, 0, st>>>(in, kp, c->d_state, c->d_hist, c->d_partial, c->n_chunks, c->d_stats);
       c->launches += 8;
+    }
+    if (c->prm.stats_mode == LOF_STATS_MAD) {
+      // robust scale: the rank floor(N/2) element of |x - median| by the three radix passes, then 1.4826 * MAD
+      // replaces the stddev in the thresholds (R1)
+      InAbsDev<In> dev{in, c->d_state, (uint64_t)C * c->prm.n_time, in.p};
+      lof_k_clear_state<<<(G + 255) / 256, 256, 0, st>>>(c->d_state2, s0, G);
+      lof_k_zero_u32<<<(unsigned)(((size_t)G * LOF_HIST_BINS + 255) / 256), 256, 0, st>>>(c->d_hist, (size_t)G * LOF_HIST_BINS);
+      lof_k_hist<InAbsDev<In>, 0><<<nb, LOF_STATS_THREADS, 0, st>>>(dev, kp, c->d_state2, c->d_hist, c->d_partial, c->n_chunks);
+      lof_k_scan<InAbsDev<In>, 0><<<G, 256, 0, st>>>(dev, kp, c->d_state2, c->d_hist, c->d_partial, c->n_chunks, c->d_stats2);
+      lof_k_hist<InAbsDev<In>, 1><<<nb, LOF_STATS_THREADS, 0, st>>>(dev, kp, c->d_state2, c->d_hist, c->d_partial, c->n_chunks);
+      lof_k_scan<InAbsDev<In>, 1><<<G, 256, 0, st>>>(dev, kp, c->d_state2, c->d_hist, c->d_partial, c->n_chunks, c->d_stats2);
+      lof_k_hist<InAbsDev<In>, 2><<<nb, LOF_STATS_THREADS, 0, st>>>(dev, kp, c->d_state2, c->d_hist, c->d_partial, c->n_chunks);
+      lof_k_scan<InAbsDev<In>, 2><<<G, 256, 0, st>>>(dev, kp, c->d_state2, c->d_hist, c->d_partial, c->n_chunks, c->d_stats2);
+      lof_k_mad_apply<<<(G + 255) / 256, 256, 0, st>>>(c->d_state, c->d_state2, kp, c->d_stats, s0, G);
+      c->lr_dirty = true;
+      c->launches += 9;
     }
     const bool fast = c->path == 0;                     // path 1 forces the shared-memory generic kernels
     int used = LOF_PATH_GENERIC;
@@ -441,7 +460,8 @@ static int flag_block_any(lof_ctx* c, In in, uint32_t* d_flags, lof_stream_stats
   if (((uintptr_t)in.p & 15) || ((uintptr_t)d_flags & 15) || ((uintptr_t)d_stats & 7)) return LOF_E_ALIGN;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   LOF_CUDA(cudaSetDevice(c->prm.device));
-  int rc = c->path == 0 ? flag_block_fused(c, in.p, d_flags, st) : 0;
+  // (the MAD scale needs a second selection pass: it runs on the multi-kernel paths)
+  int rc = (c->path == 0 && c->prm.stats_mode == LOF_STATS_PLAIN) ? flag_block_fused(c, in.p, d_flags, st) : 0;
   if (rc < 0) return rc;
   if (rc == 1) c->path_used = LOF_PATH_FUSED;
   if (rc == 0) { rc = flag_block_generic(c, in, d_flags, st); if (rc) return rc; }

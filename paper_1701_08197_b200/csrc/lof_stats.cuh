@@ -162,3 +162,29 @@ __global__ void lof_k_clear_state(LofStreamState* state, uint32_t s0, uint32_t n
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) { state[s0 + i].nonfinite = 0; state[s0 + i].prefix = 0; state[s0 + i].rank = 0; }
 }
+
+
+// ---- robust scale ("the MAD"; lof_params.stats_mode = LOF_STATS_MAD, R1)
+// Input adapter: d_i = |x_i - median(stream of i)| as float32 (one rounding of the exact difference, like the
+// oracle's); the radix-select kernels above then find its rank floor(N/2) element into a second state array.
+template <class In>
+struct InAbsDev {
+  In in;
+  const LofStreamState* state;   // of the primary statistics: median per stream
+  uint64_t N;                    // samples per stream
+  const void* p;                 // (unused; keeps the shape of an input adapter)
+  __device__ __forceinline__ float ld(size_t i) const { return fabsf(in.ld(i) - state[i / N].median); }
+  static constexpr int kBytes = 4;
+};
+
+// stddev := 1.4826 * MAD; thresholds and early-exit levels once more; the stats record reports the scale used.
+__global__ void lof_k_mad_apply(LofStreamState* __restrict__ state, const LofStreamState* __restrict__ dev_state,
+                                LofKParams prm, lof_stream_stats* __restrict__ stats, uint32_t s0, uint32_t n) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  LofStreamState& st = state[s0 + i];
+  if (st.nonfinite) return;
+  st.stddev = 1.4826 * (double)dev_state[s0 + i].median;
+  lof_write_thresholds(st, prm);
+  stats[s0 + i].stddev = st.stddev;
+}

@@ -515,3 +515,26 @@ def test_integrated_mode_nonfinite_and_constant(lof, lofo):
 def test_integrated_mode_config2_batch(lof, lofo, wl):
     w = wl.config2(0, n_stations=8, want_truth=False)
     _check_integrated(lof, lofo, w.power, w.S, w.C, w.T, max_window=64)
+
+
+# ---- NEXT-3: robust scale: 1.4826 * MAD in place of the standard deviation
+
+@pytest.mark.parametrize("S,C,T,mw", [(1, 16, 256, 32), (4, 64, 768, 64), (3, 16, 12208, 64), (2, 32, 9001, 256),
+                                      (2, 5, 77, 8), (8, 16, 768, 64)])
+def test_mad_mode(lof, lofo, wl, S, C, T, mw):
+    if (S, C, T) == (1, 16, 256):
+        x = wl.config1(0).power
+    elif (C, T) == (64, 768):
+        x = wl.config2(2, n_stations=2).power
+    else:
+        rng = np.random.default_rng(S + C + T)
+        x = rng.standard_exponential((S, C, T)).astype(np.float32)
+        x[0, C // 2, :] += 4.0
+        x[:, :, T // 3] += 9.0
+        x[S - 1, :, 20:36] += 2.5
+    res, ora = check(lof, lofo, x, S, C, T, max_window=mw, stats_mode=1)
+    plain = run_oracle(lofo, x, S, C, T, max_window=mw)
+    assert (ora["stats"]["stddev"] <= plain["stats"]["stddev"]).all()     # RFI inflates the stddev, hardly the MAD
+    if (S, C, T) == (1, 16, 256):
+        m = unpack(ora["flags"], T)[0].astype(bool)
+        assert m[wl.config1(0).extra["cls"][0] == 3].all()                # the 8 x 8 burst that plain stddev misses
