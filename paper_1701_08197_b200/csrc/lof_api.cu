@@ -416,8 +416,14 @@ template <int G>
 static void sir_time_launch(const uint32_t* in, uint32_t* out, lof_ctx* c, cudaStream_t st) {
   const uint64_t rows = (uint64_t)c->prm.n_streams * c->prm.n_channels;
   const uint64_t threads = rows * G;
-  lof_k_sir_time<G><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(in, out, c->d_stats, rows, c->prm.n_channels,
-                                                                      c->kp.W, c->prm.n_time, c->prm.sir_eta);
+  const unsigned grid = (unsigned)((threads + 255) / 256);
+  const size_t stage = (size_t)2 * (256 / G) * c->kp.W * 4;   // in and out copies of the CTA's rows
+  if (stage <= 40 * 1024)
+    lof_k_sir_time<G, true><<<grid, 256, stage, st>>>(in, out, c->d_stats, rows, c->prm.n_channels, c->kp.W,
+                                                      c->prm.n_time, c->prm.sir_eta);
+  else
+    lof_k_sir_time<G, false><<<grid, 256, 0, st>>>(in, out, c->d_stats, rows, c->prm.n_channels, c->kp.W,
+                                                   c->prm.n_time, c->prm.sir_eta);
 }
 
 static int sir_apply(lof_ctx* c, uint32_t* d_flags, cudaStream_t st) {
@@ -431,7 +437,11 @@ static int sir_apply(lof_ctx* c, uint32_t* d_flags, cudaStream_t st) {
     uint32_t m_min = 1;                                  // shortest run that grows at all
     while (m_min <= C && (uint32_t)std::floor((double)eta * (double)m_min) == 0) ++m_min;
     const uint64_t n_cols = (uint64_t)c->prm.n_streams * W;
-    lof_k_sir_freq<<<(unsigned)((n_cols + 255) / 256), 256, 0, st>>>(cur, other, c->d_stats, n_cols, C, W, eta, m_min);
+    const unsigned g128 = (unsigned)((n_cols + 127) / 128);
+    if (C == 64) lof_k_sir_freq_reg<64><<<g128, 128, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
+    else if (C == 32) lof_k_sir_freq_reg<32><<<g128, 128, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
+    else if (C == 16) lof_k_sir_freq_reg<16><<<g128, 128, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
+    else lof_k_sir_freq<<<(unsigned)((n_cols + 255) / 256), 256, 0, st>>>(cur, other, c->d_stats, n_cols, C, W, eta, m_min);
     c->launches += 1;
     uint32_t* t = cur; cur = other; other = t;
   }
@@ -511,6 +521,34 @@ static int integrated_prepare(lof_ctx* c) {
   return LOF_OK;
 }
 
+// One SumThreshold run over S vectors of n samples: the single-CTA kernel for short vectors, an inner context
+// (statistics kernels + row kernels of the long-row path) for long ones.
+static int integrated_run(lof_ctx* c, lof_ctx* inner, const float* d_vec, uint32_t n, uint32_t* d_mask,
+                          lof_stream_stats* d_stats_out, cudaStream_t st) {
+  const uint32_t S = c->prm.n_streams;
+  if (n <= LOF_VEC_MAX) {
+    const uint32_t Mpad = (n + 31) & ~31u;
+    uint32_t npad = 32;
+    while (npad < n) npad <<= 1;
+    const size_t smem = (size_t)Mpad * LOF_GEN_BYTES_PER_ELEM + 32 + (size_t)npad * 4;
+    LOF_CUDA(cudaFuncSetAttribute(lof_k_vec_flag, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    LofKParams kp = c->kp;
+    const uint32_t mw = c->prm.max_window < n ? c->prm.max_window : n;
+    uint32_t n_lev = 0;
+    while ((1u << n_lev) <= mw) ++n_lev;
+    lof_k_vec_flag<<<S, LOF_GEN_THREADS, smem, st>>>(d_vec, n, kp, n_lev, d_mask, inner->d_stats);
+    c->launches += 1;
+    LOF_CUDA(cudaGetLastError());
+    if (d_stats_out)
+      LOF_CUDA(cudaMemcpyAsync(d_stats_out, inner->d_stats, (size_t)S * sizeof(lof_stream_stats), cudaMemcpyDeviceToDevice, st));
+    return LOF_OK;
+  }
+  const uint64_t l0 = inner->launches;
+  const int rc = lof_flag_block(inner, d_vec, d_mask, d_stats_out, st);
+  c->launches += inner->launches - l0;
+  return rc;
+}
+
 extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint32_t* d_flags,
                                          lof_stream_stats* d_stats_freq, lof_stream_stats* d_stats_time,
                                          void* cuda_stream) {
@@ -530,9 +568,8 @@ extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint3
   lof_k_integ_spectrum<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(c->d_ig_rowpart, c->d_ig_spec, rows, c->ig_tiles, T);
   c->launches += 2;
   // frequency first: one SumThreshold run over the time-integrated spectrum of every stream
-  const uint64_t l0 = c->ig_freq->launches + c->ig_time->launches;
   if (c->prm.directions & LOF_DIR_FREQ) {
-    rc = lof_flag_block(c->ig_freq, c->d_ig_spec, c->d_ig_cmask, d_stats_freq, st);
+    rc = integrated_run(c, c->ig_freq, c->d_ig_spec, C, c->d_ig_cmask, d_stats_freq, st);
     if (rc) return rc;
   } else {
     LOF_CUDA(cudaMemsetAsync(c->d_ig_cmask, 0, (size_t)S * CW * 4, st));
@@ -543,7 +580,7 @@ extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint3
   lof_k_integ_series<<<(unsigned)((n_st + 255) / 256), 256, 0, st>>>(d_power, c->d_ig_colsum, c->d_ig_cmask,
                                                                     c->d_ig_series, S, C, T);
   if (c->prm.directions & LOF_DIR_TIME) {
-    rc = lof_flag_block(c->ig_time, c->d_ig_series, c->d_ig_tmask, d_stats_time, st);
+    rc = integrated_run(c, c->ig_time, c->d_ig_series, T, c->d_ig_tmask, d_stats_time, st);
     if (rc) return rc;
   } else {
     LOF_CUDA(cudaMemsetAsync(c->d_ig_tmask, 0, (size_t)S * W * 4, st));
@@ -551,7 +588,7 @@ extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint3
   }
   const uint64_t n_w = (uint64_t)S * C * W;
   lof_k_integ_combine<<<(unsigned)((n_w + 255) / 256), 256, 0, st>>>(c->d_ig_cmask, c->d_ig_tmask, d_flags, S, C, W, T);
-  c->launches += 2 + (c->ig_freq->launches + c->ig_time->launches - l0);
+  c->launches += 2;
   LOF_CUDA(cudaGetLastError());
   c->block_pending = false;                               // no row sums of this block: the history flagger needs lof_flag_block
   return LOF_OK;

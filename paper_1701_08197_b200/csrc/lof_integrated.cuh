@@ -11,6 +11,7 @@
 // This path is bound by HBM: 4 B read per sample plus 1/8 B written, and a few instructions per sample.
 #pragma once
 #include "lof_common.cuh"
+#include "lof_flag_generic.cuh"
 
 #define LOF_IG_THREADS 256
 #define LOF_IG_TILE (4 * LOF_IG_THREADS)      // time samples per CTA: one float4 per thread and channel
@@ -119,4 +120,88 @@ __global__ void lof_k_integ_combine(const uint32_t* __restrict__ cmask, const ui
   const bool cf = (cmask[(size_t)s * CW + (c >> 5)] >> (c & 31)) & 1u;
   const uint32_t full = (w == W - 1 && (T & 31)) ? ((1u << (T & 31)) - 1u) : 0xFFFFFFFFu;
   flags[gid] = cf ? full : tmask[(size_t)s * W + w];
+}
+
+// ---- one SumThreshold run over a short vector (n <= LOF_VEC_MAX), statistics included: one CTA per vector.
+// The integrated mode's two runs are over S vectors of C and of T samples; for the shapes of BASELINE.json's
+// configs 1-3 (C <= 64, T <= 768) the multi-kernel statistics of lof_stats_lr.cuh would be a dozen launches of
+// latency-bound work.  Here: load -> mean, stddev (two passes, fp64, fixed order: PAPER.md:41, readings S1-S3)
+// -> exact median by a bitonic sort of a copy in shared memory -> thresholds -> lof_line_levels (the generic
+// shared-memory SumThreshold of lof_flag_generic.cuh) -> packed mask + stats record.
+#define LOF_VEC_MAX 4096
+
+__global__ void __launch_bounds__(LOF_GEN_THREADS)
+lof_k_vec_flag(const float* __restrict__ vec, uint32_t n, LofKParams prm, uint32_t n_lev, uint32_t* __restrict__ mask,
+               lof_stream_stats* __restrict__ stats) {
+  extern __shared__ __align__(16) unsigned char vraw[];
+  __shared__ double red[32];
+  __shared__ float thr[LOF_MAX_LEVELS];
+  __shared__ uint32_t cnt[2];
+  const uint32_t s = blockIdx.x, tid = threadIdx.x;
+  const uint32_t Mpad = (n + 31) & ~31u;
+  uint32_t npad = 32;
+  while (npad < n) npad <<= 1;
+  LofLineSmem sm(vraw, Mpad);
+  float* ks = reinterpret_cast<float*>(vraw + (size_t)Mpad * LOF_GEN_BYTES_PER_ELEM + 16);
+  ks = reinterpret_cast<float*>(((uintptr_t)ks + 15) & ~(uintptr_t)15);
+  const float* v = vec + (size_t)s * n;
+  if (tid < 2) cnt[tid] = 0;
+  __syncthreads();
+  uint32_t bad = 0;
+  for (uint32_t i = tid; i < npad || i < Mpad; i += LOF_GEN_THREADS) {
+    const float x = i < n ? v[i] : 0.f;
+    if (i < Mpad) { sm.xs[i] = x; sm.fl[i] = 0; }
+    if (i < npad) ks[i] = i < n ? x : INFINITY;
+    if (i < n && !lof_finite(x)) ++bad;
+  }
+  if (bad) atomicAdd(&cnt[0], bad);
+  __syncthreads();
+  const uint32_t n_bad = cnt[0];
+  // mean, then population stddev about it: thread i adds elements i, i + 256, ... ; fixed tree over the CTA
+  double a = 0.0;
+  for (uint32_t i = tid; i < n; i += LOF_GEN_THREADS) a += (double)sm.xs[i];
+  a = lof_block_sum(a, red);
+  if (tid == 0) red[0] = a / (double)n;
+  __syncthreads();
+  const double mean = red[0];
+  __syncthreads();
+  double q = 0.0;
+  for (uint32_t i = tid; i < n; i += LOF_GEN_THREADS) { const double d = (double)sm.xs[i] - mean; q += d * d; }
+  q = lof_block_sum(q, red);
+  if (tid == 0) red[1] = sqrt(q / (double)n);
+  // bitonic sort of the copy (ascending; the padding is +inf): median = element of rank floor(n/2)
+  for (uint32_t k = 2; k <= npad; k <<= 1) {
+    for (uint32_t j = k >> 1; j > 0; j >>= 1) {
+      __syncthreads();
+      for (uint32_t i = tid; i < npad; i += LOF_GEN_THREADS) {
+        const uint32_t p = i ^ j;
+        if (p > i) {
+          const float x = ks[i], y = ks[p];
+          const bool up = (i & k) == 0;
+          if ((x > y) == up) { ks[i] = y; ks[p] = x; }
+        }
+      }
+    }
+  }
+  __syncthreads();
+  const float median = ks[n / 2];
+  const double stddev = red[1];
+  if (tid < n_lev) thr[tid] = (float)((double)median + stddev * prm.factor[tid] * prm.sensitivity);
+  __syncthreads();
+  if (n_bad) { for (uint32_t i = tid; i < Mpad; i += LOF_GEN_THREADS) sm.fl[i] = 1; __syncthreads(); }
+  else lof_line_levels<1>(sm, n, n_lev, thr);
+  const uint32_t W = (n + 31) / 32;
+  uint32_t nf = 0;
+  for (uint32_t i = tid; i < Mpad; i += LOF_GEN_THREADS) {
+    const bool f = i < n && sm.fl[i] != 0;
+    const uint32_t word = __ballot_sync(0xffffffffu, f);
+    if ((tid & 31) == 0) { mask[(size_t)s * W + (i >> 5)] = word; nf += __popc(word); }
+  }
+  if (nf) atomicAdd(&cnt[1], nf);
+  __syncthreads();
+  if (tid == 0) {
+    lof_stream_stats o;
+    o.median = median; o.n_nonfinite = n_bad; o.mean = mean; o.stddev = stddev; o.n_flagged = cnt[1];
+    stats[s] = o;
+  }
 }

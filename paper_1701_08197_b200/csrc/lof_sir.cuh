@@ -55,16 +55,29 @@ __device__ __forceinline__ void lof_sir_set(uint32_t* __restrict__ w, uint32_t l
 //    emits the right reach end + floor(eta n), the lane in which it really starts the left reach start - floor(..);
 //    an exclusive prefix maximum / suffix minimum over the lanes carries the reaches into the other blocks;
 // 3. per lane: out = in | own extensions | [block start, reach from the left) | [reach from the right, block end).
-template <int G>
+// STAGE: the CTA's 256/G rows are short enough to sit in shared memory (in and out copies, filled and drained
+// with coalesced accesses), so that the bit scans below run at shared-memory latency.
+template <int G, bool STAGE>
 __global__ void __launch_bounds__(256)
 lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_stream_stats* __restrict__ stats,
                uint64_t n_rows, uint32_t C, uint32_t W, uint32_t T, float eta) {
+  extern __shared__ uint32_t sir_sh[];                    // STAGE: [2][256/G][W]
   const uint64_t gid = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / G;
   const int j = threadIdx.x % G;
   const bool live = gid < n_rows;
   const uint64_t row = live ? gid : n_rows - 1;           // idle groups shadow the last row and write nothing
   const uint32_t* wi = in + row * W;
   uint32_t* wo = out + row * W;
+  constexpr int RPB = 256 / G;                            // rows per CTA
+  const uint64_t row0 = (uint64_t)blockIdx.x * RPB;
+  const uint32_t n_here = (uint32_t)min((uint64_t)RPB, n_rows > row0 ? n_rows - row0 : 0);
+  if (STAGE) {
+    for (uint32_t i = threadIdx.x; i < n_here * W; i += 256) sir_sh[i] = in[row0 * W + i];
+    __syncthreads();
+    const uint32_t lr = live ? (uint32_t)(gid - row0) : (n_here ? n_here - 1 : 0);
+    wi = sir_sh + lr * W;
+    wo = sir_sh + (RPB + lr) * W;
+  }
   const uint32_t B = (W + G - 1) / G;
   const uint32_t p0 = min((uint32_t)j * B * 32u, T), p1 = min(((uint32_t)j + 1u) * B * 32u, T), len = p1 - p0;
   const unsigned gmask = (G == 32) ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
@@ -112,7 +125,8 @@ lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_
     rin = __shfl_up_sync(gmask, r, 1, G); if (j == 0) rin = -1;
     lin = __shfl_down_sync(gmask, l, 1, G); if (j == G - 1) lin = 0x7FFFFFFF;
   }
-  if (!live) return;
+  if (!live && !STAGE) return;
+  if (live) {
   // 3. output words of the block
   const uint32_t w0 = (uint32_t)j * B, w1 = min(w0 + B, W);
   uint32_t before = 0, after = 0;
@@ -133,9 +147,81 @@ lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_
   for (uint32_t w = w0; w < w1; ++w) after += __popc(wo[w]);
   if (after != before)
     atomicAdd(reinterpret_cast<unsigned long long*>(&stats[row / C].n_flagged), (unsigned long long)(after - before));
+  }
+  if (STAGE) {
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < n_here * W; i += 256) out[row0 * W + i] = sir_sh[RPB * W + i];
+  }
 }
 
-// Frequency direction.  One thread per (stream, word column): the C words in[c][w] carry 32 time samples each.
+// Frequency direction, C = 16, 32 or 64 channels: one thread per (stream, word column) with the C words in
+// registers.  A run can only grow if it is at least m_min = ceil(1/eta) channels long: a bit-parallel screen (AND of
+// k consecutive words, k the largest power of two <= m_min, OR over c) names the time samples that may have such a
+// run; only those columns are turned into a C-bit column mask, extended with bit operations, and merged back.
+template <int C>
+__global__ void __launch_bounds__(128)
+lof_k_sir_freq_reg(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_stream_stats* __restrict__ stats,
+                   uint64_t n_cols /* S*W */, uint32_t W, float eta, uint32_t m_min) {
+  const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= n_cols) return;
+  const uint64_t s = gid / W;
+  const uint32_t w = (uint32_t)(gid - s * W);
+  const uint32_t* ci = in + s * C * W + w;
+  uint32_t* co = out + s * C * W + w;
+  uint32_t v[C];
+#pragma unroll
+  for (int c = 0; c < C; ++c) v[c] = __ldg(ci + (size_t)c * W);
+  // screen: and_k[c] = AND of v[c .. c+k); doubling up to the largest power of two <= m_min
+  uint32_t longrun = 0;
+  if (m_min <= C) {
+    uint32_t a[C];
+#pragma unroll
+    for (int c = 0; c < C; ++c) a[c] = v[c];
+    uint32_t k = 1;
+#pragma unroll
+    for (int d = 1; d < C; d <<= 1) {
+      if (2 * k <= m_min) {
+#pragma unroll
+        for (int c = 0; c < C; ++c) a[c] = (c + d < C) ? (a[c] & a[c + d]) : 0u;   // windows that leave the column: none
+        k *= 2;
+      }
+    }
+    // a[c] covers [c, c+k) with k the largest power of two <= m_min: a superset of the columns that matter
+    // (a run of k..m_min-1 channels is walked below and found not to grow)
+#pragma unroll
+    for (int c = 0; c < C; ++c) longrun |= a[c];
+    if (k > (uint32_t)C) longrun = 0;
+  }
+  uint32_t added = 0;
+  while (longrun) {
+    const uint32_t b = (uint32_t)__ffs((int)longrun) - 1u;
+    longrun &= longrun - 1u;
+    unsigned long long col = 0;
+#pragma unroll
+    for (int c = 0; c < C; ++c) col |= (unsigned long long)((v[c] >> b) & 1u) << c;
+    // runs of `col` from the low end: extend each by floor(eta * length) on both sides, lengths from the input
+    unsigned long long ext = 0, rest = col;
+    while (rest) {
+      const int a0 = __ffsll((long long)rest) - 1;
+      const unsigned long long from = rest >> a0;                         // run starts at bit 0 of `from`
+      const int len = (~from == 0ull) ? 64 - a0 : __ffsll((long long)~from) - 1;
+      const int e = (int)lof_sir_ext(eta, (uint32_t)len);
+      const int lo = max(a0 - e, 0), hi = min(a0 + len + e, C);
+      const unsigned long long span = (hi >= 64 ? ~0ull : ((1ull << hi) - 1ull)) & ~((1ull << lo) - 1ull);
+      ext |= span;
+      rest = (a0 + len >= 64) ? 0ull : (rest & ~((1ull << (a0 + len)) - 1ull));
+    }
+    const unsigned long long nw = ext & ~col;
+    added += (uint32_t)__popcll(nw);
+#pragma unroll
+    for (int c = 0; c < C; ++c) v[c] |= (uint32_t)((nw >> c) & 1ull) << b;
+  }
+#pragma unroll
+  for (int c = 0; c < C; ++c) co[(size_t)c * W] = v[c];
+  if (added) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[s].n_flagged), (unsigned long long)added);
+}
+
+// Frequency direction, any channel count.  One thread per (stream, word column): the C words in[c][w] carry 32 time samples each.
 // A run can only grow if it is at least m = ceil(1/eta) channels long: a bit-parallel screen (AND of m consecutive
 // words, OR over c) names the time samples that have such a run; only those columns are walked channel by channel.
 __global__ void __launch_bounds__(256)
