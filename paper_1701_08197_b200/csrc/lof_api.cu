@@ -526,6 +526,23 @@ static int integrated_prepare(lof_ctx* c) {
 static int integrated_run(lof_ctx* c, lof_ctx* inner, const float* d_vec, uint32_t n, uint32_t* d_mask,
                           lof_stream_stats* d_stats_out, cudaStream_t st) {
   const uint32_t S = c->prm.n_streams;
+  if (n <= 1024) {
+    // a warp per vector (lof_k_vec_warp), L = samples per lane
+    LofKParams kp = c->kp;
+    const uint32_t mw = c->prm.max_window < n ? c->prm.max_window : n;
+    uint32_t n_lev = 0;
+    while ((1u << n_lev) <= mw) ++n_lev;
+    const unsigned grid = (S + 7) / 8;
+    if (n <= 64) lof_k_vec_warp<2><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, inner->d_stats);
+    else if (n <= 256) lof_k_vec_warp<8><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, inner->d_stats);
+    else if (n <= 768) lof_k_vec_warp<24><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, inner->d_stats);
+    else lof_k_vec_warp<32><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, inner->d_stats);
+    c->launches += 1;
+    LOF_CUDA(cudaGetLastError());
+    if (d_stats_out)
+      LOF_CUDA(cudaMemcpyAsync(d_stats_out, inner->d_stats, (size_t)S * sizeof(lof_stream_stats), cudaMemcpyDeviceToDevice, st));
+    return LOF_OK;
+  }
   if (n <= LOF_VEC_MAX) {
     const uint32_t Mpad = (n + 31) & ~31u;
     uint32_t npad = 32;
@@ -576,9 +593,8 @@ extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint3
     if (d_stats_freq) LOF_CUDA(cudaMemsetAsync(d_stats_freq, 0, (size_t)S * sizeof(lof_stream_stats), st));
   }
   // then time: the series integrated over the channels that are left
-  const uint64_t n_st = (uint64_t)S * T;
-  lof_k_integ_series<<<(unsigned)((n_st + 255) / 256), 256, 0, st>>>(d_power, c->d_ig_colsum, c->d_ig_cmask,
-                                                                    c->d_ig_series, S, C, T);
+  lof_k_integ_series<<<dim3((T + 255) / 256, S), 256, 0, st>>>(d_power, c->d_ig_colsum, c->d_ig_cmask,
+                                                                c->d_ig_series, C, T);
   if (c->prm.directions & LOF_DIR_TIME) {
     rc = integrated_run(c, c->ig_time, c->d_ig_series, T, c->d_ig_tmask, d_stats_time, st);
     if (rc) return rc;
@@ -586,8 +602,7 @@ extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint3
     LOF_CUDA(cudaMemsetAsync(c->d_ig_tmask, 0, (size_t)S * W * 4, st));
     if (d_stats_time) LOF_CUDA(cudaMemsetAsync(d_stats_time, 0, (size_t)S * sizeof(lof_stream_stats), st));
   }
-  const uint64_t n_w = (uint64_t)S * C * W;
-  lof_k_integ_combine<<<(unsigned)((n_w + 255) / 256), 256, 0, st>>>(c->d_ig_cmask, c->d_ig_tmask, d_flags, S, C, W, T);
+  lof_k_integ_combine<<<dim3((C * W + 255) / 256, S), 256, 0, st>>>(c->d_ig_cmask, c->d_ig_tmask, d_flags, C, W, T);
   c->launches += 2;
   LOF_CUDA(cudaGetLastError());
   c->block_pending = false;                               // no row sums of this block: the history flagger needs lof_flag_block

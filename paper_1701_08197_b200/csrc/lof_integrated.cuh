@@ -12,6 +12,7 @@
 #pragma once
 #include "lof_common.cuh"
 #include "lof_flag_generic.cuh"
+#include "lof_core.cuh"
 
 #define LOF_IG_THREADS 256
 #define LOF_IG_TILE (4 * LOF_IG_THREADS)      // time samples per CTA: one float4 per thread and channel
@@ -84,42 +85,48 @@ __global__ void lof_k_integ_spectrum(const double* __restrict__ rowpart, float* 
 }
 
 // b[s][t]: mean over the unflagged channels.  cmask: [S][ceil(C/32)] words, bit c = channel c flagged.
-// One thread per (s, t); the rows of flagged channels are read again (coalesced over t), channels in index order.
-__global__ void lof_k_integ_series(const float* __restrict__ x, const double* __restrict__ colsum,
-                                   const uint32_t* __restrict__ cmask, float* __restrict__ series, uint32_t S,
-                                   uint32_t C, uint32_t T) {
-  const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= (uint64_t)S * T) return;
-  const uint32_t s = (uint32_t)(gid / T), t = (uint32_t)(gid - (uint64_t)s * T);
+// grid = (ceil(T/256), S), one thread per time sample; the rows of flagged channels are read again (coalesced
+// over t), channels in index order.
+__global__ void __launch_bounds__(256)
+lof_k_integ_series(const float* __restrict__ x, const double* __restrict__ colsum,
+                   const uint32_t* __restrict__ cmask, float* __restrict__ series, uint32_t C, uint32_t T) {
+  __shared__ uint32_t cm[8];                              // C <= 256
+  const uint32_t s = blockIdx.y, t = blockIdx.x * 256u + threadIdx.x;
   const uint32_t CW = (C + 31) / 32;
+  if (threadIdx.x < CW) cm[threadIdx.x] = cmask[(size_t)s * CW + threadIdx.x];
+  __syncthreads();
+  if (t >= T) return;
   const float* xs = x + (size_t)s * C * T + t;
   double fsum = 0.0;
   uint32_t nfl = 0;
   for (uint32_t w = 0; w < CW; ++w) {
-    uint32_t m = cmask[(size_t)s * CW + w];
+    uint32_t m = cm[w];
     nfl += __popc(m);
-    while (m) {
+    while (m) {                                           // (uniform over the CTA: every thread has the same mask)
       const uint32_t c = w * 32u + (uint32_t)__ffs((int)m) - 1u;
       m &= m - 1u;
       fsum += (double)__ldg(xs + (size_t)c * T);
     }
   }
   const uint32_t n_unf = C - nfl;
-  series[gid] = n_unf ? (float)((colsum[gid] - fsum) / (double)n_unf) : 0.f;
+  const size_t g = (size_t)s * T + t;
+  series[g] = n_unf ? (float)((colsum[g] - fsum) / (double)n_unf) : 0.f;
 }
 
-// flags[s][c][w] = channel c flagged ? all ones (padding bits 0) : tmask[s][w].  One thread per (s, c, w).
-__global__ void lof_k_integ_combine(const uint32_t* __restrict__ cmask, const uint32_t* __restrict__ tmask,
-                                    uint32_t* __restrict__ flags, uint32_t S, uint32_t C, uint32_t W, uint32_t T) {
-  const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= (uint64_t)S * C * W) return;
-  const uint32_t w = (uint32_t)(gid % W);
-  const uint64_t r = gid / W;
-  const uint32_t c = (uint32_t)(r % C), s = (uint32_t)(r / C);
+// flags[s][c][w] = channel c flagged ? all ones (padding bits 0) : tmask[s][w].  grid = (ceil(C*W/256), S).
+__global__ void __launch_bounds__(256)
+lof_k_integ_combine(const uint32_t* __restrict__ cmask, const uint32_t* __restrict__ tmask,
+                    uint32_t* __restrict__ flags, uint32_t C, uint32_t W, uint32_t T) {
+  __shared__ uint32_t cm[8];
+  const uint32_t s = blockIdx.y, i = blockIdx.x * 256u + threadIdx.x;
   const uint32_t CW = (C + 31) / 32;
-  const bool cf = (cmask[(size_t)s * CW + (c >> 5)] >> (c & 31)) & 1u;
+  if (threadIdx.x < CW) cm[threadIdx.x] = cmask[(size_t)s * CW + threadIdx.x];
+  __syncthreads();
+  if (i >= C * W) return;
+  const uint32_t c = i / W, w = i - c * W;
+  const bool cf = (cm[c >> 5] >> (c & 31)) & 1u;
   const uint32_t full = (w == W - 1 && (T & 31)) ? ((1u << (T & 31)) - 1u) : 0xFFFFFFFFu;
-  flags[gid] = cf ? full : tmask[(size_t)s * W + w];
+  flags[(size_t)s * C * W + i] = cf ? full : __ldg(tmask + (size_t)s * W + w);
 }
 
 // ---- one SumThreshold run over a short vector (n <= LOF_VEC_MAX), statistics included: one CTA per vector.
@@ -202,6 +209,90 @@ lof_k_vec_flag(const float* __restrict__ vec, uint32_t n, LofKParams prm, uint32
   if (tid == 0) {
     lof_stream_stats o;
     o.median = median; o.n_nonfinite = n_bad; o.mean = mean; o.stddev = stddev; o.n_flagged = cnt[1];
+    stats[s] = o;
+  }
+}
+
+// ---- the same for vectors of at most 1024 samples, one WARP per vector and no block barrier: lane l holds the
+// samples [l*L, l*L + L) (beyond n: -inf, which no window survives); mean / stddev by fp64 shuffle trees in a
+// fixed order, the exact median by a bitwise radix select on the monotone keys (32 votes), then the row core of
+// lof_core.cuh (the one the time run of the fused kernel uses), and the mask words gathered by shuffles.
+template <int L>
+__global__ void __launch_bounds__(256)
+lof_k_vec_warp(const float* __restrict__ vec, uint32_t n, uint32_t S, LofKParams prm, uint32_t n_lev,
+               uint32_t* __restrict__ mask, lof_stream_stats* __restrict__ stats) {
+  __shared__ float wthr[8][32];                           // per warp: [0..16) thresholds, [16..32) early-exit levels
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t s = blockIdx.x * 8u + (uint32_t)warp;
+  if (s >= S) return;                                     // whole warps leave together
+  const float* v = vec + (size_t)s * n;
+  const uint32_t i0 = (uint32_t)lane * L;
+  const uint32_t nv = i0 >= n ? 0u : (n - i0 >= (uint32_t)L ? (uint32_t)L : n - i0);      // valid samples of this lane
+  const uint32_t valid = nv >= 32 ? 0xFFFFFFFFu : ((1u << nv) - 1u);
+  float x[L];
+#pragma unroll
+  for (int j = 0; j < L; ++j) x[j] = (uint32_t)j < nv ? __ldg(v + i0 + j) : -INFINITY;
+  uint32_t bad = 0;
+  double a = 0.0;
+#pragma unroll
+  for (int j = 0; j < L; ++j) if ((uint32_t)j < nv) { bad += lof_finite(x[j]) ? 0u : 1u; a += (double)x[j]; }
+  const uint32_t n_bad = __reduce_add_sync(0xffffffffu, bad);
+  a = lof_warp_sum(a);
+  const double mean = __shfl_sync(0xffffffffu, a, 0) / (double)n;
+  double q = 0.0;
+#pragma unroll
+  for (int j = 0; j < L; ++j) if ((uint32_t)j < nv) { const double d = (double)x[j] - mean; q += d * d; }
+  q = lof_warp_sum(q);
+  const double stddev = sqrt(__shfl_sync(0xffffffffu, q, 0) / (double)n);
+  // exact median: the key of rank floor(n/2), one bit per vote from the top
+  uint32_t cand = valid, rank = n / 2, prefix = 0;
+#pragma unroll 1
+  for (int b = 31; b >= 0; --b) {
+    uint32_t ones = 0;
+#pragma unroll
+    for (int j = 0; j < L; ++j) ones |= ((lof_key(x[j]) >> b) & 1u) << j;
+    const uint32_t zeros = cand & ~ones;
+    const uint32_t c0 = __reduce_add_sync(0xffffffffu, (uint32_t)__popc(zeros));
+    if (rank < c0) cand = zeros;
+    else { rank -= c0; cand &= ones; prefix |= 1u << b; }
+  }
+  const float median = lof_unkey(prefix);
+  if ((uint32_t)lane < n_lev) {
+    wthr[warp][lane] = (float)((double)median + stddev * prm.factor[lane] * prm.sensitivity);
+    wthr[warp][16 + lane] = lof_dead_level((double)median, stddev, prm.factor, prm.sensitivity, lane, n_lev);
+  }
+  __syncwarp();
+  uint32_t fb = 0;
+  float lane_sum = 0.f;
+  if (n_bad) fb = valid;                                  // S6
+  else {
+    auto load = [&](float2 (&x2)[L / 2], bool) {
+#pragma unroll
+      for (int m = 0; m < L / 2; ++m) x2[m] = make_float2(x[2 * m], x[2 * m + 1]);
+    };
+    lof_row_flag<L>(load, fb, wthr[warp], wthr[warp] + 16, (int)n_lev, lane, lane_sum);
+    fb &= valid;
+  }
+  // word w of the vector = bits [32w, 32w+32) gathered from the lanes' L-bit masks
+  {
+    const uint32_t W = (n + 31) / 32;
+    const int q0 = (32 * lane) / L, r0 = 32 * lane - L * q0;
+    uint32_t word = 0;
+    constexpr int NI = (31 + L) / L + 1;
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+      const int src = q0 + i;
+      uint32_t w = __shfl_sync(0xffffffffu, fb, src & 31);
+      if (src > 31) w = 0;
+      const int sh = i * L - r0;
+      if (sh < 32) word |= sh >= 0 ? (w << sh) : (w >> (-sh));
+    }
+    if ((uint32_t)lane < W) mask[(size_t)s * W + lane] = word;
+  }
+  const uint32_t nf = __reduce_add_sync(0xffffffffu, (uint32_t)__popc(fb));
+  if (lane == 0) {
+    lof_stream_stats o;
+    o.median = median; o.n_nonfinite = n_bad; o.mean = mean; o.stddev = stddev; o.n_flagged = nf;
     stats[s] = o;
   }
 }
