@@ -115,6 +115,15 @@ __device__ __forceinline__ float lof_dead_level(double median, double stddev, co
   return tmin > 0.0 ? (float)(tmin * (1.0 - 2e-6)) : -1.0e34f;
 }
 
+// The same from the thresholds already rounded to fp32 (thr[k], each within 2^-24 relative of the fp64 value):
+// 3e-6 relative below their minimum stays under the bound above.
+__device__ __forceinline__ float lof_dead_level_f(const float* thr, uint32_t j, uint32_t n_lev) {
+  if (j + 1 >= n_lev) return 3.0e38f;
+  float tmin = thr[j + 1];
+  for (uint32_t k = j + 2; k < n_lev; ++k) tmin = fminf(tmin, thr[k]);
+  return tmin > 0.f ? tmin * (1.0f - 3e-6f) : -1.0e34f;
+}
+
 __device__ __forceinline__ float lof_max3(float a, float b, float c) {
   float d;
   asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));   // FMNMX3: one issue slot, sm_100+

@@ -163,14 +163,13 @@ __device__ __forceinline__ void lof_block_sum2(double& a, double& b, double* red
 //
 // LofStatPlan places the value histogram of one stream; every thread holds the same values.
 struct LofStatPlan {
-  float K, scale, off;     // K: centre of the shifted sums; bin(x) = round(clamp(x*scale + off)) in [0, LOF_F_NBINS)
+  float K, scale, off, s1, o1;
 };
-
-__device__ __forceinline__ uint32_t lof_stat_bin(float x, float scale, float off) {
-  float yb = fmaf(x, scale, off);
-  yb = fminf(fmaxf(yb, 0.f), (float)(LOF_F_NBINS - 1) + 0.4f);
-  return __float_as_uint(yb + LOF_F_MAGIC) & (uint32_t)(LOF_F_NBINS - 1);
+__device__ __forceinline__ uint32_t lof_stat_binoff(float x, float s1, float o1) {
+  const float y = __saturatef(fmaf(x, s1, o1));
+  return __float_as_uint(fmaf(y, 4.0f * (float)(LOF_F_NBINS - 1), LOF_F_MAGIC)) & (uint32_t)(4 * LOF_F_NBINS - 4);
 }
+__device__ __forceinline__ uint32_t lof_stat_bin(float x, const LofStatPlan& pl) { return lof_stat_binoff(x, pl.s1, pl.o1) >> 2; }
 
 // Plan from one strided sample per thread: each warp sorts its 32 samples (bitonic, shuffles) and reads off
 // their median and interquartile range; the plan centres the histogram on the mean of the warp medians with
@@ -207,6 +206,8 @@ __device__ __forceinline__ LofStatPlan lof_stat_plan(float v, float* red /* >= 2
   pl.K = K;
   pl.scale = (float)(LOF_F_NBINS - 2) / (2.0f * h);
   pl.off = fmaf(-(K - h), pl.scale, 1.0f);               // x = K-h -> 1, x = K+h -> NBINS-1
+  pl.s1 = pl.scale * (1.0f / (float)(LOF_F_NBINS - 1));
+  pl.o1 = pl.off * (1.0f / (float)(LOF_F_NBINS - 1));
   return pl;
 }
 
@@ -217,20 +218,25 @@ template <int C, int L>
 __device__ __forceinline__ void lof_stat_row(const LofFusedSmem& sm, int c, const LofStatPlan& pl, int lane) {
   constexpr int T = 32 * L;
   const float4* rp = reinterpret_cast<const float4*>(sm.xs + c * T);
-  const float K = pl.K, scale = pl.scale, off = pl.off;
+  const float s1 = pl.s1, o1 = pl.o1;
+  const float2 nK = make_float2(-pl.K, -pl.K);
+  unsigned char* hist = reinterpret_cast<unsigned char*>(sm.hist);
   double da = 0.0, dq = 0.0;
-  float ga = 0.f, gq = 0.f;
+  float2 ga = make_float2(0.f, 0.f), gq = make_float2(0.f, 0.f);   // packed: .x and .y each take 8 samples a group
 #pragma unroll
   for (int q = 0; q < L / 4; ++q) {
     const float4 v = rp[q * 32 + lane];
-    const float xv[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const float d = xv[i] - K;
-      ga += d; gq = fmaf(d, d, gq);
-      atomicAdd(&sm.hist[lof_stat_bin(xv[i], scale, off)], 1u);
+    const float2 d0 = __fadd2_rn(make_float2(v.x, v.y), nK), d1 = __fadd2_rn(make_float2(v.z, v.w), nK);
+    ga = __fadd2_rn(__fadd2_rn(ga, d0), d1);
+    gq = __ffma2_rn(d1, d1, __ffma2_rn(d0, d0, gq));
+    atomicAdd(reinterpret_cast<uint32_t*>(hist + lof_stat_binoff(v.x, s1, o1)), 1u);
+    atomicAdd(reinterpret_cast<uint32_t*>(hist + lof_stat_binoff(v.y, s1, o1)), 1u);
+    atomicAdd(reinterpret_cast<uint32_t*>(hist + lof_stat_binoff(v.z, s1, o1)), 1u);
+    atomicAdd(reinterpret_cast<uint32_t*>(hist + lof_stat_binoff(v.w, s1, o1)), 1u);
+    if ((q & 3) == 3 || q == L / 4 - 1) {
+      da += (double)ga.x + (double)ga.y; dq += (double)gq.x + (double)gq.y;
+      ga = make_float2(0.f, 0.f); gq = make_float2(0.f, 0.f);
     }
-    if ((q & 1) == 1 || q == L / 4 - 1) { da += (double)ga; dq += (double)gq; ga = 0.f; gq = 0.f; }
   }
   da = lof_warp_sum(da); dq = lof_warp_sum(dq);
   if (lane == 0) { sm.rowpart[2 * c] = da; sm.rowpart[2 * c + 1] = dq; }
@@ -300,20 +306,46 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
         }
       } else {
         const float inv = 1.0f / pl.scale;
-        const float v0 = ((float)bin - 0.5f - pl.off) * inv, v1 = ((float)bin + 0.5f - pl.off) * inv;
+        const float v0 = ((float)bin - 0.5f - pl.off) * inv, v1 = ((float)bin + 1.0f - pl.off) * inv;
         const float eps = 8e-7f * (fabsf(v0) + fabsf(v1) + fabsf(pl.off) * inv) + 8e-4f * inv;
         const float vmid = 0.5f * (v0 + v1), vhalf = 0.5f * (v1 - v0) + eps;
-        auto take = [&](float xq) {
-          if (fabsf(xq - vmid) <= vhalf && lof_stat_bin(xq, pl.scale, pl.off) == bin) {
-            const uint32_t slot = atomicAdd(&sm.ctl[CT_NCAND], 1u);
-            if (slot < LOF_F_CAP) sm.cand[slot] = xq;
+        // the four samples of a chunk near the bin: membership without branches (range and exact bin function),
+        // then one reservation in the candidate list for the chunk's members (there are a few dozen per stream)
+        auto take4 = [&](const float4& v) {
+          const float xq[4] = {v.x, v.y, v.z, v.w};
+          uint32_t mk = 0;
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+            mk |= ((uint32_t)(fabsf(xq[k] - vmid) <= vhalf) & (uint32_t)(lof_stat_bin(xq[k], pl) == bin)) << k;
+          if (mk) {
+            uint32_t slot = atomicAdd(&sm.ctl[CT_NCAND], (uint32_t)__popc(mk));
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+              if ((mk >> k) & 1u) { if (slot < LOF_F_CAP) sm.cand[slot] = xq[k]; ++slot; }
           }
         };
-#pragma unroll 4
-        for (int i = tid; i < N / 4; i += NT - 32) {
-          const float4 v = x4[i];
-          const float dmin = fminf(fminf(fabsf(v.x - vmid), fabsf(v.y - vmid)), fminf(fabsf(v.z - vmid), fabsf(v.w - vmid)));
-          if (dmin <= vhalf) { take(v.x); take(v.y); take(v.z); take(v.w); }
+        // pass 1, no branches: which of the thread's chunks have a sample within the bounds (one bit per chunk;
+        // a thread takes N/4/(NT-32) <= 32 chunks).  pass 2: the few chunks that have (about one in 250).
+        constexpr int STR = NT - 32;
+        static_assert((N / 4 + STR - 1) / STR <= 32, "one hit bit per chunk of a thread");
+        uint32_t hits = 0;
+        constexpr int NCH = (N / 4 + STR - 1) / STR;        // chunks per thread (the last one may not exist)
+#pragma unroll
+        for (int k0 = 0; k0 < NCH; k0 += 8) {               // eight 16-byte loads in flight, no branch
+          float4 v[8];
+#pragma unroll
+          for (int r = 0; r < 8; ++r) if (k0 + r < NCH) v[r] = x4[min(tid + (k0 + r) * STR, N / 4 - 1)];
+#pragma unroll
+          for (int r = 0; r < 8; ++r) if (k0 + r < NCH) {
+            const float dmin = fminf(fminf(fabsf(v[r].x - vmid), fabsf(v[r].y - vmid)),
+                                     fminf(fabsf(v[r].z - vmid), fabsf(v[r].w - vmid)));
+            hits |= ((dmin <= vhalf) & (tid + (k0 + r) * STR < N / 4) ? 1u : 0u) << (k0 + r);
+          }
+        }
+        while (hits) {
+          const int k = __ffs((int)hits) - 1;
+          hits &= hits - 1;
+          take4(x4[tid + k * STR]);
         }
       }
       dp_done = true;
@@ -325,14 +357,16 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
       if (nc != n_b) ok = false;                         // bounds too tight (cannot happen): stay exact anyway
       else if (nc <= 256) {
         how = 0;
-        for (uint32_t i = tid; i < nc; i += NT) {
+        // a warp per candidate i, its lanes over the other candidates: less = #{j : c_j < c_i, or equal and j < i}
+        for (uint32_t i = (uint32_t)(tid >> 5); i < nc; i += NT / 32) {
           const float v = sm.cand[i];
           uint32_t less = 0;
-          for (uint32_t j = 0; j < nc; ++j) {
-            const float w = sm.cand[j];
-            less += (w < v || (w == v && j < i)) ? 1u : 0u;
+          for (uint32_t j0 = 0; j0 < nc; j0 += 32) {
+            const uint32_t j = j0 + (uint32_t)lane;
+            const float w = j < nc ? sm.cand[j] : INFINITY;
+            less += __popc(__ballot_sync(0xffffffffu, j < nc && (w < v || (w == v && j < i))));
           }
-          if (less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
+          if (lane == 0 && less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
         }
         __syncthreads();
         ok = sm.ctl[CT_FOUND] != 0;
@@ -355,10 +389,12 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
       if (!(var > 0.0)) var = 0.0;
       mean = (double)pl.K + da / n; stddev = sqrt(var);
     }
-    if ((uint32_t)lane < prm.n_levels) {                 // threshold_I, one per lane
+    if ((uint32_t)lane < prm.n_levels)                   // threshold_I, one per lane
       sm.thr[lane] = (float)((double)median + stddev * prm.factor[lane] * prm.sensitivity);
-      sm.thr[16 + lane] = lof_dead_level((double)median, stddev, prm.factor, prm.sensitivity, lane, prm.n_lev_f);
-      sm.thr[32 + lane] = lof_dead_level((double)median, stddev, prm.factor, prm.sensitivity, lane, prm.n_lev_t);
+    __syncwarp();
+    if ((uint32_t)lane < prm.n_levels) {                 // early-exit levels (lof_dead_level_f), from the fp32 thresholds
+      sm.thr[16 + lane] = lof_dead_level_f(sm.thr, lane, prm.n_lev_f);
+      sm.thr[32 + lane] = lof_dead_level_f(sm.thr, lane, prm.n_lev_t);
     }
     if (lane == 0) sm.thr[48] = LOF_BELOW_MARK;            // "threshold" of a run that is switched off
     if (lane == 0) {
