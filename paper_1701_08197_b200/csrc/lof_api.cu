@@ -358,7 +358,7 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
 
 // ---- fused path: streams that fit one SM's shared memory (lof_fused.cuh)
 // Shapes with a fused instantiation, as (C, L) with T = 32 L.
-#define LOF_FUSED_SHAPES(X) X(64, 24) X(16, 24) X(32, 24) X(16, 8)
+#define LOF_FUSED_SHAPES(X) X(64, 24) X(16, 24) X(32, 24) X(16, 8) X(32, 32) X(64, 16) X(16, 32)
 
 // lof_create: opt the kernel of this shape in to its shared memory and size the persistent grid (SMs x CTAs per
 // SM) once; both are per device, so every context does it for its own device (idempotent, no shared state).
@@ -380,6 +380,7 @@ static cudaError_t fused_prepare(lof_ctx* c) {
 static cudaError_t fused_prepare_any(lof_ctx* c) {
   const uint32_t C = c->prm.n_channels, T = c->prm.n_time;
   c->fused_grid = 0;
+  if (c->kp.n_lev_t > 10) return cudaSuccess;            // the row core runs windows of up to 512 samples
 #define X(CC, LL) if (C == CC && T == 32 * LL) return fused_prepare<CC, LL>(c);
   LOF_FUSED_SHAPES(X)
 #undef X

@@ -325,10 +325,10 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
           }
         };
         // pass 1, no branches: which of the thread's chunks have a sample within the bounds (one bit per chunk;
-        // a thread takes N/4/(NT-32) <= 32 chunks).  pass 2: the few chunks that have (about one in 250).
+        // a thread takes N/4/(NT-32) <= 64 chunks).  pass 2: the few chunks that have (about one in 250).
         constexpr int STR = NT - 32;
-        static_assert((N / 4 + STR - 1) / STR <= 32, "one hit bit per chunk of a thread");
-        uint32_t hits = 0;
+        static_assert((N / 4 + STR - 1) / STR <= 64, "one hit bit per chunk of a thread");
+        unsigned long long hits = 0;
         constexpr int NCH = (N / 4 + STR - 1) / STR;        // chunks per thread (the last one may not exist)
 #pragma unroll
         for (int k0 = 0; k0 < NCH; k0 += 8) {               // eight 16-byte loads in flight, no branch
@@ -339,11 +339,11 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
           for (int r = 0; r < 8; ++r) if (k0 + r < NCH) {
             const float dmin = fminf(fminf(fabsf(v[r].x - vmid), fabsf(v[r].y - vmid)),
                                      fminf(fabsf(v[r].z - vmid), fabsf(v[r].w - vmid)));
-            hits |= ((dmin <= vhalf) & (tid + (k0 + r) * STR < N / 4) ? 1u : 0u) << (k0 + r);
+            hits |= ((dmin <= vhalf) & (tid + (k0 + r) * STR < N / 4) ? 1ull : 0ull) << (k0 + r);
           }
         }
         while (hits) {
-          const int k = __ffs((int)hits) - 1;
+          const int k = __ffsll((long long)hits) - 1;
           hits &= hits - 1;
           take4(x4[tid + k * STR]);
         }

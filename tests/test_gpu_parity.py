@@ -145,6 +145,7 @@ def test_config5_cut_with_history(lof, lofo, wl):
     (2, 16, 3000, 128, 3), (1, 32, 5003, 64, 3), (3, 64, 2100, 32, 3), (2, 16, 1025, 64, 2), (1, 32, 4096, 256, 3),
     # the fused shapes with windows beyond 64 (levels 7-9 of the row core with L = 24 and L = 8)
     (2, 64, 768, 1024, 3), (3, 16, 768, 256, 3), (2, 16, 256, 128, 3), (2, 32, 768, 512, 2), (3, 16, 768, 128, 2),
+    (3, 32, 1024, 64, 3), (3, 64, 512, 64, 3), (5, 16, 1024, 256, 3), (2, 32, 1024, 1024, 3),
     # long rows with max_window 1024 (the cooperative tiles stop at 512: generic time kernel) and 512 (cross-warp
     # exchange at distance 256)
     (1, 16, 9000, 1024, 3), (1, 32, 20011, 512, 3)])
@@ -390,7 +391,8 @@ def test_fused_nonfinite_streams_inside_persistent_loop(lof, lofo, wl, C, T, mw)
 
 def test_path_used_reports_the_decomposition(lof):
     import torch
-    for (S, C, T, mw, want) in [(2, 64, 768, 64, "FUSED"), (2, 16, 256, 32, "FUSED"), (2, 64, 704, 64, "LONGROW_SEG"), (2, 48, 768, 64, "GENERIC"),
+    for (S, C, T, mw, want) in [(2, 64, 768, 64, "FUSED"), (2, 16, 256, 32, "FUSED"), (2, 32, 1024, 64, "FUSED"),
+                                (2, 64, 512, 64, "FUSED"), (2, 16, 1024, 64, "FUSED"), (2, 64, 704, 64, "LONGROW_SEG"), (2, 48, 768, 64, "GENERIC"),
                                 (1, 16, 12208, 64, "LONGROW_SEG"), (1, 32, 20000, 256, "LONGROW_COOP"),
                                 (1, 32, 20000, 1024, "GENERIC"), (2, 5, 77, 8, "GENERIC")]:
         f = lof.Flagger(S, C, T, max_window=mw)
