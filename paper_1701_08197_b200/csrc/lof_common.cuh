@@ -69,7 +69,7 @@ struct InCI16 {
   __device__ __forceinline__ float ld(size_t i) const {
     const short2 v = __ldg(reinterpret_cast<const short2*>(p) + i);
     const int re = v.x, im = v.y;
-    return __uint2float_rn((unsigned)(re * re + im * im));
+    return __uint2float_rn((unsigned)(re * re) + (unsigned)(im * im));     // unsigned: (-32768, -32768) gives 2^31
   }
   __device__ __forceinline__ void ld4(size_t i, float (&x)[4]) const {
     const int4 v = __ldg(reinterpret_cast<const int4*>(p + 2 * i));
@@ -77,7 +77,7 @@ struct InCI16 {
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       const int re = (int)(short)(w[k] & 0xFFFF), im = w[k] >> 16;
-      x[k] = __uint2float_rn((unsigned)(re * re + im * im));
+      x[k] = __uint2float_rn((unsigned)(re * re) + (unsigned)(im * im));
     }
   }
   static constexpr int kBytes = 4;

@@ -71,6 +71,12 @@ def _station_events(rng, C, T, spike_rate=5.0, burst_rate=8.0):
     return ev
 
 
+def event_class(c0, c1, t0, t1, C, T):
+    """Injection class of a rectangle of the shared event model: 1 persistent narrow-band channel (all of time),
+    2 broadband spike (all channels), 3 burst."""
+    return 1 if (t0 == 0 and t1 == T) else (2 if (c0 == 0 and c1 == C) else 3)
+
+
 def config2(seed=0, n_subbands=1, n_stations=48, C=64, T=768, want_truth=True):
     """LOFAR-like pre-correlation block: (48 stations x 2 pol) x n_subbands streams of 64 x 768.
     g[c]*Exp(1) with g = 1 + 0.3 sin(2 pi c / C); both polarisations of a station share events."""
@@ -78,6 +84,8 @@ def config2(seed=0, n_subbands=1, n_stations=48, C=64, T=768, want_truth=True):
     g = (1.0 + 0.3 * np.sin(2 * np.pi * np.arange(C) / C)).astype(np.float32)
     x = np.empty((S, C, T), np.float32)
     truth = np.zeros((S, C, T), np.uint8) if want_truth else None
+    cls = np.zeros((S, C, T), np.uint8) if want_truth else None      # 1 narrow-band, 2 spike, 3 burst; amp: its A
+    amp = np.zeros((S, C, T), np.float32) if want_truth else None
     for b in range(n_subbands):
         for st in range(n_stations):
             ev = _station_events(_rng(seed, 2, b, st, 1), C, T)
@@ -89,8 +97,12 @@ def config2(seed=0, n_subbands=1, n_stations=48, C=64, T=768, want_truth=True):
                     xs[c0:c1, t0:t1] += np.float32(A)
                     if want_truth:
                         truth[s, c0:c1, t0:t1] = 1
+                        k = event_class(c0, c1, t0, t1, C, T)
+                        cls[s, c0:c1, t0:t1] = np.maximum(cls[s, c0:c1, t0:t1], k)
+                        amp[s, c0:c1, t0:t1] += np.float32(A)
                 x[s] = xs
-    return Workload(f"cfg2_precorr_x{n_subbands}", S, C, T, 64, power=x, truth=truth)
+    return Workload(f"cfg2_precorr_x{n_subbands}", S, C, T, 64, power=x, truth=truth,
+                    extra={"cls": cls, "amp": amp} if want_truth else {})
 
 
 def config3(seed=0, n_stations=62, C=16, T=768, max_baselines=None, want_truth=True):
@@ -103,6 +115,7 @@ def config3(seed=0, n_stations=62, C=16, T=768, max_baselines=None, want_truth=T
     events = [_station_events(_rng(seed, 3, 0, st, 1), C, T) for st in range(n_stations)]
     x = np.empty((S, C, T), np.float32)
     truth = np.zeros((S, C, T), np.uint8) if want_truth else None
+    cls = np.zeros((S, C, T), np.uint8) if want_truth else None
     for b, (i, j) in enumerate(pairs):
         for pol in range(4):
             s = b * 4 + pol
@@ -116,8 +129,9 @@ def config3(seed=0, n_stations=62, C=16, T=768, max_baselines=None, want_truth=T
                     im[c0:c1, t0:t1] += np.float32(math.sqrt(A) * math.sin(phi))
                     if want_truth:
                         truth[s, c0:c1, t0:t1] = 1
+                        cls[s, c0:c1, t0:t1] = np.maximum(cls[s, c0:c1, t0:t1], event_class(c0, c1, t0, t1, C, T))
             x[s] = re * re + im * im
-    return Workload("cfg3_visibility", S, C, T, 64, power=x, truth=truth)
+    return Workload("cfg3_visibility", S, C, T, 64, power=x, truth=truth, extra={"cls": cls} if want_truth else {})
 
 
 # ----------------------------------------------------------------------------- config 4
@@ -130,6 +144,7 @@ def config4(seed=0, n_stations=48, C=32, T=195312, want_truth=False):
     sec = T / 195312.0
     v = np.empty((S, C, T, 2), np.int16)
     truth = np.zeros((S, C, T), np.uint8) if want_truth else None
+    cls = np.zeros((S, C, T), np.uint8) if want_truth else None       # 2 spike (all subbands), 3 burst
     for st in range(n_stations):
         r = _rng(seed, 4, 0, st, 1)
         ev = []
@@ -149,10 +164,11 @@ def config4(seed=0, n_stations=48, C=32, T=195312, want_truth=False):
                 f[c0:c1, t0:t1, 1] += np.float32(A * math.sin(phi))
                 if want_truth:
                     truth[s, c0:c1, t0:t1] = 1
+                    cls[s, c0:c1, t0:t1] = np.maximum(cls[s, c0:c1, t0:t1], 2 if (c0 == 0 and c1 == C) else 3)
             np.rint(f, out=f)
             np.clip(f, -32768, 32767, out=f)
             v[s] = f.astype(np.int16)
-    return Workload("cfg4_rawvoltage", S, C, T, 256, volt=v, truth=truth)
+    return Workload("cfg4_rawvoltage", S, C, T, 256, volt=v, truth=truth, extra={"cls": cls} if want_truth else {})
 
 
 # ----------------------------------------------------------------------------- config 5
