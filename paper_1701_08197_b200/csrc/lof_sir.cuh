@@ -55,32 +55,15 @@ __device__ __forceinline__ void lof_sir_set(uint32_t* __restrict__ w, uint32_t l
 //    emits the right reach end + floor(eta n), the lane in which it really starts the left reach start - floor(..);
 //    an exclusive prefix maximum / suffix minimum over the lanes carries the reaches into the other blocks;
 // 3. per lane: out = in | own extensions | [block start, reach from the left) | [reach from the right, block end).
-// STAGE: the CTA's 256/G rows are short enough to sit in shared memory (in and out copies, filled and drained
-// with coalesced accesses), so that the bit scans below run at shared-memory latency.
-template <int G, bool STAGE>
-__global__ void __launch_bounds__(256)
-lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_stream_stats* __restrict__ stats,
-               uint64_t n_rows, uint32_t C, uint32_t W, uint32_t T, float eta) {
-  extern __shared__ uint32_t sir_sh[];                    // STAGE: [2][256/G][W]
-  const uint64_t gid = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / G;
-  const int j = threadIdx.x % G;
-  const bool live = gid < n_rows;
-  const uint64_t row = live ? gid : n_rows - 1;           // idle groups shadow the last row and write nothing
-  const uint32_t* wi = in + row * W;
-  uint32_t* wo = out + row * W;
-  constexpr int RPB = 256 / G;                            // rows per CTA
-  const uint64_t row0 = (uint64_t)blockIdx.x * RPB;
-  const uint32_t n_here = (uint32_t)min((uint64_t)RPB, n_rows > row0 ? n_rows - row0 : 0);
-  if (STAGE) {
-    for (uint32_t i = threadIdx.x; i < n_here * W; i += 256) sir_sh[i] = in[row0 * W + i];
-    __syncthreads();
-    const uint32_t lr = live ? (uint32_t)(gid - row0) : (n_here ? n_here - 1 : 0);
-    wi = sir_sh + lr * W;
-    wo = sir_sh + (RPB + lr) * W;
-  }
+// The row operator for one row: lane j of a group of G lanes (gmask = the group's lanes within the warp) owns the
+// words [j*B, j*B+B) of the row wi[0..W) (B = ceil(W/G)); the output words go to wo (a different buffer).  Every
+// lane of the group must call it; `live` = false makes the group compute and write nothing.  Returns the number
+// of bits this lane's words gained.
+template <int G>
+__device__ __forceinline__ uint32_t lof_sir_time_row(const uint32_t* wi, uint32_t* wo, int j, unsigned gmask,
+                                                     uint32_t W, uint32_t T, float eta, bool live) {
   const uint32_t B = (W + G - 1) / G;
   const uint32_t p0 = min((uint32_t)j * B * 32u, T), p1 = min(((uint32_t)j + 1u) * B * 32u, T), len = p1 - p0;
-  const unsigned gmask = (G == 32) ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
   // 1. block summary and the carries
   const uint32_t lead = lof_sir_next(wi, p0, p1, false) - p0;
   const bool all = lead == len;
@@ -125,8 +108,7 @@ lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_
     rin = __shfl_up_sync(gmask, r, 1, G); if (j == 0) rin = -1;
     lin = __shfl_down_sync(gmask, l, 1, G); if (j == G - 1) lin = 0x7FFFFFFF;
   }
-  if (!live && !STAGE) return;
-  if (live) {
+  if (!live) return 0;
   // 3. output words of the block
   const uint32_t w0 = (uint32_t)j * B, w1 = min(w0 + B, W);
   uint32_t before = 0, after = 0;
@@ -145,13 +127,56 @@ lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_
   if (rin > (int)p0) lof_sir_set(wo, p0, min((uint32_t)rin, p1));
   if (lin < (int)p1) lof_sir_set(wo, max((uint32_t)max(lin, 0), p0), p1);
   for (uint32_t w = w0; w < w1; ++w) after += __popc(wo[w]);
-  if (after != before)
-    atomicAdd(reinterpret_cast<unsigned long long*>(&stats[row / C].n_flagged), (unsigned long long)(after - before));
+  return after - before;
+}
+
+// STAGE: the CTA's 256/G rows are short enough to sit in shared memory (in and out copies, filled and drained
+// with coalesced accesses), so that the bit scans run at shared-memory latency.
+template <int G, bool STAGE>
+__global__ void __launch_bounds__(256)
+lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_stream_stats* __restrict__ stats,
+               uint64_t n_rows, uint32_t C, uint32_t W, uint32_t T, float eta) {
+  extern __shared__ uint32_t sir_sh[];                    // STAGE: [2][256/G][W]
+  const uint64_t gid = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / G;
+  const int j = threadIdx.x % G;
+  const bool live = gid < n_rows;
+  const uint64_t row = live ? gid : n_rows - 1;           // idle groups shadow the last row and write nothing
+  const uint32_t* wi = in + row * W;
+  uint32_t* wo = out + row * W;
+  constexpr int RPB = 256 / G;                            // rows per CTA
+  const uint64_t row0 = (uint64_t)blockIdx.x * RPB;
+  const uint32_t n_here = (uint32_t)min((uint64_t)RPB, n_rows > row0 ? n_rows - row0 : 0);
+  if (STAGE) {
+    for (uint32_t i = threadIdx.x; i < n_here * W; i += 256) sir_sh[i] = in[row0 * W + i];
+    __syncthreads();
+    const uint32_t lr = live ? (uint32_t)(gid - row0) : (n_here ? n_here - 1 : 0);
+    wi = sir_sh + lr * W;
+    wo = sir_sh + (RPB + lr) * W;
   }
+  const unsigned gmask = (G == 32) ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
+  const uint32_t added = lof_sir_time_row<G>(wi, wo, j, gmask, W, T, eta, live);
+  if (added) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[row / C].n_flagged), (unsigned long long)added);
   if (STAGE) {
     __syncthreads();
     for (uint32_t i = threadIdx.x; i < n_here * W; i += 256) out[row0 * W + i] = sir_sh[RPB * W + i];
   }
+}
+
+// The frequency operator on one word column held as a C-bit mask per lane (lane = time sample of the word):
+// returns the bits to add (runs of the input mask, each grown by floor(eta * length) on both sides, clipped).
+template <int C>
+__device__ __forceinline__ unsigned long long lof_sir_col_ext(unsigned long long col, float eta) {
+  unsigned long long ext = 0, rest = col;
+  while (rest) {
+    const int a0 = __ffsll((long long)rest) - 1;
+    const unsigned long long from = rest >> a0;                           // the run starts at bit 0 of `from`
+    const int len = (~from == 0ull) ? 64 - a0 : __ffsll((long long)~from) - 1;
+    const int e = (int)lof_sir_ext(eta, (uint32_t)len);
+    const int lo = max(a0 - e, 0), hi = min(a0 + len + e, C);
+    ext |= (hi >= 64 ? ~0ull : ((1ull << hi) - 1ull)) & ~((1ull << lo) - 1ull);
+    rest = (a0 + len >= 64) ? 0ull : (rest & ~((1ull << (a0 + len)) - 1ull));
+  }
+  return ext & ~col;
 }
 
 // Frequency direction, C = 16, 32 or 64 channels: one thread per (stream, word column) with the C words in
@@ -199,19 +224,7 @@ lof_k_sir_freq_reg(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, 
     unsigned long long col = 0;
 #pragma unroll
     for (int c = 0; c < C; ++c) col |= (unsigned long long)((v[c] >> b) & 1u) << c;
-    // runs of `col` from the low end: extend each by floor(eta * length) on both sides, lengths from the input
-    unsigned long long ext = 0, rest = col;
-    while (rest) {
-      const int a0 = __ffsll((long long)rest) - 1;
-      const unsigned long long from = rest >> a0;                         // run starts at bit 0 of `from`
-      const int len = (~from == 0ull) ? 64 - a0 : __ffsll((long long)~from) - 1;
-      const int e = (int)lof_sir_ext(eta, (uint32_t)len);
-      const int lo = max(a0 - e, 0), hi = min(a0 + len + e, C);
-      const unsigned long long span = (hi >= 64 ? ~0ull : ((1ull << hi) - 1ull)) & ~((1ull << lo) - 1ull);
-      ext |= span;
-      rest = (a0 + len >= 64) ? 0ull : (rest & ~((1ull << (a0 + len)) - 1ull));
-    }
-    const unsigned long long nw = ext & ~col;
+    const unsigned long long nw = lof_sir_col_ext<C>(col, eta);
     added += (uint32_t)__popcll(nw);
 #pragma unroll
     for (int c = 0; c < C; ++c) v[c] |= (uint32_t)((nw >> c) & 1ull) << b;
