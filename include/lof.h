@@ -176,7 +176,7 @@ int lof_set_path(lof_ctx* ctx, int path);
 /* Which kernels the last lof_flag_block[_ci16] of this context ran (the steps of PAPER.md:37-47, :83 are the
  * same on every path; only the decomposition differs):
  *   LOF_PATH_FUSED         one kernel per block: (n_channels, n_time) in {(64,768), (32,768), (16,768), (16,256),
- *                          (32,1024), (64,512), (16,1024)}, float32 input, stats_mode PLAIN — a stream fits one
+ *                          (32,1024), (64,512), (16,1024)}, max_window <= 64, float32 input, stats_mode PLAIN — a stream fits one
  *                          SM's shared memory (n_time is a template parameter of that kernel: 32 x the samples a
  *                          lane holds; other shapes take the paths below, with the same results);
  *   LOF_PATH_LONGROW_SEG   statistics kernels + register-resident column kernel + independent row segments

@@ -380,7 +380,7 @@ static cudaError_t fused_prepare(lof_ctx* c) {
 static cudaError_t fused_prepare_any(lof_ctx* c) {
   const uint32_t C = c->prm.n_channels, T = c->prm.n_time;
   c->fused_grid = 0;
-  if (c->kp.n_lev_t > 10) return cudaSuccess;            // the row core runs windows of up to 512 samples
+  if (c->kp.n_lev_t > LOF_FUSED_KMAX + 1) return cudaSuccess;   // the fused kernel compiles windows of up to 64 samples in
 #define X(CC, LL) if (C == CC && T == 32 * LL) return fused_prepare<CC, LL>(c);
   LOF_FUSED_SHAPES(X)
 #undef X
@@ -527,7 +527,7 @@ static int integrated_prepare(lof_ctx* c) {
 static int integrated_run(lof_ctx* c, lof_ctx* inner, const float* d_vec, uint32_t n, uint32_t* d_mask,
                           lof_stream_stats* d_stats_out, cudaStream_t st) {
   const uint32_t S = c->prm.n_streams;
-  if (n <= 1024) {
+  if (n <= 1024 && (c->prm.max_window < 1024 || n < 1024)) {     // (the row core runs windows of up to 512 samples)
     // a warp per vector (lof_k_vec_warp), L = samples per lane
     LofKParams kp = c->kp;
     const uint32_t mw = c->prm.max_window < n ? c->prm.max_window : n;

@@ -431,9 +431,11 @@ __device__ __forceinline__ float lof_lane_sum(const float2 (&u2)[NP]) {
 // anywhere: every flag so far is in fb and is re-applied).  The samples are not kept in registers across the
 // levels.  fb leaves as the line's final mask (bit j = sample l*L + j); lane_sum as the sum of the lane's
 // unflagged samples under that mask.  Warp-uniform control flow.
-template <int L, class Load>
+// KMAX: the largest iteration compiled in (windows up to 2^KMAX <= 512); the caller guarantees nlt <= KMAX + 1.
+template <int L, int KMAX, class Load>
 __device__ __forceinline__ void lof_row_flag(Load load, uint32_t& fb, const float* thr, const float* dead, int nlt,
                                              int lane, float& lane_sum) {
+  static_assert(KMAX >= 1 && KMAX <= 9, "row core: windows of 2 .. 512 samples");
   constexpr int NP = L / 2;
   const uint32_t maskL = (L == 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
   float2 u2[NP], e2[NP];
@@ -456,11 +458,11 @@ __device__ __forceinline__ void lof_row_flag(Load load, uint32_t& fb, const floa
     // one test per level on the way down: past the last level -> done; new flags with levels to go ->
     // back to level 0 under the new mask (continue), re-doubling up to k_next without testing
 #define LOF_ROW_LEVEL(K)                                                                 \
-    if (K >= nlt) break;                                                                 \
-    lof_row_step<L, (1 << (K - 1))>(u2, e2, lane);                                       \
+    if (K > KMAX || K >= nlt) break;                                                     \
+    lof_row_step<L, (1 << ((K <= KMAX ? K : 1) - 1))>(u2, e2, lane);                     \
     if (K >= k_next) {                                                                   \
       bool dead_;                                                                        \
-      if (lof_row_eval<L, K>(u2, e2, lane, thr[K], dead[K], fb, dead_)) {                \
+      if (lof_row_eval<L, (K <= KMAX ? K : 1)>(u2, e2, lane, thr[K], dead[K], fb, dead_)) { \
         k_next = K + 1 < nlt ? K + 1 : 99;                /* 99: level 0 once more, for the row sum */ \
         LOF_PROF_CNT(7);                                                                  \
         continue;                                                                        \

@@ -23,6 +23,11 @@
 #include "lof_common.cuh"
 #include "lof_core.cuh"
 
+// iterations of the time run compiled into the fused kernel: windows up to 2^6 = 64 ("7 iterations", the low end of
+// PAPER.md:45's 7-10; BASELINE's configs 1-3 use 32 and 64).  Larger windows on these shapes take the row kernels of
+// lof_longrow.cuh: the unrolled levels 7-9 alone were a third of the kernel's code, and two CTAs per SM in different
+// phases already miss the instruction cache (no_instruction stalls: 11 % on config 3).
+#define LOF_FUSED_KMAX 6
 #define LOF_F_NBINS 4096
 #define LOF_F_CAP 1024
 #define LOF_F_MAGIC 12582912.0f   // 1.5 * 2^23: adding it leaves round-to-nearest(x) in the low mantissa bits
@@ -542,7 +547,7 @@ __device__ void lof_fused_time(const LofFusedSmem& sm, const LofKParams& prm, ui
     // turns them into the mask and sums the rest.
     uint32_t fb = 0;
     float lane_sum = 0.f;
-    lof_row_flag<L>(load, fb, nlt > 0 ? sm.thr : sm.thr + 48, sm.thr + 32, nlt > 0 ? (int)nlt : 1, lane, lane_sum);
+    lof_row_flag<L, LOF_FUSED_KMAX>(load, fb, nlt > 0 ? sm.thr : sm.thr + 48, sm.thr + 32, nlt > 0 ? (int)nlt : 1, lane, lane_sum);
     // bit-pack: word w of the row = bits [32w, 32w+32) gathered from the lanes' L-bit masks
     {
       const int q0 = (32 * lane) / L, r0 = 32 * lane - L * q0;

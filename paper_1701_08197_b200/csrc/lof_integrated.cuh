@@ -270,7 +270,7 @@ lof_k_vec_warp(const float* __restrict__ vec, uint32_t n, uint32_t S, LofKParams
 #pragma unroll
       for (int m = 0; m < L / 2; ++m) x2[m] = make_float2(x[2 * m], x[2 * m + 1]);
     };
-    lof_row_flag<L>(load, fb, wthr[warp], wthr[warp] + 16, (int)n_lev, lane, lane_sum);
+    lof_row_flag<L, 9>(load, fb, wthr[warp], wthr[warp] + 16, (int)n_lev, lane, lane_sum);
     fb &= valid;
   }
   // word w of the vector = bits [32w, 32w+32) gathered from the lanes' L-bit masks

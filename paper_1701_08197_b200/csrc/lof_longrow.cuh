@@ -111,7 +111,7 @@ lof_k_time_seg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
   bool have_sum = false;
   if (st.nonfinite) fb = valid;                           // DESIGN.md S6: the whole stream is flagged
   else if (prm.n_lev_t > 0) {
-    lof_row_flag<32>(load, fb, st.thr_f, st.dead_t, (int)prm.n_lev_t, lane, lane_sum);
+    lof_row_flag<32, 7>(load, fb, st.thr_f, st.dead_t, (int)prm.n_lev_t, lane, lane_sum);
     have_sum = true;
   }
   fb &= valid;
