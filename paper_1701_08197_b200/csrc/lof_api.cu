@@ -594,7 +594,7 @@ extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint3
     if (d_stats_freq) LOF_CUDA(cudaMemsetAsync(d_stats_freq, 0, (size_t)S * sizeof(lof_stream_stats), st));
   }
   // then time: the series integrated over the channels that are left
-  lof_k_integ_series<<<dim3((T + 255) / 256, S), 256, 0, st>>>(d_power, c->d_ig_colsum, c->d_ig_cmask,
+  lof_k_integ_series<<<dim3((T + 256 * LOF_IG_SER - 1) / (256 * LOF_IG_SER), S), 256, 0, st>>>(d_power, c->d_ig_colsum, c->d_ig_cmask,
                                                                 c->d_ig_series, C, T);
   if (c->prm.directions & LOF_DIR_TIME) {
     rc = integrated_run(c, c->ig_time, c->d_ig_series, T, c->d_ig_tmask, d_stats_time, st);
@@ -603,7 +603,7 @@ extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint3
     LOF_CUDA(cudaMemsetAsync(c->d_ig_tmask, 0, (size_t)S * W * 4, st));
     if (d_stats_time) LOF_CUDA(cudaMemsetAsync(d_stats_time, 0, (size_t)S * sizeof(lof_stream_stats), st));
   }
-  lof_k_integ_combine<<<dim3((C * W + 255) / 256, S), 256, 0, st>>>(c->d_ig_cmask, c->d_ig_tmask, d_flags, C, W, T);
+  lof_k_integ_combine<<<S, 256, 0, st>>>(c->d_ig_cmask, c->d_ig_tmask, d_flags, C, W, T);
   c->launches += 2;
   LOF_CUDA(cudaGetLastError());
   c->block_pending = false;                               // no row sums of this block: the history flagger needs lof_flag_block

@@ -85,48 +85,71 @@ __global__ void lof_k_integ_spectrum(const double* __restrict__ rowpart, float* 
 }
 
 // b[s][t]: mean over the unflagged channels.  cmask: [S][ceil(C/32)] words, bit c = channel c flagged.
-// grid = (ceil(T/256), S), one thread per time sample; the rows of flagged channels are read again (coalesced
-// over t), channels in index order.
+// grid = (ceil(T / (256 * LOF_IG_SER)), S): a thread takes LOF_IG_SER time samples 256 apart; the rows of flagged
+// channels are read again (coalesced over t), channels in index order.
+#define LOF_IG_SER 4
 __global__ void __launch_bounds__(256)
 lof_k_integ_series(const float* __restrict__ x, const double* __restrict__ colsum,
                    const uint32_t* __restrict__ cmask, float* __restrict__ series, uint32_t C, uint32_t T) {
   __shared__ uint32_t cm[8];                              // C <= 256
-  const uint32_t s = blockIdx.y, t = blockIdx.x * 256u + threadIdx.x;
+  const uint32_t s = blockIdx.y;
   const uint32_t CW = (C + 31) / 32;
   if (threadIdx.x < CW) cm[threadIdx.x] = cmask[(size_t)s * CW + threadIdx.x];
   __syncthreads();
-  if (t >= T) return;
-  const float* xs = x + (size_t)s * C * T + t;
-  double fsum = 0.0;
   uint32_t nfl = 0;
+  for (uint32_t w = 0; w < CW; ++w) nfl += __popc(cm[w]);
+  const uint32_t n_unf = C - nfl;
+  const double inv = n_unf ? 1.0 / (double)n_unf : 0.0;
+  (void)inv;
+  const uint32_t t0 = blockIdx.x * (256u * LOF_IG_SER) + threadIdx.x;
+  const float* xs = x + (size_t)s * C * T;
+  double fsum[LOF_IG_SER];
+#pragma unroll
+  for (int k = 0; k < LOF_IG_SER; ++k) fsum[k] = 0.0;
   for (uint32_t w = 0; w < CW; ++w) {
     uint32_t m = cm[w];
-    nfl += __popc(m);
     while (m) {                                           // (uniform over the CTA: every thread has the same mask)
       const uint32_t c = w * 32u + (uint32_t)__ffs((int)m) - 1u;
       m &= m - 1u;
-      fsum += (double)__ldg(xs + (size_t)c * T);
+#pragma unroll
+      for (int k = 0; k < LOF_IG_SER; ++k) {
+        const uint32_t t = t0 + 256u * k;
+        if (t < T) fsum[k] += (double)__ldg(xs + (size_t)c * T + t);
+      }
     }
   }
-  const uint32_t n_unf = C - nfl;
-  const size_t g = (size_t)s * T + t;
-  series[g] = n_unf ? (float)((colsum[g] - fsum) / (double)n_unf) : 0.f;
+#pragma unroll
+  for (int k = 0; k < LOF_IG_SER; ++k) {
+    const uint32_t t = t0 + 256u * k;
+    if (t < T) {
+      const size_t g = (size_t)s * T + t;
+      series[g] = n_unf ? (float)((colsum[g] - fsum[k]) / (double)n_unf) : 0.f;
+    }
+  }
 }
 
-// flags[s][c][w] = channel c flagged ? all ones (padding bits 0) : tmask[s][w].  grid = (ceil(C*W/256), S).
+// flags[s][c][w] = channel c flagged ? all ones (padding bits 0) : tmask[s][w].  One CTA per stream: the time
+// mask's W words sit in shared memory (W <= LOF_IG_TM words, else they are read from global memory).
+#define LOF_IG_TM 1024
 __global__ void __launch_bounds__(256)
 lof_k_integ_combine(const uint32_t* __restrict__ cmask, const uint32_t* __restrict__ tmask,
                     uint32_t* __restrict__ flags, uint32_t C, uint32_t W, uint32_t T) {
   __shared__ uint32_t cm[8];
-  const uint32_t s = blockIdx.y, i = blockIdx.x * 256u + threadIdx.x;
+  __shared__ uint32_t tm[LOF_IG_TM];
+  const uint32_t s = blockIdx.x;
   const uint32_t CW = (C + 31) / 32;
   if (threadIdx.x < CW) cm[threadIdx.x] = cmask[(size_t)s * CW + threadIdx.x];
+  const bool staged = W <= LOF_IG_TM;
+  if (staged) for (uint32_t w = threadIdx.x; w < W; w += 256) tm[w] = tmask[(size_t)s * W + w];
   __syncthreads();
-  if (i >= C * W) return;
-  const uint32_t c = i / W, w = i - c * W;
-  const bool cf = (cm[c >> 5] >> (c & 31)) & 1u;
-  const uint32_t full = (w == W - 1 && (T & 31)) ? ((1u << (T & 31)) - 1u) : 0xFFFFFFFFu;
-  flags[(size_t)s * C * W + i] = cf ? full : __ldg(tmask + (size_t)s * W + w);
+  const uint32_t last = (T & 31) ? ((1u << (T & 31)) - 1u) : 0xFFFFFFFFu;
+  uint32_t* fo = flags + (size_t)s * C * W;
+  for (uint32_t i = threadIdx.x; i < C * W; i += 256) {
+    const uint32_t c = i / W, w = i - c * W;
+    const bool cf = (cm[c >> 5] >> (c & 31)) & 1u;
+    const uint32_t full = (w == W - 1) ? last : 0xFFFFFFFFu;
+    fo[i] = cf ? full : (staged ? tm[w] : __ldg(tmask + (size_t)s * W + w));
+  }
 }
 
 // ---- one SumThreshold run over a short vector (n <= LOF_VEC_MAX), statistics included: one CTA per vector.
