@@ -151,6 +151,8 @@ static cudaError_t lof_generic_set_attributes(size_t smem_freq, size_t smem_time
   A(cudaFuncSetAttribute(lof_k_freq_generic<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, f));
   A(cudaFuncSetAttribute(lof_k_time_generic<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, t));
   A(cudaFuncSetAttribute(lof_k_time_generic<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, t));
+  A(cudaFuncSetAttribute(lof_k_time_seg<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, LOF_SEG_SMEM));
+  A(cudaFuncSetAttribute(lof_k_time_seg<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, LOF_SEG_SMEM));
   A(cudaFuncSetAttribute(lof_k_time_coop<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LofCoopSmem)));
   A(cudaFuncSetAttribute(lof_k_time_coop<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LofCoopSmem)));
   return e;
@@ -334,14 +336,20 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
     if (fast && c->lr_time) {
       if (freq_reg) used = LOF_PATH_LONGROW_SEG;
       n_part = c->n_seg;
-      const uint32_t nb_t = (uint32_t)(((uint64_t)rows * n_part + LOF_LR_WARPS - 1) / LOF_LR_WARPS);
-      lof_k_time_seg<In><<<nb_t, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum,
+      uint32_t nb_t = (uint32_t)(((uint64_t)rows * n_part + LOF_LR_WARPS - 1) / LOF_LR_WARPS);
+      if (nb_t > (uint32_t)c->sm_count * 2) nb_t = (uint32_t)c->sm_count * 2;     // persistent: two CTAs per SM
+      lof_k_time_seg<In><<<nb_t, LOF_LR_THREADS, LOF_SEG_SMEM, st>>>(in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum,
                                                         c->d_part_cnt, c->d_stats, c->seg_out, c->seg_halo, n_part, rows);
     } else if (fast && kp.n_lev_t <= 10) {                // the cooperative kernel exchanges windows of up to 512
       if (freq_reg) used = LOF_PATH_LONGROW_COOP;
       n_part = c->n_co;
-      lof_k_time_coop<In><<<rows * n_part, LOF_CO_WARPS * 32, sizeof(LofCoopSmem), st>>>(
-          in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum, c->d_part_cnt, c->d_stats, c->co_out, c->seg_halo, n_part);
+      {
+        const uint32_t n_units = rows * n_part;               // persistent: two CTAs per SM walk over the tiles
+        const uint32_t grid = n_units < (uint32_t)c->sm_count * 2 ? n_units : (uint32_t)c->sm_count * 2;
+        lof_k_time_coop<In><<<grid, LOF_CO_WARPS * 32, sizeof(LofCoopSmem), st>>>(
+            in, kp, c->d_state, c->d_fmask, d_flags, c->d_part_sum, c->d_part_cnt, c->d_stats, c->co_out, c->seg_halo, n_part,
+            n_units);
+      }
     } else {
       n_part = c->n_tiles;
       lof_k_time_generic<In><<<rows * c->n_tiles, LOF_GEN_THREADS, c->smem_time, st>>>(

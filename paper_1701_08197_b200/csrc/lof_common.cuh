@@ -63,6 +63,9 @@ struct InF32 {
     x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
   }
   static constexpr int kBytes = 4;
+  // a sample as it lies in memory (4 bytes) <-> the float32 power; `is_raw` = false: the word already holds the power
+  __device__ __forceinline__ static uint32_t raw_of(float x) { return __float_as_uint(x); }
+  __device__ __forceinline__ static float from_raw(uint32_t w, bool) { return __uint_as_float(w); }
 };
 struct InCI16 {
   const int16_t* p;
@@ -81,6 +84,14 @@ struct InCI16 {
     }
   }
   static constexpr int kBytes = 4;
+  // staging strips filled by asynchronous copies hold the voltage pair itself (is_raw), those filled through ld()
+  // the power
+  __device__ __forceinline__ static uint32_t raw_of(float x) { return __float_as_uint(x); }
+  __device__ __forceinline__ static float from_raw(uint32_t w, bool is_raw) {
+    if (!is_raw) return __uint_as_float(w);
+    const int re = (int)(short)(w & 0xFFFFu), im = (int)w >> 16;
+    return __uint2float_rn((unsigned)(re * re) + (unsigned)(im * im));
+  }
 };
 
 // cycles of thread 0 per phase, summed over CTAs and streams, when built with -DLOF_FUSED_PROF (profiling builds

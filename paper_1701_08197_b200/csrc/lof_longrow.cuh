@@ -13,6 +13,7 @@
 #define LOF_LR_THREADS 256
 #define LOF_LR_WARPS (LOF_LR_THREADS / 32)
 #define LOF_LR_TILE 1024
+#define LOF_SEG_SMEM (2 * LOF_LR_WARPS * LOF_LR_TILE * 4)
 
 template <int C, class In>
 __global__ void __launch_bounds__(LOF_LR_THREADS)
@@ -56,84 +57,118 @@ __device__ __forceinline__ float lof_sum_unflagged(const float2 (&x2)[16], uint3
   return (p0 + p1) + (p2 + p3);
 }
 
+// 16-byte asynchronous global -> shared copy (LDGSTS), and "all of this thread's copy groups but the newest n"
+__device__ __forceinline__ void lof_lr_cp16(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void lof_lr_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void lof_lr_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// Persistent: a warp walks over units (row segments) gw, gw + #warps, ...  When the rows are 16-byte aligned
+// (T % 4 == 0) the strip of the NEXT unit is on its way into the warp's second staging strip (LDGSTS, raw 4-byte
+// samples: float32, or complex int16 turned into power when the registers are filled) while the current one is
+// processed: the kernel had been stalled on its own loads (3.1 warps per issued instruction waiting on global
+// memory, 16 warps per SM).  Otherwise the strip is filled synchronously as before.
 template <class In>
 __global__ void __launch_bounds__(LOF_LR_THREADS, 2)
 lof_k_time_seg(In in, LofKParams prm, const LofStreamState* __restrict__ state, const uint32_t* __restrict__ fmask,
                uint32_t* __restrict__ flags, double* __restrict__ part_sum, uint32_t* __restrict__ part_cnt,
                lof_stream_stats* __restrict__ stats, uint32_t OUT, uint32_t H, uint32_t n_seg, uint32_t n_rows) {
-  __shared__ __align__(16) float stage[LOF_LR_WARPS][LOF_LR_TILE];
+  extern __shared__ __align__(16) unsigned char seg_raw[];          // LOF_SEG_SMEM bytes: [2][warps][tile] words
+  uint32_t (*stage)[LOF_LR_WARPS][LOF_LR_TILE] = reinterpret_cast<uint32_t (*)[LOF_LR_WARPS][LOF_LR_TILE]>(seg_raw);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint64_t unit = (uint64_t)blockIdx.x * LOF_LR_WARPS + warp;
-  if (unit >= (uint64_t)n_rows * n_seg) return;
-  const uint32_t rl = (uint32_t)(unit / n_seg), seg = (uint32_t)(unit - (uint64_t)rl * n_seg);
   const uint32_t W = prm.W, C = prm.C, T = prm.T;
-  const uint64_t row = (uint64_t)prm.s0 * C + rl;
-  const uint32_t s = (uint32_t)(row / C);
-  const LofStreamState& st = state[s];
-  const uint32_t o_lo = seg * OUT, o_hi = min(T, o_lo + OUT);
-  const uint32_t t_lo = o_lo >= H ? o_lo - H : 0;        // multiple of 32
-  float* sg = stage[warp];
-  const uint64_t base = row * T;
-  if ((T & 3) == 0) {
-    // 16-byte loads, eight in flight per lane (t_lo is a multiple of 32, the row start of 4 when T is)
-    float4* sg4 = reinterpret_cast<float4*>(sg);
+  const uint64_t n_units = (uint64_t)n_rows * n_seg, n_warps = (uint64_t)gridDim.x * LOF_LR_WARPS;
+  const bool async = (T & 3) == 0;
+  const unsigned char* raw = reinterpret_cast<const unsigned char*>(in.p);
+  // strip of unit u -> staging strip `buf` (chunks beyond the row's end are left alone: masked when read)
+  auto issue = [&](uint64_t u, int buf) {
+    const uint32_t rl = (uint32_t)(u / n_seg), seg = (uint32_t)(u - (uint64_t)rl * n_seg);
+    const uint64_t row = (uint64_t)prm.s0 * C + rl;
+    const uint32_t o_lo = seg * OUT, t_lo = o_lo >= H ? o_lo - H : 0;
+    uint4* sg4 = reinterpret_cast<uint4*>(stage[buf][warp]);
 #pragma unroll
     for (int q = 0; q < LOF_LR_TILE / 128; ++q) {
       const int g = q * 32 + lane;
       const uint32_t t = t_lo + 4 * g;
-      float v[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};   // beyond the row: never flagged, kills windows
-      if (t < T) in.ld4(base + t, v);
-      sg4[g ^ ((g >> 3) & 7)] = make_float4(v[0], v[1], v[2], v[3]);
+      if (t < T) lof_lr_cp16(sg4 + (g ^ ((g >> 3) & 7)), raw + (row * T + t) * 4);
     }
-  } else {
-#pragma unroll 4
-    for (int q = 0; q < LOF_LR_TILE / 32; ++q) {
-      const int i = q * 32 + lane;
-      const uint32_t t = t_lo + i;
-      sg[lof_lr_swz(i)] = t < T ? in.ld(base + t) : -INFINITY;
-    }
-  }
-  __syncwarp();
-  // the lane's 32 samples from the staging strip (again on a restart: the strip keeps the raw samples)
-  auto load = [&](float2 (&x2)[16], bool) {
-#pragma unroll
-    for (int q = 0; q < 8; ++q) {
-      const float4 v = reinterpret_cast<const float4*>(sg)[(8 * lane + q) ^ (lane & 7)];
-      x2[2 * q] = make_float2(v.x, v.y); x2[2 * q + 1] = make_float2(v.z, v.w);
-    }
+    lof_lr_commit();
   };
-  const uint32_t t_w = t_lo + 32 * lane;                  // first sample of this lane's word
-  const uint32_t valid = t_w >= T ? 0u : (T - t_w >= 32 ? 0xFFFFFFFFu : ((1u << (T - t_w)) - 1u));
-  // start from the frequency run's mask (F10): its flagged samples enter the row core as LOF_MARK
-  uint32_t fb = 0;
-  if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];
-  float lane_sum = 0.f;
-  bool have_sum = false;
-  if (st.nonfinite) fb = valid;                           // DESIGN.md S6: the whole stream is flagged
-  else if (prm.n_lev_t > 0) {
-    lof_row_flag<32, 7>(load, fb, st.thr_f, st.dead_t, (int)prm.n_lev_t, lane, lane_sum);
-    have_sum = true;
-  }
-  fb &= valid;
-  const bool mine = t_w >= o_lo && t_w < o_hi;            // this lane's word belongs to the segment's output
-  if (mine) flags[row * W + (t_w >> 5)] = fb;
-  if (!have_sum || valid != 0xFFFFFFFFu) {                // (-inf beyond the row's end)
-    float2 x2[16];
-    load(x2, true);
-    lane_sum = lof_sum_unflagged(x2, fb | ~valid);
-  }
-  double rs = mine ? (double)lane_sum : 0.0;
-  rs = lof_warp_sum(rs);
-  uint32_t nf = mine ? __popc(fb) : 0u, nu = mine ? __popc(valid & ~fb) : 0u;
+  uint64_t unit = (uint64_t)blockIdx.x * LOF_LR_WARPS + warp;
+  int buf = 0;
+  if (async && unit < n_units) issue(unit, 0);
+#pragma unroll 1
+  for (; unit < n_units; unit += n_warps, buf ^= 1) {
+    const uint32_t rl = (uint32_t)(unit / n_seg), seg = (uint32_t)(unit - (uint64_t)rl * n_seg);
+    const uint64_t row = (uint64_t)prm.s0 * C + rl;
+    const uint32_t s = (uint32_t)(row / C);
+    const LofStreamState& st = state[s];
+    const uint32_t o_lo = seg * OUT, o_hi = min(T, o_lo + OUT);
+    const uint32_t t_lo = o_lo >= H ? o_lo - H : 0;        // multiple of 32
+    uint32_t* sg = stage[buf][warp];
+    const uint64_t base = row * T;
+    if (async) {
+      if (unit + n_warps < n_units) { issue(unit + n_warps, buf ^ 1); lof_lr_wait<1>(); }
+      else lof_lr_wait<0>();
+    } else {
+#pragma unroll 4
+      for (int q = 0; q < LOF_LR_TILE / 32; ++q) {
+        const int i = q * 32 + lane;
+        const uint32_t t = t_lo + i;
+        sg[lof_lr_swz(i)] = t < T ? In::raw_of(in.ld(base + t)) : 0u;
+      }
+    }
+    __syncwarp();
+    const uint32_t t_w = t_lo + 32 * lane;                  // first sample of this lane's word
+    const uint32_t valid = t_w >= T ? 0u : (T - t_w >= 32 ? 0xFFFFFFFFu : ((1u << (T - t_w)) - 1u));
+    // the lane's 32 samples from the staging strip (again on a restart: the strip keeps the raw samples);
+    // beyond the row's end: -inf, which never exceeds a threshold and kills every window it is part of
+    auto load = [&](float2 (&x2)[16], bool) {
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    nf += __shfl_down_sync(0xffffffffu, nf, o);
-    nu += __shfl_down_sync(0xffffffffu, nu, o);
-  }
-  if (lane == 0) {
-    part_sum[(uint64_t)rl * n_seg + seg] = rs;
-    part_cnt[(uint64_t)rl * n_seg + seg] = nu;
-    if (nf) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[s].n_flagged), (unsigned long long)nf);
+      for (int q = 0; q < 8; ++q) {
+        const uint4 v = reinterpret_cast<const uint4*>(sg)[(8 * lane + q) ^ (lane & 7)];
+        x2[2 * q] = make_float2(In::from_raw(v.x, async), In::from_raw(v.y, async));
+        x2[2 * q + 1] = make_float2(In::from_raw(v.z, async), In::from_raw(v.w, async));
+      }
+      if (valid != 0xFFFFFFFFu) {
+#pragma unroll
+        for (int m = 0; m < 16; ++m) {
+          if (!((valid >> (2 * m)) & 1u)) x2[m].x = -INFINITY;
+          if (!((valid >> (2 * m + 1)) & 1u)) x2[m].y = -INFINITY;
+        }
+      }
+    };
+    // start from the frequency run's mask (F10): its flagged samples enter the row core as LOF_MARK
+    uint32_t fb = 0;
+    if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];
+    float lane_sum = 0.f;
+    bool have_sum = false;
+    if (st.nonfinite) fb = valid;                           // DESIGN.md S6: the whole stream is flagged
+    else if (prm.n_lev_t > 0) {
+      lof_row_flag<32, 7>(load, fb, st.thr_f, st.dead_t, (int)prm.n_lev_t, lane, lane_sum);
+      have_sum = true;
+    }
+    fb &= valid;
+    const bool mine = t_w >= o_lo && t_w < o_hi;            // this lane's word belongs to the segment's output
+    if (mine) flags[row * W + (t_w >> 5)] = fb;
+    if (!have_sum || valid != 0xFFFFFFFFu) {
+      float2 x2[16];
+      load(x2, true);
+      lane_sum = lof_sum_unflagged(x2, fb | ~valid);
+    }
+    double rs = mine ? (double)lane_sum : 0.0;
+    rs = lof_warp_sum(rs);
+    const uint32_t nf = __reduce_add_sync(0xffffffffu, mine ? (uint32_t)__popc(fb) : 0u);
+    const uint32_t nu = __reduce_add_sync(0xffffffffu, mine ? (uint32_t)__popc(valid & ~fb) : 0u);
+    if (lane == 0) {
+      part_sum[(uint64_t)rl * n_seg + seg] = rs;
+      part_cnt[(uint64_t)rl * n_seg + seg] = nu;
+      if (nf) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[s].n_flagged), (unsigned long long)nf);
+    }
+    __syncwarp();                                           // the strip is free for the prefetch after next
   }
 }
 
@@ -145,7 +180,8 @@ lof_k_time_seg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
 #define LOF_CO_TILE (LOF_CO_WARPS * LOF_LR_TILE)
 
 struct LofCoopSmem {
-  float stage[LOF_CO_WARPS][LOF_LR_TILE];               // load staging, one 1024-sample strip per warp
+  uint32_t stage[2][LOF_CO_WARPS][LOF_LR_TILE];         // load staging (raw 4-byte samples), one 1024-sample strip per
+                                                        // warp, double-buffered over the CTA's tiles
   float bu[2][LOF_CO_WARPS][256];                       // published window sums (double-buffered by level)
   float be[2][LOF_CO_WARPS][256];                       // published counts
   int wmax[LOF_CO_WARPS];                               // last fired window start per warp
@@ -242,49 +278,72 @@ template <class In>
 __global__ void __launch_bounds__(LOF_CO_WARPS * 32, 2)
 lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state, const uint32_t* __restrict__ fmask,
                 uint32_t* __restrict__ flags, double* __restrict__ part_sum, uint32_t* __restrict__ part_cnt,
-                lof_stream_stats* __restrict__ stats, uint32_t OUT, uint32_t H, uint32_t n_tile) {
+                lof_stream_stats* __restrict__ stats, uint32_t OUT, uint32_t H, uint32_t n_tile, uint32_t n_units) {
   extern __shared__ __align__(16) unsigned char co_raw[];
   LofCoopSmem& sm = *reinterpret_cast<LofCoopSmem*>(co_raw);
   __shared__ double red_sum[LOF_CO_WARPS];
   __shared__ uint32_t red_cnt[2][LOF_CO_WARPS];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint32_t rl = blockIdx.x / n_tile, tile = blockIdx.x - rl * n_tile;
   const uint32_t W = prm.W, C = prm.C, T = prm.T;
+  const bool async = (T & 3) == 0;
+  const unsigned char* raw = reinterpret_cast<const unsigned char*>(in.p);
+  // persistent over tiles: the strips of the NEXT tile are on their way (LDGSTS) while this one is processed — the
+  // kernel had 5 warps per issued instruction waiting on its own global loads
+  auto issue = [&](uint32_t u, int buf) {
+    const uint32_t rl = u / n_tile, tile = u - rl * n_tile;
+    const uint64_t row = (uint64_t)prm.s0 * C + rl;
+    const uint32_t o_lo = tile * OUT;
+    const uint32_t t_lo = (o_lo >= H ? o_lo - H : 0) + warp * LOF_LR_TILE;
+    uint4* sg4 = reinterpret_cast<uint4*>(sm.stage[buf][warp]);
+#pragma unroll
+    for (int q = 0; q < LOF_LR_TILE / 128; ++q) {
+      const int g = q * 32 + lane;
+      const uint32_t t = t_lo + 4 * g;
+      if (t < T) lof_lr_cp16(sg4 + (g ^ ((g >> 3) & 7)), raw + (row * T + t) * 4);
+    }
+    lof_lr_commit();
+  };
+  int buf = 0;
+  if (async && blockIdx.x < n_units) issue(blockIdx.x, 0);
+#pragma unroll 1
+  for (uint32_t unit = blockIdx.x; unit < n_units; unit += gridDim.x, buf ^= 1) {
+  const uint32_t rl = unit / n_tile, tile = unit - rl * n_tile;
   const uint64_t row = (uint64_t)prm.s0 * C + rl;
   const uint32_t s = (uint32_t)(row / C);
   const LofStreamState& st = state[s];
   const uint32_t o_lo = tile * OUT, o_hi = min(T, o_lo + OUT);
   const uint32_t t_lo = (o_lo >= H ? o_lo - H : 0) + warp * LOF_LR_TILE;   // this warp's strip
-  float* sg = sm.stage[warp];
+  uint32_t* sg = sm.stage[buf][warp];
   const uint64_t base = row * T;
-  if ((T & 3) == 0) {
-    float4* sg4 = reinterpret_cast<float4*>(sg);
-#pragma unroll
-    for (int q = 0; q < LOF_LR_TILE / 128; ++q) {
-      const int g = q * 32 + lane;
-      const uint32_t t = t_lo + 4 * g;
-      float v[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-      if (t < T) in.ld4(base + t, v);
-      sg4[g ^ ((g >> 3) & 7)] = make_float4(v[0], v[1], v[2], v[3]);
-    }
+  if (async) {
+    if (unit + gridDim.x < n_units) { issue(unit + gridDim.x, buf ^ 1); lof_lr_wait<1>(); }
+    else lof_lr_wait<0>();
   } else {
 #pragma unroll 4
     for (int q = 0; q < LOF_LR_TILE / 32; ++q) {
       const int i = q * 32 + lane;
       const uint32_t t = t_lo + i;
-      sg[lof_lr_swz(i)] = t < T ? in.ld(base + t) : -INFINITY;
+      sg[lof_lr_swz(i)] = t < T ? In::raw_of(in.ld(base + t)) : 0u;
     }
   }
   __syncwarp();
+  const uint32_t t_w = t_lo + 32 * lane;
+  const uint32_t valid = t_w >= T ? 0u : (T - t_w >= 32 ? 0xFFFFFFFFu : ((1u << (T - t_w)) - 1u));
   auto load = [&](float2 (&x2)[16]) {
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
-      const float4 v = reinterpret_cast<const float4*>(sg)[(8 * lane + q) ^ (lane & 7)];
-      x2[2 * q] = make_float2(v.x, v.y); x2[2 * q + 1] = make_float2(v.z, v.w);
+      const uint4 v = reinterpret_cast<const uint4*>(sg)[(8 * lane + q) ^ (lane & 7)];
+      x2[2 * q] = make_float2(In::from_raw(v.x, async), In::from_raw(v.y, async));
+      x2[2 * q + 1] = make_float2(In::from_raw(v.z, async), In::from_raw(v.w, async));
+    }
+    if (valid != 0xFFFFFFFFu) {                           // beyond the row's end: -inf
+#pragma unroll
+      for (int m = 0; m < 16; ++m) {
+        if (!((valid >> (2 * m)) & 1u)) x2[m].x = -INFINITY;
+        if (!((valid >> (2 * m + 1)) & 1u)) x2[m].y = -INFINITY;
+      }
     }
   };
-  const uint32_t t_w = t_lo + 32 * lane;
-  const uint32_t valid = t_w >= T ? 0u : (T - t_w >= 32 ? 0xFFFFFFFFu : ((1u << (T - t_w)) - 1u));
   uint32_t fb = 0;
   if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];   // the frequency run's flags (F10)
   const int nlt = (int)prm.n_lev_t;
@@ -363,5 +422,7 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
     part_sum[(uint64_t)rl * n_tile + tile] = a;
     part_cnt[(uint64_t)rl * n_tile + tile] = cu;
     if (cf) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[s].n_flagged), (unsigned long long)cf);
+  }
+  __syncthreads();                                        // the reductions' scratch and the staging strips are free
   }
 }
