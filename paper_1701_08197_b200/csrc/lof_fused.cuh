@@ -42,7 +42,11 @@ struct LofFusedCfg {
 #else
   static constexpr int NT = (C >= 64) ? 512 : 256;
 #endif
+#ifdef LOF_FUSED_MINB
+  static constexpr int MINB = LOF_FUSED_MINB;
+#else
   static constexpr int MINB = (C >= 64) ? 1 : 2;
+#endif
   // the next stream's statistics pass runs inside the time pass when the SM holds a single CTA; with two
   // CTAs per SM their phases interleave anyway and the plain order measured faster
 #ifdef LOF_STAT_OVERLAP

@@ -16,7 +16,7 @@
 #define LOF_SEG_SMEM (2 * LOF_LR_WARPS * LOF_LR_TILE * 4)
 
 template <int C, class In>
-__global__ void __launch_bounds__(LOF_LR_THREADS)
+__global__ void __launch_bounds__(LOF_LR_THREADS, (C <= 32 ? 2 : 1))
 lof_k_freq_reg(In in, LofKParams prm, const LofStreamState* __restrict__ state, uint32_t* __restrict__ fmask,
                uint32_t n_group_streams) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -182,9 +182,11 @@ lof_k_time_seg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
 struct LofCoopSmem {
   uint32_t stage[2][LOF_CO_WARPS][LOF_LR_TILE];         // load staging (raw 4-byte samples), one 1024-sample strip per
                                                         // warp, double-buffered over the CTA's tiles
-  float bu[2][LOF_CO_WARPS][256];                       // published window sums (double-buffered by level)
-  float be[2][LOF_CO_WARPS][256];                       // published counts
+  float bu[LOF_CO_WARPS][512];                          // published window sums: the first D of step D at [D, 2D), so
+  float be[LOF_CO_WARPS][512];                          // every step keeps its own (a strip that sits out a restart
+                                                        // does not publish again); be: the counts
   int wmax[LOF_CO_WARPS];                               // last fired window start per warp
+  int chg[LOF_CO_WARPS];                                // strip got new flags in the last test
 };
 
 // One doubling step of distance D on a strip of 1024 samples (lane l: 32 samples as 16 pairs); partners beyond
@@ -228,7 +230,8 @@ __device__ __forceinline__ void lof_row_step_coop(float2 (&u2)[16], float2 (&e2)
 // into this one (carry through wmax[]), and "any" is taken over the CTA.  Contains __syncthreads: CTA-uniform.
 template <int K>
 __device__ __forceinline__ bool lof_row_eval_coop(const float2 (&u2)[16], const float2 (&e2)[16], int lane, int warp,
-                                                  float thr, float tdead, uint32_t& fb, int* wmax, bool& dead) {
+                                                  float thr, float tdead, uint32_t& fb, int* wmax, int* chg,
+                                                  bool& dead) {
   constexpr int I = 1 << K;
   const float2 negT = make_float2(-thr, -thr), negD = make_float2(-tdead, -tdead);
   float tm[2] = {-INFINITY, -INFINITY}, td[2] = {-INFINITY, -INFINITY};
@@ -269,6 +272,8 @@ __device__ __forceinline__ bool lof_row_eval_coop(const float2 (&u2)[16], const 
   const uint32_t nf = fb | own | pre;
   const bool changed = nf != fb;
   fb = nf;
+  const bool wch = __any_sync(0xffffffffu, changed);
+  if (lane == 0) chg[warp] = wch;
   return __syncthreads_or(changed) != 0;
 }
 
@@ -359,16 +364,22 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
     bool again = true;
     const bool has_nb = warp + 1 < LOF_CO_WARPS;
     have_sum = true;
+    // A restart rebuilds the trees only in the strips that can have changed: those with new flags and the one
+    // before each (its windows reach up to 511 samples into the next strip).  The other warps keep the trees of
+    // the iteration that fired, whose published sums are still in place, and join again at iteration k_next;
+    // they pass the same barriers.  (Restarting all 8 warps for every new flag in 8192 samples had been most of
+    // this kernel's instructions.)
+    bool sit = false;
+    float mu = 0.f;
 #pragma unroll 1
     while (again) {
-      float mu = 0.f;
-      {
+      if (!sit) {
         float2 x2[16];
         load(x2);
         if (fb) lof_mark<16>(x2, fb);                     // flags of the frequency run and of earlier restarts
         fb = ~lof_level0<16>(x2, T0, u2, e2, mu);
+        lane_sum = lof_lane_sum<16>(u2);
       }
-      lane_sum = lof_lane_sum<16>(u2);
       // no iteration left, or no unflagged sample of the tile above every later threshold (lof_dead_level)
       if (k_next >= nlt || __syncthreads_and(mu <= D0)) break;
       again = false;
@@ -376,9 +387,10 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
 #define LOF_CO_LEVEL(K)                                                                          \
       if (K < nlt && !again && !dead_) {                                                         \
         constexpr int D = 1 << (K - 1);                                                          \
-        float* pbu = sm.bu[K & 1][warp]; float* pbe = sm.be[K & 1][warp];                        \
+        const bool act = !sit || K >= k_next;                                                    \
+        float* pbu = sm.bu[warp] + D; float* pbe = sm.be[warp] + D;                              \
         /* publish the first D sums / counts of this strip for the previous warp */             \
-        if (lane * 32 < D) {                                                                     \
+        if (act && lane * 32 < D) {                                                              \
           _Pragma("unroll") for (int m = 0; m < 16; ++m) if (lane * 32 + 2 * m < D) {            \
             if (D == 1) { pbu[0] = u2[0].x; pbe[0] = e2[0].x; }                                  \
             else { *reinterpret_cast<float2*>(pbu + lane * 32 + 2 * m) = u2[m];                  \
@@ -386,10 +398,11 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
           }                                                                                      \
         }                                                                                        \
         __syncthreads();                                                                         \
-        lof_row_step_coop<D>(u2, e2, lane, sm.bu[K & 1][has_nb ? warp + 1 : warp],               \
-                             sm.be[K & 1][has_nb ? warp + 1 : warp], has_nb);                    \
-        if (K >= k_next && lof_row_eval_coop<K>(u2, e2, lane, warp, thr[K], dead[K], fb, sm.wmax, dead_)) { \
+        if (act) lof_row_step_coop<D>(u2, e2, lane, sm.bu[has_nb ? warp + 1 : warp] + D,         \
+                                      sm.be[has_nb ? warp + 1 : warp] + D, has_nb);              \
+        if (K >= k_next && lof_row_eval_coop<K>(u2, e2, lane, warp, thr[K], dead[K], fb, sm.wmax, sm.chg, dead_)) { \
           again = true; k_next = K + 1 < nlt ? K + 1 : 99;                                       \
+          sit = !(sm.chg[warp] || (has_nb && sm.chg[warp + 1]));                                 \
         }                                                                                        \
       }
       LOF_CO_LEVEL(1) LOF_CO_LEVEL(2) LOF_CO_LEVEL(3) LOF_CO_LEVEL(4) LOF_CO_LEVEL(5)
