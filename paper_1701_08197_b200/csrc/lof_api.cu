@@ -151,6 +151,10 @@ static cudaError_t lof_generic_set_attributes(size_t smem_freq, size_t smem_time
   A(cudaFuncSetAttribute(lof_k_freq_generic<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, f));
   A(cudaFuncSetAttribute(lof_k_time_generic<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, t));
   A(cudaFuncSetAttribute(lof_k_time_generic<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, t));
+  A(cudaFuncSetAttribute(lof_k_freq_stg<32, InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, LOF_FREQ_SMEM(32)));
+  A(cudaFuncSetAttribute(lof_k_freq_stg<32, InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, LOF_FREQ_SMEM(32)));
+  A(cudaFuncSetAttribute(lof_k_freq_stg<64, InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, LOF_FREQ_SMEM(64)));
+  A(cudaFuncSetAttribute(lof_k_freq_stg<64, InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, LOF_FREQ_SMEM(64)));
   A(cudaFuncSetAttribute(lof_k_time_seg<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, LOF_SEG_SMEM));
   A(cudaFuncSetAttribute(lof_k_time_seg<InCI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, LOF_SEG_SMEM));
   A(cudaFuncSetAttribute(lof_k_time_coop<InF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LofCoopSmem)));
@@ -319,13 +323,16 @@ static int flag_block_generic(lof_ctx* c, In in, uint32_t* d_flags, cudaStream_t
     const bool fast = c->path == 0;                     // path 1 forces the shared-memory generic kernels
     int used = LOF_PATH_GENERIC;
     if (kp.n_lev_f) {
-      const uint32_t nb_f = (uint32_t)(((uint64_t)G * kp.W + LOF_LR_WARPS - 1) / LOF_LR_WARPS);
-      if (fast && c->lr_freq && C == 16)
-        lof_k_freq_reg<16, In><<<nb_f, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, G);
+      // persistent: as many CTAs as the SMs hold (2 / 1 per SM for 32 / 64 channels)
+      const uint32_t nb_all = (uint32_t)(((uint64_t)G * kp.W + LOF_LR_WARPS - 1) / LOF_LR_WARPS);
+      const uint32_t nb_res = (uint32_t)c->sm_count * (C == 32 ? 2u : 1u);
+      const uint32_t nb_f = nb_all < nb_res ? nb_all : nb_res;
+      if (fast && c->lr_freq && C == 16)                  // not staged: a CTA per 8 units
+        lof_k_freq_reg<16, In><<<nb_all, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, G);
       else if (fast && c->lr_freq && C == 32)
-        lof_k_freq_reg<32, In><<<nb_f, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, G);
+        lof_k_freq_stg<32, In><<<nb_f, LOF_LR_THREADS, LOF_FREQ_SMEM(32), st>>>(in, kp, c->d_state, c->d_fmask, G);
       else if (fast && c->lr_freq && C == 64)
-        lof_k_freq_reg<64, In><<<nb_f, LOF_LR_THREADS, 0, st>>>(in, kp, c->d_state, c->d_fmask, G);
+        lof_k_freq_stg<64, In><<<nb_f, LOF_LR_THREADS, LOF_FREQ_SMEM(64), st>>>(in, kp, c->d_state, c->d_fmask, G);
       else
         lof_k_freq_generic<In><<<G * kp.W, LOF_GEN_THREADS, c->smem_freq, st>>>(in, kp, c->d_state, c->d_fmask);
       c->launches += 1;

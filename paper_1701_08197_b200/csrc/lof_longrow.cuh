@@ -2,7 +2,8 @@
 // memory (BASELINE.json configs 4 and 5: rows of 195 312 and 12 208 samples).  Same column / row cores as
 // the fused kernel (lof_col_flag, lof_row_flag in lof_fused.cuh), fed from global memory after the
 // statistics passes of lof_stats_lr.cuh (one group of streams per launch sequence).
-//   lof_k_freq_reg<C>: a warp per group of 32 time columns, a thread per column.
+//   lof_k_freq_reg<C> / lof_k_freq_stg<C>: a warp per group of 32 time columns, a thread per column;
+//                      the second one persistent with the next unit staged by LDGSTS (32 and 64 channels).
 //   lof_k_time_seg   : a warp per row segment of 1024 samples = OUT output samples + a halo of H on
 //                      each side, H >= the dependency cone sum_k (2^k - 1) of the time run, so segments
 //                      are independent; lane l holds samples [32 l, 32 l + 32).
@@ -15,6 +16,8 @@
 #define LOF_LR_TILE 1024
 #define LOF_SEG_SMEM (2 * LOF_LR_WARPS * LOF_LR_TILE * 4)
 
+// One launch of a warp per unit, loads straight into registers: the form kept for 16 channels, which is bound by
+// instruction issue (70 % of the issue slots) and measured 8 % slower in the staged form below.
 template <int C, class In>
 __global__ void __launch_bounds__(LOF_LR_THREADS, (C <= 32 ? 2 : 1))
 lof_k_freq_reg(In in, LofKParams prm, const LofStreamState* __restrict__ state, uint32_t* __restrict__ fmask,
@@ -37,6 +40,78 @@ lof_k_freq_reg(In in, LofKParams prm, const LofStreamState* __restrict__ state, 
   if (C > 32 && lane + 32 < C) fmask[((uint64_t)s * C + lane + 32) * W + w] = mine1;
 }
 
+// 16-byte asynchronous global -> shared copy (LDGSTS), and "all of this thread's copy groups but the newest n"
+__device__ __forceinline__ void lof_lr_cp16(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void lof_lr_cp4(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void lof_lr_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void lof_lr_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// Persistent: a warp walks over units (stream, group of 32 columns).  With 16-byte aligned rows (T % 4 == 0) the
+// C x 32 samples of the NEXT unit are on their way into the warp's second staging strip (LDGSTS, C x 128 bytes,
+// raw 4-byte samples) while the current columns are processed: one load phase and one compute phase per warp had
+// left the SM waiting on memory with 8-16 warps resident (20 % of the warp slots, 4.6 warps per issued
+// instruction on the long scoreboard).  Shared memory: LOF_FREQ_SMEM(C) = 2 strips x 8 warps x C x 128 bytes.
+#define LOF_FREQ_SMEM(C) (2 * LOF_LR_WARPS * (C) * 128)
+template <int C, class In>
+__global__ void __launch_bounds__(LOF_LR_THREADS, (C <= 32 ? 2 : 1))
+lof_k_freq_stg(In in, LofKParams prm, const LofStreamState* __restrict__ state, uint32_t* __restrict__ fmask,
+               uint32_t n_group_streams) {
+  extern __shared__ __align__(16) unsigned char fr_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t W = prm.W, T = prm.T;
+  const uint64_t n_units = (uint64_t)n_group_streams * W, n_warps = (uint64_t)gridDim.x * LOF_LR_WARPS;
+  const bool async = (T & 3) == 0;
+  const unsigned char* raw = reinterpret_cast<const unsigned char*>(in.p);
+  auto strip = [&](int buf) { return reinterpret_cast<uint32_t*>(fr_raw) + (size_t)(buf * LOF_LR_WARPS + warp) * C * 32; };
+  auto issue = [&](uint64_t u, int buf) {
+    const uint32_t sl = (uint32_t)(u / W), w = (uint32_t)(u - (uint64_t)sl * W), s = prm.s0 + sl;
+    uint32_t* sg = strip(buf);
+#pragma unroll
+    for (int q = 0; q < C / 4; ++q) {
+      const int i = q * 32 + lane, c = i >> 3, ch = i & 7;
+      const uint32_t t = w * 32 + ch * 4;
+      if (t < T) lof_lr_cp16(sg + c * 32 + ch * 4, raw + (((uint64_t)s * C + c) * T + t) * 4);
+    }
+    lof_lr_commit();
+  };
+  uint64_t unit = (uint64_t)blockIdx.x * LOF_LR_WARPS + warp;
+  int buf = 0;
+  if (async && unit < n_units) issue(unit, 0);
+#pragma unroll 1
+  for (; unit < n_units; unit += n_warps, buf ^= 1) {
+    const uint32_t sl = (uint32_t)(unit / W), w = (uint32_t)(unit - (uint64_t)sl * W), s = prm.s0 + sl;
+    const uint32_t t = w * 32 + lane;
+    const bool valid = t < T;
+    const uint64_t base = (uint64_t)s * C * T + (valid ? t : 0);
+    const uint32_t* sg = strip(buf);
+    if (async) {
+      if (unit + n_warps < n_units) { issue(unit + n_warps, buf ^ 1); lof_lr_wait<1>(); }
+      else lof_lr_wait<0>();
+      __syncwarp();
+    }
+    const float* thr = state[s].thr_f;
+    // a column beyond the row's end holds -inf: it never exceeds a threshold and any window sum with it is -inf
+    const uint64_t fb = lof_col_flag<C>(
+        [&](int c) {
+          if (!valid) return -INFINITY;
+          return async ? In::from_raw(sg[c * 32 + lane], true) : in.ld(base + (uint64_t)c * T);
+        },
+        thr, state[s].dead_f, (int)prm.n_lev_f);
+    uint32_t mine0, mine1;
+    lof_col_words<C>(fb, lane, mine0, mine1);
+    if (lane < C) fmask[((uint64_t)s * C + lane) * W + w] = mine0;
+    if (C > 32 && lane + 32 < C) fmask[((uint64_t)s * C + lane + 32) * W + w] = mine1;
+    __syncwarp();                                         // the strip is free for the copy after next
+  }
+}
+
 // element i of a warp's 1024-sample staging tile: float4 chunk g = i/4 stored at g ^ ((g/8) & 7), so the
 // coalesced fill (lanes = consecutive i) and the per-lane reads of 32 consecutive floats are conflict-free
 __device__ __forceinline__ int lof_lr_swz(int i) {
@@ -56,15 +131,6 @@ __device__ __forceinline__ float lof_sum_unflagged(const float2 (&x2)[16], uint3
   }
   return (p0 + p1) + (p2 + p3);
 }
-
-// 16-byte asynchronous global -> shared copy (LDGSTS), and "all of this thread's copy groups but the newest n"
-__device__ __forceinline__ void lof_lr_cp16(void* smem_dst, const void* gsrc) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void lof_lr_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void lof_lr_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // Persistent: a warp walks over units (row segments) gw, gw + #warps, ...  When the rows are 16-byte aligned
 // (T % 4 == 0) the strip of the NEXT unit is on its way into the warp's second staging strip (LDGSTS, raw 4-byte
@@ -187,6 +253,7 @@ struct LofCoopSmem {
                                                         // does not publish again); be: the counts
   int wmax[LOF_CO_WARPS];                               // last fired window start per warp
   int chg[LOF_CO_WARPS];                                // strip got new flags in the last test
+  uint32_t fm[2][LOF_CO_WARPS][32];                     // the strips' frequency-run mask words, copied with them
 };
 
 // One doubling step of distance D on a strip of 1024 samples (lane l: 32 samples as 16 pairs); partners beyond
@@ -306,6 +373,7 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
       const uint32_t t = t_lo + 4 * g;
       if (t < T) lof_lr_cp16(sg4 + (g ^ ((g >> 3) & 7)), raw + (row * T + t) * 4);
     }
+    if (prm.n_lev_f > 0 && t_lo + 32 * lane < T) lof_lr_cp4(&sm.fm[buf][warp][lane], fmask + row * W + (t_lo >> 5) + lane);
     lof_lr_commit();
   };
   int buf = 0;
@@ -350,7 +418,7 @@ lof_k_time_coop(In in, LofKParams prm, const LofStreamState* __restrict__ state,
     }
   };
   uint32_t fb = 0;
-  if (prm.n_lev_f > 0 && valid) fb = fmask[row * W + (t_w >> 5)];   // the frequency run's flags (F10)
+  if (prm.n_lev_f > 0 && valid) fb = async ? sm.fm[buf][warp][lane] : fmask[row * W + (t_w >> 5)];   // the frequency run's flags (F10)
   const int nlt = (int)prm.n_lev_t;
   float lane_sum = 0.f;
   bool have_sum = false;
