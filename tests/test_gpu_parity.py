@@ -353,6 +353,32 @@ def test_long_rows_several_groups(lof, lofo, wl, S, C, T, mw, group, ci16, want)
         check(lof, lofo, x, S, C, T, max_window=mw, group=group, want_path=want_path)
 
 
+@pytest.mark.parametrize("T,mw,dirs,seed", [(8192 * 3 - 1024 * 2 + 17, 256, 3, 0), (20000, 512, 2, 1),
+                                            (7168 * 2, 128 * 2, 3, 2), (30011, 256, 3, 3)])
+def test_cooperative_tiles_partial_restarts(lof, lofo, T, mw, dirs, seed):
+    """lof_k_time_coop rebuilds, after new flags, only the strips that changed and the strip before each; the other
+    warps keep their trees and the sums they published.  Events of every length from 1 to 600 samples and
+    amplitudes from just above the widest window's threshold to 40 sigma, several per 8192-sample tile, so that
+    iterations of every window size fire in some strips and not in their neighbours; events across strip (1024)
+    and tile borders; flags compared bit by bit with the oracle (exact: the margin set must come out empty or
+    explained) on both the register path and the generic one."""
+    rng = np.random.default_rng(9100 + seed)
+    S, C = 2, 16
+    x = rng.standard_exponential((S, C, T)).astype(np.float32)
+    for s in range(S):
+        for c in range(C):
+            n_ev = int(rng.integers(T // 1500, T // 500))
+            for _ in range(n_ev):
+                ln = int(2 ** rng.uniform(0, np.log2(600)))
+                t0 = int(rng.integers(0, T - ln))
+                if rng.random() < 0.3:                   # pinned to a strip or tile border
+                    b = int(rng.integers(1, T // 1024)) * 1024
+                    t0 = max(0, min(T - ln, b - int(rng.integers(0, ln + 1))))
+                amp = float(np.exp(rng.uniform(np.log(0.3), np.log(40.0)))) / np.sqrt(max(1.0, ln / 8.0)) + 0.15
+                x[s, c, t0:t0 + ln] += np.float32(amp)
+    check(lof, lofo, x, S, C, T, max_window=mw, directions=dirs, want_path=lof.PATH_LONGROW_COOP)
+
+
 def test_generic_path_more_than_1024_streams(lof, lofo):
     """S > 1024: the generic path splits the block into groups of at most 1024 streams."""
     rng = np.random.default_rng(21)
