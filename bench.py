@@ -273,7 +273,10 @@ def run_gpu(args):
     if dist:
         dist.barrier()
     # ---- headline: BASELINE.json configs[1] batched over 64 subbands (each rank flags its own subbands)
-    r = time_config(lof, args.config, args.steps, args.warmup, local, seed=rank, sampler=sampler)
+    # --row: one of SURVEY.md §8(f)'s rows instead of the plain block (for profiling; use with --quick)
+    row_kw = {"sir": dict(sir_eta=0.2), "mad": dict(stats_mode=1)}.get(args.row, {})
+    r = time_config(lof, args.config, args.steps, args.warmup, local, seed=rank, sampler=sampler,
+                    mode="integrated" if args.row == "integrated" else "block", **row_kw)
     if dist:
         dist.barrier()
     sampler.stop_flag = True
@@ -316,7 +319,7 @@ def run_gpu(args):
         "ms_per_step_median": r["per"][len(r["per"]) // 2],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "real_time_factor": world * r["block_s"] * args.steps / (total_ms * 1e-3),
-        "config": {"workload": r["desc"], "S": S, "C": C, "T": T, **kw, "input_bytes": n_samples * 4,
+        "config": {"workload": r["desc"], "row": args.row, "S": S, "C": C, "T": T, **kw, "input_bytes": n_samples * 4,
                    "l2": "input larger than L2 (126 MB), two buffers alternated, no flush",
                    "preheat": "1.5 s of untimed steps before the timed ones (sustained clocks)"},
         "gpu_launches": r["launches"], "path": r["path"],
@@ -438,6 +441,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="lof", choices=["lof", "reference"])
     ap.add_argument("--config", default="cfg2")
+    ap.add_argument("--row", default="block", choices=["block", "sir", "integrated", "mad"],
+                    help="time the plain block (default) or a §8(f) row: SIR operator, integrated mode, MAD scale")
     ap.add_argument("--quick", action="store_true", help="headline only: no per_config / linearity / next_rows")
     args = ap.parse_args()
     if args.impl == "reference":
