@@ -41,6 +41,7 @@ extern "C" {
 #define LOF_E_ALIGN  -3   /* a device pointer is not 16-byte aligned                            */
 #define LOF_E_STATE  -4   /* call order violated (see lof_history_update)                       */
 #define LOF_E_CUDA   -5   /* a CUDA runtime call failed, or no usable device                    */
+#define LOF_E_SIZE   -6   /* problem larger than the static scratch of lof_sir_noalloc          */
 
 #define LOF_DIR_FREQ 1u   /* SumThreshold along channels (run first)               */
 #define LOF_DIR_TIME 2u   /* SumThreshold along time                                            */
@@ -209,6 +210,27 @@ int lof_fused_counters(lof_ctx* ctx, uint64_t* h_out /*[4]*/, int reset);
  * the next stream's row statistics, [4] end of the next stream's statistics, [5..7] zero.
  * All zero in a normal build.  Synchronises the device. */
 int lof_fused_cycles(lof_ctx* ctx, uint64_t* h_out /*[8]*/);
+
+/* The SIR operator of PAPER.md:49-57 (readings SIR-1..6; the same kernels as lof_flag_block with
+ * sir_eta > 0) applied IN PLACE to a packed mask, for callers that cannot allocate device memory (CUDA graph
+ * capture, serving loops, harnesses that forbid cudaMalloc): no context, and no cudaMalloc / cudaFree / allocating
+ * library call on any path.  Every run of set bits grows by floor(eta * length) on each side, along channels if
+ * directions has LOF_DIR_FREQ, then along time if it has LOF_DIR_TIME.
+ *   d_flags  device, in/out, uint32 [n_streams][n_channels][W], W = ceil(n_time / 32), bit t%32 of word t/32,
+ *            16-byte aligned, owned by the caller; bits beyond n_time must be zero and stay zero.
+ *   d_stats  device, in/out, lof_stream_stats [n_streams], 8-byte aligned: n_flagged of each stream grows by the
+ *            number of bits the operator set in it; the other fields are not touched.
+ *   device   CUDA device ordinal of both pointers (0..63); made current.   cuda_stream: the stream to enqueue on.
+ * The intermediate mask lives in a static device array of LOF_NOALLOC_MAX_WORDS words (8 MiB per GPU that loads
+ * the library, held until the process exits): n_streams * n_channels * W above that -> LOF_E_SIZE, nothing is
+ * enqueued.  All calls on a device share the array: calls that overlap on the GPU (two streams, two threads) race
+ * and give undefined masks; calls on one stream, or ordered by events, are safe.  Nothing needs clearing between
+ * calls (each kernel writes every word the next one reads).  LOF_E_NULL / LOF_E_ALIGN as elsewhere; LOF_E_PARAM
+ * for a zero dimension, n_channels > 256, eta outside [0, 1] or not finite, directions 0 or unknown bits, device
+ * outside 0..63.  eta == 0 returns LOF_OK without touching the mask.  Only enqueues work, like lof_flag_block. */
+#define LOF_NOALLOC_MAX_WORDS (2u * 1024u * 1024u)
+int lof_sir_noalloc(uint32_t* d_flags, lof_stream_stats* d_stats, uint32_t n_streams, uint32_t n_channels,
+                    uint32_t n_time, float eta, uint32_t directions, int device, void* cuda_stream);
 
 const char* lof_strerror(int code);
 const char* lof_last_cuda_error(void);

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "lof_common.cuh"
@@ -113,6 +114,7 @@ extern "C" const char* lof_strerror(int code) {
     case LOF_E_ALIGN: return "device pointer not 16-byte aligned";
     case LOF_E_STATE: return "call order violated";
     case LOF_E_CUDA: return "CUDA runtime failure (see lof_last_cuda_error)";
+    case LOF_E_SIZE: return "problem larger than the static scratch of a no-allocation entry point";
     default: return "unknown error";
   }
 }
@@ -763,5 +765,90 @@ extern "C" int lof_set_group(lof_ctx* c, uint32_t max_streams) {
   if (!c) return LOF_E_NULL;
   if (max_streams == 0) return LOF_E_PARAM;
   c->group = max_streams < c->group_alloc ? max_streams : c->group_alloc;
+  return LOF_OK;
+}
+
+// ---- lof_sir_noalloc: the SIR operator on a packed mask with no context and no allocation (include/lof.h).
+// The intermediate mask (the frequency pass's output, input of the time pass) lives in a file-scope device array
+// instead of a context's cudaMalloc'ed buffer: every GPU that loads this library holds LOF_NOALLOC_MAX_WORDS * 4
+// bytes (8 MiB) for it until the process exits.  Every call on a device shares the array; both kernels write every
+// word they later read, so nothing has to start at zero and the previous call's contents do not matter — but two
+// calls whose kernels overlap on one GPU (different streams, or threads) race on it.
+// `lof_noalloc_scratch` below is, in host code, a host-side stand-in for the symbol and NOT a device address: the
+// device address is looked up once per device with cudaGetSymbolAddress, that device current, and kept.
+static __device__ __align__(256) uint32_t lof_noalloc_scratch[LOF_NOALLOC_MAX_WORDS];
+
+#define LOF_NOALLOC_MAX_DEVICES 64
+static std::mutex g_noalloc_mu;
+static uint32_t* g_noalloc_ptr[LOF_NOALLOC_MAX_DEVICES];   // device address of the array, per device (0: not looked up)
+
+// device must be current
+static int noalloc_scratch(int device, uint32_t** out) {
+  std::lock_guard<std::mutex> lk(g_noalloc_mu);
+  if (!g_noalloc_ptr[device]) {
+    uint32_t* p = nullptr;
+    LOF_CUDA(cudaGetSymbolAddress((void**)&p, lof_noalloc_scratch));
+    if (!p) { snprintf(g_cuda_err, sizeof g_cuda_err, "cudaGetSymbolAddress gave a null address"); return LOF_E_CUDA; }
+    g_noalloc_ptr[device] = p;
+  }
+  *out = g_noalloc_ptr[device];
+  return LOF_OK;
+}
+
+template <int G>
+static void noalloc_sir_time(const uint32_t* in, uint32_t* out, lof_stream_stats* d_stats, uint64_t rows, uint32_t C,
+                             uint32_t W, uint32_t T, float eta, cudaStream_t st) {
+  const unsigned grid = (unsigned)((rows * G + 255) / 256);
+  const size_t stage = (size_t)2 * (256 / G) * W * 4;
+  if (stage <= 40 * 1024) lof_k_sir_time<G, true><<<grid, 256, stage, st>>>(in, out, d_stats, rows, C, W, T, eta);
+  else lof_k_sir_time<G, false><<<grid, 256, 0, st>>>(in, out, d_stats, rows, C, W, T, eta);
+}
+
+extern "C" int lof_sir_noalloc(uint32_t* d_flags, lof_stream_stats* d_stats, uint32_t n_streams, uint32_t n_channels,
+                               uint32_t n_time, float eta, uint32_t directions, int device, void* cuda_stream) {
+  if (!d_flags || !d_stats) return LOF_E_NULL;
+  if (((uintptr_t)d_flags & 15) || ((uintptr_t)d_stats & 7)) return LOF_E_ALIGN;
+  if (n_streams == 0 || n_channels == 0 || n_time == 0 || n_channels > 256) return LOF_E_PARAM;
+  if (!(eta >= 0.f && eta <= 1.f)) return LOF_E_PARAM;                  // also rejects NaN
+  if (directions == 0 || (directions & ~(uint32_t)(LOF_DIR_FREQ | LOF_DIR_TIME))) return LOF_E_PARAM;
+  if (device < 0 || device >= LOF_NOALLOC_MAX_DEVICES) return LOF_E_PARAM;
+  const uint32_t S = n_streams, C = n_channels, T = n_time, W = (T + 31) / 32;
+  const uint64_t words = (uint64_t)S * C * W;
+  if (words > (uint64_t)LOF_NOALLOC_MAX_WORDS) return LOF_E_SIZE;
+  if (!(eta > 0.f)) return LOF_OK;                                      // the operator is the identity
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LOF_CUDA(cudaSetDevice(device));
+  uint32_t* scratch = nullptr;
+  const int rc = noalloc_scratch(device, &scratch);
+  if (rc) return rc;
+  uint32_t* cur = d_flags;
+  uint32_t* other = scratch;
+  if (directions & LOF_DIR_FREQ) {
+    uint32_t m_min = 1;                                  // shortest run that grows at all
+    while (m_min <= C && (uint32_t)std::floor((double)eta * (double)m_min) == 0) ++m_min;
+    const uint64_t n_cols = (uint64_t)S * W;
+    const unsigned g128 = (unsigned)((n_cols + 127) / 128);
+    if (C == 64) lof_k_sir_freq_reg<64><<<g128, 128, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
+    else if (C == 32) lof_k_sir_freq_reg<32><<<g128, 128, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
+    else if (C == 16) lof_k_sir_freq_reg<16><<<g128, 128, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
+    else lof_k_sir_freq<<<(unsigned)((n_cols + 255) / 256), 256, 0, st>>>(cur, other, d_stats, n_cols, C, W, eta, m_min);
+    uint32_t* t = cur; cur = other; other = t;
+  }
+  if (directions & LOF_DIR_TIME) {
+    const uint64_t rows = (uint64_t)S * C;
+    uint32_t G = 1;
+    while (G < 32 && G * 8 < W) G <<= 1;                  // about eight words per lane
+    switch (G) {
+      case 1: noalloc_sir_time<1>(cur, other, d_stats, rows, C, W, T, eta, st); break;
+      case 2: noalloc_sir_time<2>(cur, other, d_stats, rows, C, W, T, eta, st); break;
+      case 4: noalloc_sir_time<4>(cur, other, d_stats, rows, C, W, T, eta, st); break;
+      case 8: noalloc_sir_time<8>(cur, other, d_stats, rows, C, W, T, eta, st); break;
+      case 16: noalloc_sir_time<16>(cur, other, d_stats, rows, C, W, T, eta, st); break;
+      default: noalloc_sir_time<32>(cur, other, d_stats, rows, C, W, T, eta, st); break;
+    }
+    uint32_t* t = cur; cur = other; other = t;
+  }
+  LOF_CUDA(cudaGetLastError());
+  if (cur != d_flags) LOF_CUDA(cudaMemcpyAsync(d_flags, cur, words * 4, cudaMemcpyDeviceToDevice, st));
   return LOF_OK;
 }

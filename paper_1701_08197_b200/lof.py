@@ -14,13 +14,14 @@ LIB_PATH = os.environ.get("LOF_LIB_PATH") or os.path.join(_DIR, "liblof.so")   #
 DIR_FREQ, DIR_TIME = 1, 2
 STATS_PLAIN, STATS_MAD = 0, 1
 MAX_LEVELS = 11
-E_NULL, E_PARAM, E_ALIGN, E_STATE, E_CUDA = -1, -2, -3, -4, -5
+E_NULL, E_PARAM, E_ALIGN, E_STATE, E_CUDA, E_SIZE = -1, -2, -3, -4, -5, -6
+NOALLOC_MAX_WORDS = 2 * 1024 * 1024      # include/lof.h LOF_NOALLOC_MAX_WORDS
 PATH_NONE, PATH_FUSED, PATH_LONGROW_SEG, PATH_LONGROW_COOP, PATH_GENERIC = 0, 1, 2, 3, 4
 
 EXPORTS = ["lof_create", "lof_destroy", "lof_flag_block", "lof_flag_block_ci16", "lof_flag_block_integrated",
            "lof_integrated_vectors", "lof_history_update",
            "lof_reset", "lof_row_sums", "lof_history_export", "lof_flag_block_host", "lof_factor_table",
-           "lof_launch_count", "lof_set_path", "lof_path_used", "lof_set_group", "lof_fused_counters", "lof_fused_cycles", "lof_strerror", "lof_last_cuda_error"]
+           "lof_launch_count", "lof_set_path", "lof_path_used", "lof_set_group", "lof_fused_counters", "lof_fused_cycles", "lof_sir_noalloc", "lof_strerror", "lof_last_cuda_error"]
 
 
 class Params(C.Structure):
@@ -61,7 +62,7 @@ def lib():
                      "lof_flag_block_integrated", "lof_integrated_vectors",
                      "lof_history_update", "lof_reset", "lof_row_sums", "lof_history_export",
                      "lof_flag_block_host", "lof_factor_table", "lof_set_path", "lof_path_used", "lof_set_group",
-                     "lof_fused_counters", "lof_fused_cycles"):
+                     "lof_fused_counters", "lof_fused_cycles", "lof_sir_noalloc"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -217,6 +218,16 @@ class Flagger:
         out = (C.c_uint64 * 4)()
         _check(lib().lof_fused_counters(self.h, out, C.c_int(1 if reset else 0)))
         return [int(v) for v in out]
+
+
+def sir_noalloc(flags, stats, n_time, eta, directions=3, stream=None):
+    """lof_sir_noalloc (include/lof.h): the SIR operator in place on a packed mask, no context, no allocation.
+    flags: int32/uint32 [S][C][W] CUDA tensor; stats: uint8 [S][32] CUDA tensor (n_flagged grows)."""
+    S, Cn, W = flags.shape
+    assert W == (n_time + 31) // 32 and flags.is_contiguous() and stats.is_contiguous()
+    _check(lib().lof_sir_noalloc(_ptr(flags), _ptr(stats), C.c_uint32(S), C.c_uint32(Cn), C.c_uint32(n_time),
+                                 C.c_float(eta), C.c_uint32(directions), C.c_int(flags.device.index),
+                                 _stream(stream)))
 
 
 def stats_to_numpy(stats):
