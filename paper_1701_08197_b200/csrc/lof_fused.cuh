@@ -90,38 +90,47 @@ enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS,
 // gives the last bin.  Groups of 32 bins are summed by warps (one bin per lane: no bank conflicts), warp 0
 // scans the group sums and then the 32 bins of the group it lands in.
 template <int NB>
-__device__ void lof_find_bin(const uint32_t* hist, uint32_t rank, uint32_t* part /*>= NB/32*/, uint32_t* ctl) {
-  constexpr int NG = NB / 32, PERL = NG / 32;
-  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, nw = blockDim.x >> 5;
+__device__ __forceinline__ void lof_find_bin_sums(const uint32_t* hist, uint32_t* part /*>= NB/32*/) {
+  constexpr int NG = NB / 32;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
   for (int g = w; g < NG; g += nw) {
     const uint32_t s = __reduce_add_sync(0xffffffffu, hist[g * 32 + lane]);
     if (lane == 0) part[g] = s;
   }
+}
+// the scan over the group sums and then over the 32 bins of the group that holds `rank`; one warp (all 32 lanes)
+template <int NB>
+__device__ __forceinline__ void lof_find_bin_scan(const uint32_t* hist, uint32_t rank, const uint32_t* part, uint32_t* ctl) {
+  constexpr int NG = NB / 32, PERL = NG / 32;
+  const int lane = threadIdx.x & 31;
+  uint32_t p[PERL], s = 0;
+#pragma unroll
+  for (int j = 0; j < PERL; ++j) { p[j] = part[lane * PERL + j]; s += p[j]; }
+  uint32_t inc = s;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+  const uint32_t exc = inc - s;
+  const bool mine = (rank >= exc && rank < inc) || (lane == 31 && rank >= inc);
+  uint32_t acc = exc; int j = 0;
+#pragma unroll
+  for (int jj = 0; jj < PERL - 1; ++jj) { if (j == jj && acc + p[jj] <= rank) { acc += p[jj]; j = jj + 1; } }
+  const int src = __ffs(__ballot_sync(0xffffffffu, mine)) - 1;
+  const int g = __shfl_sync(0xffffffffu, lane * PERL + j, src);
+  acc = __shfl_sync(0xffffffffu, acc, src);
+  const uint32_t hv = hist[g * 32 + lane];
+  uint32_t binc = hv;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, binc, o); if (lane >= o) binc += v; }
+  const uint32_t hit = __ballot_sync(0xffffffffu, acc + binc > rank);
+  const int bl = hit ? __ffs(hit) - 1 : 31;
+  const uint32_t before = acc + __shfl_sync(0xffffffffu, binc - hv, bl);
+  if (lane == 0) { ctl[CT_BIN] = g * 32 + bl; ctl[CT_BEFORE] = before; }
+}
+template <int NB>
+__device__ void lof_find_bin(const uint32_t* hist, uint32_t rank, uint32_t* part /*>= NB/32*/, uint32_t* ctl) {
+  lof_find_bin_sums<NB>(hist, part);
   __syncthreads();
-  if (tid < 32) {
-    uint32_t p[PERL], s = 0;
-#pragma unroll
-    for (int j = 0; j < PERL; ++j) { p[j] = part[lane * PERL + j]; s += p[j]; }
-    uint32_t inc = s;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-    const uint32_t exc = inc - s;
-    const bool mine = (rank >= exc && rank < inc) || (lane == 31 && rank >= inc);
-    uint32_t acc = exc; int j = 0;
-#pragma unroll
-    for (int jj = 0; jj < PERL - 1; ++jj) { if (j == jj && acc + p[jj] <= rank) { acc += p[jj]; j = jj + 1; } }
-    const int src = __ffs(__ballot_sync(0xffffffffu, mine)) - 1;
-    const int g = __shfl_sync(0xffffffffu, lane * PERL + j, src);
-    acc = __shfl_sync(0xffffffffu, acc, src);
-    const uint32_t hv = hist[g * 32 + lane];
-    uint32_t binc = hv;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, binc, o); if (lane >= o) binc += v; }
-    const uint32_t hit = __ballot_sync(0xffffffffu, acc + binc > rank);
-    const int bl = hit ? __ffs(hit) - 1 : 31;
-    const uint32_t before = acc + __shfl_sync(0xffffffffu, binc - hv, bl);
-    if (lane == 0) { ctl[CT_BIN] = g * 32 + bl; ctl[CT_BEFORE] = before; }
-  }
+  if (threadIdx.x < 32) lof_find_bin_scan<NB>(hist, rank, part, ctl);
   __syncthreads();
 }
 
@@ -260,11 +269,15 @@ template <int C, int L>
 __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& prm, const LofStatPlan& pl,
                                       lof_stream_stats* out, float& median_out, unsigned long long* diag) {
   using Cfg = LofFusedCfg<C, L>;
-  constexpr int N = Cfg::N, NT = Cfg::NT;
-  const int tid = threadIdx.x, lane = tid & 31;
+  constexpr int N = Cfg::N, NT = Cfg::NT, NW = NT / 32;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   uint32_t* part = sm.part;
   const float4* x4 = reinterpret_cast<const float4*>(sm.xs);
-  if (tid < 32) {
+  // The steps below are latency chains between block barriers (12 k cycles per stream when each had its own): they
+  // are paired so that one barrier serves two of them.  Here: the row partials added by the last warp (which also
+  // resets the work counters of the passes that follow: nothing reads them inside this function), and the group
+  // sums of the histogram for the bin search by every warp.
+  if (warp == NW - 1) {
     double a = 0.0, q = 0.0;
 #pragma unroll
     for (int c = lane; c < C; c += 32) { a += sm.rowpart[2 * c]; q += sm.rowpart[2 * c + 1]; }
@@ -272,8 +285,10 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
     if (lane == 0) {
       sm.red[0] = a; sm.red[1] = q;
       sm.ctl[CT_NCAND] = 0; sm.ctl[CT_BAD] = 0; sm.ctl[CT_FOUND] = 0;
+      sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_ROW] = 0; sm.ctl[CT_COLGRP] = 0; sm.ctl[CT_SROW] = 0;
     }
   }
+  lof_find_bin_sums<LOF_F_NBINS>(sm.hist, part);
   __syncthreads();
   double da = sm.red[0], dq = sm.red[1];
   uint32_t n_bad = 0;
@@ -294,9 +309,10 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
   const uint32_t rank = N / 2;
   float median = 0.f;
   int how = 3;
-  bool dp_done = false;
+  bool dp_done = false, fast = false;
   if (n_bad == 0) {
-    lof_find_bin<LOF_F_NBINS>(sm.hist, rank, part, sm.ctl);
+    if (tid < 32) lof_find_bin_scan<LOF_F_NBINS>(sm.hist, rank, part, sm.ctl);
+    __syncthreads();
     LOF_PROF_T(tb);
     const uint32_t bin = sm.ctl[CT_BIN], before = sm.ctl[CT_BEFORE];
     const uint32_t n_b = sm.hist[bin];
@@ -307,12 +323,17 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
       // does the fp64 end of mean and stddev meanwhile (a long dependent chain that would otherwise sit
       // on one thread between two barriers).
       if (tid >= NT - 32) {
+        double sd = 0.0;
         if (lane == 0) {
           const double n = (double)N;
           double var = (dq - da * da / n) / n;
           if (!(var > 0.0)) var = 0.0;
-          sm.red[2] = (double)pl.K + da / n; sm.red[3] = sqrt(var);
+          sd = sqrt(var);
+          sm.red[2] = (double)pl.K + da / n; sm.red[3] = sd;
         }
+        // ... and the part of each threshold that does not need the median: stddev * factor_I
+        sd = __shfl_sync(0xffffffffu, sd, 0);
+        if ((uint32_t)lane < prm.n_levels) sm.red[8 + lane] = sd * prm.factor[lane];
       } else {
         const float inv = 1.0f / pl.scale;
         const float v0 = ((float)bin - 0.5f - pl.off) * inv, v1 = ((float)bin + 1.0f - pl.off) * inv;
@@ -366,20 +387,24 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
       if (nc != n_b) ok = false;                         // bounds too tight (cannot happen): stay exact anyway
       else if (nc <= 256) {
         how = 0;
-        // a warp per candidate i, its lanes over the other candidates: less = #{j : c_j < c_i, or equal and j < i}
-        for (uint32_t i = (uint32_t)(tid >> 5); i < nc; i += NT / 32) {
-          const float v = sm.cand[i];
+        // a thread per candidate i (there are a few dozen) over all candidates, independent broadcast loads:
+        // less = #{j : c_j < c_i, or equal and j < i}.  The histogram is zeroed for the next stream under the
+        // same barrier (its last read was hist[bin] above).
+        if ((uint32_t)tid < nc) {
+          const float v = sm.cand[tid];
           uint32_t less = 0;
-          for (uint32_t j0 = 0; j0 < nc; j0 += 32) {
-            const uint32_t j = j0 + (uint32_t)lane;
-            const float w = j < nc ? sm.cand[j] : INFINITY;
-            less += __popc(__ballot_sync(0xffffffffu, j < nc && (w < v || (w == v && j < i))));
+#pragma unroll 8
+          for (uint32_t j = 0; j < nc; ++j) {
+            const float w = sm.cand[j];
+            less += (w < v || (w == v && j < (uint32_t)tid)) ? 1u : 0u;
           }
-          if (lane == 0 && less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
+          if (less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
         }
+        for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
         __syncthreads();
         ok = sm.ctl[CT_FOUND] != 0;
         median = __uint_as_float(sm.ctl[CT_MEDBITS]);
+        fast = ok;
       } else {
         how = 1;
         median = lof_radix_select_smem<NT>(sm.cand, (int)nc, want, sm.hist, part, sm.ctl);
@@ -388,6 +413,29 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
     if (!ok) { how = 2; median = lof_radix_select_smem<NT>(sm.xs, N, rank, sm.hist, part, sm.ctl); }
   }
   LOF_PROF_T(tc);
+  if (fast) {
+    // the usual case: every warp forms the thresholds and early-exit levels itself (same inputs, same bits) and
+    // goes on to the frequency pass without another block barrier
+    if ((uint32_t)lane < prm.n_levels)
+      sm.thr[lane] = (float)((double)median + sm.red[8 + lane] * prm.sensitivity);
+    __syncwarp();
+    if ((uint32_t)lane < prm.n_levels) {
+      sm.thr[16 + lane] = lof_dead_level_f(sm.thr, lane, prm.n_lev_f);
+      sm.thr[32 + lane] = lof_dead_level_f(sm.thr, lane, prm.n_lev_t);
+    }
+    if (lane == 0) sm.thr[48] = LOF_BELOW_MARK;
+    if (tid == 0) {
+      lof_stream_stats o;
+      o.median = median; o.n_nonfinite = 0; o.mean = sm.red[2]; o.stddev = sm.red[3];
+      o.n_flagged = 0;
+      *out = o;
+      atomicAdd(&diag[0], 1ull);
+    }
+    __syncwarp();
+    LOF_PROF_T(te);
+    median_out = median;
+    return 0;
+  }
   for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
   if (tid < 32) {
     double mean, stddev;
