@@ -387,18 +387,24 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
       if (nc != n_b) ok = false;                         // bounds too tight (cannot happen): stay exact anyway
       else if (nc <= 256) {
         how = 0;
-        // a thread per candidate i (there are a few dozen) over all candidates, independent broadcast loads:
-        // less = #{j : c_j < c_i, or equal and j < i}.  The histogram is zeroed for the next stream under the
-        // same barrier (its last read was hist[bin] above).
-        if ((uint32_t)tid < nc) {
-          const float v = sm.cand[tid];
+        // G threads per candidate i (there are a few dozen candidates; G = 8 or 4 then), each over every G-th
+        // candidate j: less = #{j : c_j < c_i, or equal and j < i}, added over the group by shuffles.  The
+        // histogram is zeroed for the next stream under the same barrier (its last read was hist[bin] above).
+        {
+          uint32_t lg = 0;
+          while (lg < 5 && (nc << (lg + 1)) <= (uint32_t)NT) ++lg;
+          const uint32_t G = 1u << lg, i = (uint32_t)tid >> lg, sub = (uint32_t)tid & (G - 1);
+          const float v = sm.cand[i < nc ? i : 0];
           uint32_t less = 0;
-#pragma unroll 8
-          for (uint32_t j = 0; j < nc; ++j) {
-            const float w = sm.cand[j];
-            less += (w < v || (w == v && j < (uint32_t)tid)) ? 1u : 0u;
+          if (i < nc) {
+#pragma unroll 4
+            for (uint32_t j = sub; j < nc; j += G) {
+              const float w = sm.cand[j];
+              less += (w < v || (w == v && j < i)) ? 1u : 0u;
+            }
           }
-          if (less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
+          for (uint32_t o = G >> 1; o > 0; o >>= 1) less += __shfl_xor_sync(0xffffffffu, less, o);
+          if (i < nc && sub == 0 && less == want) { sm.ctl[CT_MEDBITS] = __float_as_uint(v); sm.ctl[CT_FOUND] = 1; }
         }
         for (int b = tid; b < LOF_F_NBINS; b += NT) sm.hist[b] = 0;
         __syncthreads();
@@ -416,12 +422,23 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
   if (fast) {
     // the usual case: every warp forms the thresholds and early-exit levels itself (same inputs, same bits) and
     // goes on to the frequency pass without another block barrier
-    if ((uint32_t)lane < prm.n_levels)
-      sm.thr[lane] = (float)((double)median + sm.red[8 + lane] * prm.sensitivity);
-    __syncwarp();
+    float t = INFINITY;
     if ((uint32_t)lane < prm.n_levels) {
-      sm.thr[16 + lane] = lof_dead_level_f(sm.thr, lane, prm.n_lev_f);
-      sm.thr[32 + lane] = lof_dead_level_f(sm.thr, lane, prm.n_lev_t);
+      t = (float)((double)median + sm.red[8 + lane] * prm.sensitivity);
+      sm.thr[lane] = t;
+    }
+    // early-exit levels (lof_dead_level_f: the minimum over the later thresholds of the run) by suffix minima
+    // over the lanes
+    float mf = (uint32_t)lane < prm.n_lev_f ? t : INFINITY, mt = (uint32_t)lane < prm.n_lev_t ? t : INFINITY;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+      const float a = __shfl_down_sync(0xffffffffu, mf, o), b = __shfl_down_sync(0xffffffffu, mt, o);
+      if (lane + o < 32) { mf = fminf(mf, a); mt = fminf(mt, b); }
+    }
+    mf = __shfl_down_sync(0xffffffffu, mf, 1); mt = __shfl_down_sync(0xffffffffu, mt, 1);
+    if ((uint32_t)lane < prm.n_levels) {
+      sm.thr[16 + lane] = (uint32_t)lane + 1 >= prm.n_lev_f ? 3.0e38f : (mf > 0.f ? mf * (1.0f - 3e-6f) : -1.0e34f);
+      sm.thr[32 + lane] = (uint32_t)lane + 1 >= prm.n_lev_t ? 3.0e38f : (mt > 0.f ? mt * (1.0f - 3e-6f) : -1.0e34f);
     }
     if (lane == 0) sm.thr[48] = LOF_BELOW_MARK;
     if (tid == 0) {
