@@ -193,7 +193,8 @@ __device__ __forceinline__ uint32_t lof_stat_bin(float x, const LofStatPlan& pl)
 // their median and interquartile range; the plan centres the histogram on the mean of the warp medians with
 // a half-width of 2.5 mean interquartile ranges.  Rank statistics, because RFI of 100 sigma in a few per cent
 // of the samples inflates a plain standard deviation tenfold and the bins with it.  Any K and any range give
-// the same exact results; they only decide how fast the median is found.  Contains __syncthreads.
+// the same exact results; they only decide how fast the median is found.  Contains one __syncthreads; call it
+// right after a block barrier, and put another one before anything else writes `red`.
 template <int NT>
 __device__ __forceinline__ LofStatPlan lof_stat_plan(float v, float* red /* >= 2*NT/32 floats */) {
   constexpr int NW = NT / 32;
@@ -210,14 +211,14 @@ __device__ __forceinline__ LofStatPlan lof_stat_plan(float v, float* red /* >= 2
   }
   const float q1 = __shfl_sync(0xffffffffu, v, 8), m0 = __shfl_sync(0xffffffffu, v, 15),
               m1 = __shfl_sync(0xffffffffu, v, 16), q3 = __shfl_sync(0xffffffffu, v, 24);
-  __syncthreads();
+  // (no barrier here: every caller comes from one, and nothing writes `red` between that and this point)
   if (lane == 0) { red[w] = 0.5f * (m0 + m1); red[NW + w] = q3 - q1; }
   __syncthreads();
   float K = 0.f, iqr = 0.f;
 #pragma unroll
   for (int i = 0; i < NW; ++i) { K += red[i]; iqr += red[NW + i]; }
   K *= 1.0f / NW; iqr *= 1.0f / NW;
-  __syncthreads();
+  // (none here either: the next writer of `red`, lof_stat_finalize, is behind the callers' next barrier)
   float h = 2.5f * iqr;                                   // Gaussian: +-3.4 sigma; exponential: 96 % of the samples
   if (!(h > 0.f) || !lof_finite(h)) h = fmaxf(fabsf(K) * 1e-6f, 1e-30f);
   LofStatPlan pl;
