@@ -541,24 +541,27 @@ static int integrated_prepare(lof_ctx* c) {
 
 // One SumThreshold run over S vectors of n samples: the single-CTA kernel for short vectors, an inner context
 // (statistics kernels + row kernels of the long-row path) for long ones.
+// vectors of n samples take the warp-per-vector kernel (the row core runs windows of up to 512 samples)
+static bool integrated_warp_path(const lof_ctx* c, uint32_t n) {
+  return n <= 1024 && (c->prm.max_window < 1024 || n < 1024);
+}
 static int integrated_run(lof_ctx* c, lof_ctx* inner, const float* d_vec, uint32_t n, uint32_t* d_mask,
-                          lof_stream_stats* d_stats_out, cudaStream_t st) {
+                          lof_stream_stats* d_stats_out, cudaStream_t st, LofVecFuse fz = LofVecFuse{}) {
   const uint32_t S = c->prm.n_streams;
-  if (n <= 1024 && (c->prm.max_window < 1024 || n < 1024)) {     // (the row core runs windows of up to 512 samples)
+  if (integrated_warp_path(c, n)) {
     // a warp per vector (lof_k_vec_warp), L = samples per lane
     LofKParams kp = c->kp;
     const uint32_t mw = c->prm.max_window < n ? c->prm.max_window : n;
     uint32_t n_lev = 0;
     while ((1u << n_lev) <= mw) ++n_lev;
     const unsigned grid = (S + 7) / 8;
-    if (n <= 64) lof_k_vec_warp<2><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, inner->d_stats);
-    else if (n <= 256) lof_k_vec_warp<8><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, inner->d_stats);
-    else if (n <= 768) lof_k_vec_warp<24><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, inner->d_stats);
-    else lof_k_vec_warp<32><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, inner->d_stats);
+    lof_stream_stats* so = d_stats_out ? d_stats_out : inner->d_stats;     // straight into the caller's array
+    if (n <= 64) lof_k_vec_warp<2><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, so, fz);
+    else if (n <= 256) lof_k_vec_warp<8><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, so, fz);
+    else if (n <= 768) lof_k_vec_warp<24><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, so, fz);
+    else lof_k_vec_warp<32><<<grid, 256, 0, st>>>(d_vec, n, S, kp, n_lev, d_mask, so, fz);
     c->launches += 1;
     LOF_CUDA(cudaGetLastError());
-    if (d_stats_out)
-      LOF_CUDA(cudaMemcpyAsync(d_stats_out, inner->d_stats, (size_t)S * sizeof(lof_stream_stats), cudaMemcpyDeviceToDevice, st));
     return LOF_OK;
   }
   if (n <= LOF_VEC_MAX) {
@@ -600,28 +603,46 @@ extern "C" int lof_flag_block_integrated(lof_ctx* c, const float* d_power, uint3
   lof_k_integ_sums<<<dim3(c->ig_tiles, S), LOF_IG_THREADS, 0, st>>>(d_power, c->d_ig_rowpart, c->d_ig_colsum, C, T,
                                                                     c->ig_tiles);
   const uint64_t rows = (uint64_t)S * C;
-  lof_k_integ_spectrum<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(c->d_ig_rowpart, c->d_ig_spec, rows, c->ig_tiles, T);
-  c->launches += 2;
+  c->launches += 1;
+  // the spectrum a[s][c]: formed inside the spectrum run's kernel when that is the warp-per-vector one
+  const bool fuse_f = (c->prm.directions & LOF_DIR_FREQ) && integrated_warp_path(c, C);
+  const bool fuse_t = (c->prm.directions & LOF_DIR_TIME) && integrated_warp_path(c, T);
+  if (!fuse_f) {
+    lof_k_integ_spectrum<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(c->d_ig_rowpart, c->d_ig_spec, rows, c->ig_tiles, T);
+    c->launches += 1;
+  }
   // frequency first: one SumThreshold run over the time-integrated spectrum of every stream
   if (c->prm.directions & LOF_DIR_FREQ) {
-    rc = integrated_run(c, c->ig_freq, c->d_ig_spec, C, c->d_ig_cmask, d_stats_freq, st);
+    LofVecFuse fz{};
+    if (fuse_f) { fz.rowpart = c->d_ig_rowpart; fz.n_tiles = c->ig_tiles; fz.T = T; fz.spec_out = c->d_ig_spec; }
+    rc = integrated_run(c, c->ig_freq, c->d_ig_spec, C, c->d_ig_cmask, d_stats_freq, st, fz);
     if (rc) return rc;
   } else {
     LOF_CUDA(cudaMemsetAsync(c->d_ig_cmask, 0, (size_t)S * CW * 4, st));
     if (d_stats_freq) LOF_CUDA(cudaMemsetAsync(d_stats_freq, 0, (size_t)S * sizeof(lof_stream_stats), st));
   }
   // then time: the series integrated over the channels that are left
-  lof_k_integ_series<<<dim3((T + 256 * LOF_IG_SER - 1) / (256 * LOF_IG_SER), S), 256, 0, st>>>(d_power, c->d_ig_colsum, c->d_ig_cmask,
-                                                                c->d_ig_series, C, T);
+  if (!fuse_t) {
+    lof_k_integ_series<<<dim3((T + 256 * LOF_IG_SER - 1) / (256 * LOF_IG_SER), S), 256, 0, st>>>(d_power, c->d_ig_colsum, c->d_ig_cmask,
+                                                                  c->d_ig_series, C, T);
+    c->launches += 1;
+  }
   if (c->prm.directions & LOF_DIR_TIME) {
-    rc = integrated_run(c, c->ig_time, c->d_ig_series, T, c->d_ig_tmask, d_stats_time, st);
+    LofVecFuse fz{};
+    if (fuse_t) {                                          // the series run forms the series and writes the block's flags
+      fz.cmask = c->d_ig_cmask; fz.flags = d_flags; fz.C = C;
+      fz.block = d_power; fz.colsum = c->d_ig_colsum; fz.series_out = c->d_ig_series;
+    }
+    rc = integrated_run(c, c->ig_time, c->d_ig_series, T, c->d_ig_tmask, d_stats_time, st, fz);
     if (rc) return rc;
   } else {
     LOF_CUDA(cudaMemsetAsync(c->d_ig_tmask, 0, (size_t)S * W * 4, st));
     if (d_stats_time) LOF_CUDA(cudaMemsetAsync(d_stats_time, 0, (size_t)S * sizeof(lof_stream_stats), st));
   }
-  lof_k_integ_combine<<<S, 256, 0, st>>>(c->d_ig_cmask, c->d_ig_tmask, d_flags, C, W, T);
-  c->launches += 2;
+  if (!fuse_t) {
+    lof_k_integ_combine<<<S, 256, 0, st>>>(c->d_ig_cmask, c->d_ig_tmask, d_flags, C, W, T);
+    c->launches += 1;
+  }
   LOF_CUDA(cudaGetLastError());
   c->block_pending = false;                               // no row sums of this block: the history flagger needs lof_flag_block
   return LOF_OK;

@@ -240,10 +240,21 @@ lof_k_vec_flag(const float* __restrict__ vec, uint32_t n, LofKParams prm, uint32
 // samples [l*L, l*L + L) (beyond n: -inf, which no window survives); mean / stddev by fp64 shuffle trees in a
 // fixed order, the exact median by a bitwise radix select on the monotone keys (32 votes), then the row core of
 // lof_core.cuh (the one the time run of the fused kernel uses), and the mask words gathered by shuffles.
+// Two neighbours of the integrated mode can ride on this kernel instead of being launches of their own
+// (LofVecFuse, all pointers optional): the spectrum a[s][c] = (float)(sum over tiles / T) formed from the row
+// partials when the vector is loaded (what lof_k_integ_spectrum does), and the final flags[s][c][w] written from
+// the mask words while they are in the warp's registers (what lof_k_integ_combine does); for the series run also
+// the series itself, b[s][t] = (column sum - sum over the flagged channels) / #unflagged, same operations in the
+// same order as lof_k_integ_series.
+struct LofVecFuse {
+  const double* rowpart; uint32_t n_tiles, T; float* spec_out;      // vec[s][i] = (float)(sum_j rowpart[(s n + i) n_tiles + j] / T)
+  const uint32_t* cmask; uint32_t* flags; uint32_t C;               // flags[s][c][w] = channel c flagged ? ones : mask word w
+  const float* block; const double* colsum; float* series_out;      // vec[s][t] = series b[s][t] from the block [S][C][n]
+};
 template <int L>
 __global__ void __launch_bounds__(256)
 lof_k_vec_warp(const float* __restrict__ vec, uint32_t n, uint32_t S, LofKParams prm, uint32_t n_lev,
-               uint32_t* __restrict__ mask, lof_stream_stats* __restrict__ stats) {
+               uint32_t* __restrict__ mask, lof_stream_stats* __restrict__ stats, LofVecFuse fz) {
   __shared__ float wthr[8][32];                           // per warp: [0..16) thresholds, [16..32) early-exit levels
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t s = blockIdx.x * 8u + (uint32_t)warp;
@@ -253,8 +264,48 @@ lof_k_vec_warp(const float* __restrict__ vec, uint32_t n, uint32_t S, LofKParams
   const uint32_t nv = i0 >= n ? 0u : (n - i0 >= (uint32_t)L ? (uint32_t)L : n - i0);      // valid samples of this lane
   const uint32_t valid = nv >= 32 ? 0xFFFFFFFFu : ((1u << nv) - 1u);
   float x[L];
+  if (fz.rowpart) {
 #pragma unroll
-  for (int j = 0; j < L; ++j) x[j] = (uint32_t)j < nv ? __ldg(v + i0 + j) : -INFINITY;
+    for (int j = 0; j < L; ++j) {
+      x[j] = -INFINITY;
+      if ((uint32_t)j < nv) {
+        const uint64_t r = (uint64_t)s * n + i0 + j;
+        double a = 0.0;
+        for (uint32_t k = 0; k < fz.n_tiles; ++k) a += fz.rowpart[r * fz.n_tiles + k];
+        x[j] = (float)(a / (double)fz.T);
+        fz.spec_out[r] = x[j];
+      }
+    }
+  } else if (fz.colsum) {
+    const uint32_t CW = (fz.C + 31) / 32;
+    const uint32_t cmw = (uint32_t)lane < CW ? fz.cmask[(size_t)s * CW + lane] : 0u;
+    const uint32_t n_unf = fz.C - __reduce_add_sync(0xffffffffu, (uint32_t)__popc(cmw));
+    const float* xs = fz.block + (size_t)s * fz.C * n;
+    double fs[L];
+#pragma unroll
+    for (int j = 0; j < L; ++j) fs[j] = 0.0;
+    for (uint32_t w = 0; w < CW; ++w) {
+      uint32_t m = __shfl_sync(0xffffffffu, cmw, (int)w);   // the same for every lane: uniform loops
+      while (m) {
+        const uint32_t c = w * 32u + (uint32_t)__ffs((int)m) - 1u;
+        m &= m - 1u;
+#pragma unroll
+        for (int j = 0; j < L; ++j) if ((uint32_t)j < nv) fs[j] += (double)__ldg(xs + (size_t)c * n + i0 + j);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < L; ++j) {
+      x[j] = -INFINITY;
+      if ((uint32_t)j < nv) {
+        const size_t g = (size_t)s * n + i0 + j;
+        x[j] = n_unf ? (float)((fz.colsum[g] - fs[j]) / (double)n_unf) : 0.f;
+        fz.series_out[g] = x[j];
+      }
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < L; ++j) x[j] = (uint32_t)j < nv ? __ldg(v + i0 + j) : -INFINITY;
+  }
   uint32_t bad = 0;
   double a = 0.0;
 #pragma unroll
@@ -269,15 +320,25 @@ lof_k_vec_warp(const float* __restrict__ vec, uint32_t n, uint32_t S, LofKParams
   const double stddev = sqrt(__shfl_sync(0xffffffffu, q, 0) / (double)n);
   // exact median: the key of rank floor(n/2), one bit per vote from the top
   uint32_t cand = valid, rank = n / 2, prefix = 0;
+  uint32_t key[L];
+#pragma unroll
+  for (int j = 0; j < L; ++j) key[j] = lof_key(x[j]);
+  uint32_t left = n;                                       // candidates left (warp-uniform)
 #pragma unroll 1
-  for (int b = 31; b >= 0; --b) {
+  for (int b = 31; b >= 0 && left > 1; --b) {
     uint32_t ones = 0;
 #pragma unroll
-    for (int j = 0; j < L; ++j) ones |= ((lof_key(x[j]) >> b) & 1u) << j;
+    for (int j = 0; j < L; ++j) ones |= ((key[j] >> b) & 1u) << j;
     const uint32_t zeros = cand & ~ones;
     const uint32_t c0 = __reduce_add_sync(0xffffffffu, (uint32_t)__popc(zeros));
-    if (rank < c0) cand = zeros;
-    else { rank -= c0; cand &= ones; prefix |= 1u << b; }
+    if (rank < c0) { cand = zeros; left = c0; }
+    else { rank -= c0; cand &= ones; left -= c0; prefix |= 1u << b; }
+  }
+  if (left == 1) {                                         // a single candidate: its key is the answer (usually after
+    uint32_t k = 0;                                        // about 20 of the 32 votes)
+#pragma unroll
+    for (int j = 0; j < L; ++j) if ((cand >> j) & 1u) k = key[j];
+    prefix = __shfl_sync(0xffffffffu, k, __ffs((int)__ballot_sync(0xffffffffu, cand != 0u)) - 1);
   }
   const float median = lof_unkey(prefix);
   if ((uint32_t)lane < n_lev) {
@@ -311,6 +372,23 @@ lof_k_vec_warp(const float* __restrict__ vec, uint32_t n, uint32_t S, LofKParams
       if (sh < 32) word |= sh >= 0 ? (w << sh) : (w >> (-sh));
     }
     if ((uint32_t)lane < W) mask[(size_t)s * W + lane] = word;
+    if (fz.flags) {
+      const uint32_t CW = (fz.C + 31) / 32, tot = fz.C * W;
+      const uint32_t cmw = (uint32_t)lane < CW ? fz.cmask[(size_t)s * CW + lane] : 0u;     // C <= 256: 8 words
+      const uint32_t last = (n & 31) ? ((1u << (n & 31)) - 1u) : 0xFFFFFFFFu;
+      uint32_t* fo = fz.flags + (size_t)s * tot;
+      const uint32_t d32 = 32u / W, r32 = 32u - d32 * W;  // i -> i + 32: c += d32, w += r32 (with carry)
+      uint32_t cq = (uint32_t)lane / W, w = (uint32_t)lane - cq * W;
+      for (uint32_t i0w = 0; i0w < tot; i0w += 32) {       // warp-uniform trip count: shuffles inside
+        const uint32_t i = i0w + (uint32_t)lane;
+        const uint32_t c = cq < fz.C ? cq : fz.C - 1;
+        const uint32_t cmv = __shfl_sync(0xffffffffu, cmw, (int)(c >> 5));
+        const uint32_t tv = __shfl_sync(0xffffffffu, word, (int)w);
+        if (i < tot) fo[i] = ((cmv >> (c & 31)) & 1u) ? (w == W - 1 ? last : 0xFFFFFFFFu) : tv;
+        cq += d32; w += r32;
+        if (w >= W) { w -= W; ++cq; }
+      }
+    }
   }
   const uint32_t nf = __reduce_add_sync(0xffffffffu, (uint32_t)__popc(fb));
   if (lane == 0) {
