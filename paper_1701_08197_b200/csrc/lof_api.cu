@@ -455,10 +455,10 @@ static int sir_apply(lof_ctx* c, uint32_t* d_flags, cudaStream_t st) {
     uint32_t m_min = 1;                                  // shortest run that grows at all
     while (m_min <= C && (uint32_t)std::floor((double)eta * (double)m_min) == 0) ++m_min;
     const uint64_t n_cols = (uint64_t)c->prm.n_streams * W;
-    const unsigned g128 = (unsigned)((n_cols + 127) / 128);
-    if (C == 64) lof_k_sir_freq_reg<64><<<g128, 128, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
-    else if (C == 32) lof_k_sir_freq_reg<32><<<g128, 128, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
-    else if (C == 16) lof_k_sir_freq_reg<16><<<g128, 128, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
+    const unsigned g8 = (unsigned)((n_cols + 7) / 8);          // a warp per word column
+    if (C == 64) lof_k_sir_freq_reg<64><<<g8, 256, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
+    else if (C == 32) lof_k_sir_freq_reg<32><<<g8, 256, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
+    else if (C == 16) lof_k_sir_freq_reg<16><<<g8, 256, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
     else lof_k_sir_freq<<<(unsigned)((n_cols + 255) / 256), 256, 0, st>>>(cur, other, c->d_stats, n_cols, C, W, eta, m_min);
     c->launches += 1;
     uint32_t* t = cur; cur = other; other = t;
@@ -848,10 +848,10 @@ extern "C" int lof_sir_noalloc(uint32_t* d_flags, lof_stream_stats* d_stats, uin
     uint32_t m_min = 1;                                  // shortest run that grows at all
     while (m_min <= C && (uint32_t)std::floor((double)eta * (double)m_min) == 0) ++m_min;
     const uint64_t n_cols = (uint64_t)S * W;
-    const unsigned g128 = (unsigned)((n_cols + 127) / 128);
-    if (C == 64) lof_k_sir_freq_reg<64><<<g128, 128, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
-    else if (C == 32) lof_k_sir_freq_reg<32><<<g128, 128, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
-    else if (C == 16) lof_k_sir_freq_reg<16><<<g128, 128, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
+    const unsigned g8 = (unsigned)((n_cols + 7) / 8);          // a warp per word column
+    if (C == 64) lof_k_sir_freq_reg<64><<<g8, 256, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
+    else if (C == 32) lof_k_sir_freq_reg<32><<<g8, 256, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
+    else if (C == 16) lof_k_sir_freq_reg<16><<<g8, 256, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
     else lof_k_sir_freq<<<(unsigned)((n_cols + 255) / 256), 256, 0, st>>>(cur, other, d_stats, n_cols, C, W, eta, m_min);
     uint32_t* t = cur; cur = other; other = t;
   }

@@ -179,59 +179,61 @@ __device__ __forceinline__ unsigned long long lof_sir_col_ext(unsigned long long
   return ext & ~col;
 }
 
-// Frequency direction, C = 16, 32 or 64 channels: one thread per (stream, word column) with the C words in
-// registers.  A run can only grow if it is at least m_min = ceil(1/eta) channels long: a bit-parallel screen (AND of
-// k consecutive words, k the largest power of two <= m_min, OR over c) names the time samples that may have such a
-// run; only those columns are turned into a C-bit column mask, extended with bit operations, and merged back.
+// 32 x 32 bit-matrix transpose across a warp: lane r holds row r (bit i = column i); afterwards lane i holds column
+// i (bit r = row r).  Five exchange steps (blocks of 16, 8, 4, 2, 1); its own inverse.
+__device__ __forceinline__ uint32_t lof_bit_transpose32(uint32_t x, int lane) {
+  uint32_t m = 0x0000FFFFu;
+#pragma unroll
+  for (int j = 16; j > 0; j >>= 1) {
+    const uint32_t p = __shfl_xor_sync(0xffffffffu, x, j);
+    if ((lane & j) == 0) x ^= (((x >> j) ^ p) & m) << j;
+    else x ^= ((p >> j) ^ x) & m;
+    m ^= m << (j >> 1);
+  }
+  return x;
+}
+
+// Frequency direction, C = 16, 32 or 64 channels: a WARP per (stream, word column).  Lane c loads the word of
+// channel c (and c + 32): 32 time samples each.  Two bit-matrix transposes turn them into one C-bit column mask
+// per lane = time sample; a run can only grow if it is at least m_min = ceil(1/eta) channels long, which a few
+// shifts and ANDs of the mask decide; the lanes with such a run extend theirs (lof_sir_col_ext); if any lane added
+// a bit, two more transposes bring the new bits back to the channel words.  (The first version was a thread per word
+// column with the C words in registers and a loop over the time samples with long runs: the lanes of a warp waited
+// for the one whose word lay inside a burst — 32 samples x 400 instructions — and the kernel took 150 us for the
+// 38 MB mask of config 2 x 64 subbands.)  grid.x = ceil(n_cols / 8), 256 threads.
 template <int C>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(256)
 lof_k_sir_freq_reg(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_stream_stats* __restrict__ stats,
                    uint64_t n_cols /* S*W */, uint32_t W, float eta, uint32_t m_min) {
-  const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= n_cols) return;
-  const uint64_t s = gid / W;
-  const uint32_t w = (uint32_t)(gid - s * W);
+  const int lane = threadIdx.x & 31;
+  const uint64_t gw = (uint64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (gw >= n_cols) return;                               // whole warps leave together
+  const uint64_t s = gw / W;
+  const uint32_t w = (uint32_t)(gw - s * W);
   const uint32_t* ci = in + s * C * W + w;
   uint32_t* co = out + s * C * W + w;
-  uint32_t v[C];
-#pragma unroll
-  for (int c = 0; c < C; ++c) v[c] = __ldg(ci + (size_t)c * W);
-  // screen: and_k[c] = AND of v[c .. c+k); doubling up to the largest power of two <= m_min
-  uint32_t longrun = 0;
-  if (m_min <= C) {
-    uint32_t a[C];
-#pragma unroll
-    for (int c = 0; c < C; ++c) a[c] = v[c];
+  uint32_t lo = lane < C ? __ldg(ci + (size_t)lane * W) : 0u;
+  uint32_t hi = C > 32 ? __ldg(ci + (size_t)(lane + 32) * W) : 0u;
+  const uint32_t tl = lof_bit_transpose32(lo, lane);
+  const uint32_t th = C > 32 ? lof_bit_transpose32(hi, lane) : 0u;
+  const unsigned long long col = (unsigned long long)tl | ((unsigned long long)th << 32);
+  // does this time sample's column hold a run of at least m_min channels?  r = AND of col >> 0 .. m_min-1
+  unsigned long long r = col;
+  if (m_min > (uint32_t)C) r = 0;
+  else {
     uint32_t k = 1;
-#pragma unroll
-    for (int d = 1; d < C; d <<= 1) {
-      if (2 * k <= m_min) {
-#pragma unroll
-        for (int c = 0; c < C; ++c) a[c] = (c + d < C) ? (a[c] & a[c + d]) : 0u;   // windows that leave the column: none
-        k *= 2;
-      }
-    }
-    // a[c] covers [c, c+k) with k the largest power of two <= m_min: a superset of the columns that matter
-    // (a run of k..m_min-1 channels is walked below and found not to grow)
-#pragma unroll
-    for (int c = 0; c < C; ++c) longrun |= a[c];
-    if (k > (uint32_t)C) longrun = 0;
+    while (2 * k <= m_min) { r &= r >> k; k *= 2; }
+    if (m_min > k) r &= r >> (m_min - k);
   }
-  uint32_t added = 0;
-  while (longrun) {
-    const uint32_t b = (uint32_t)__ffs((int)longrun) - 1u;
-    longrun &= longrun - 1u;
-    unsigned long long col = 0;
-#pragma unroll
-    for (int c = 0; c < C; ++c) col |= (unsigned long long)((v[c] >> b) & 1u) << c;
-    const unsigned long long nw = lof_sir_col_ext<C>(col, eta);
-    added += (uint32_t)__popcll(nw);
-#pragma unroll
-    for (int c = 0; c < C; ++c) v[c] |= (uint32_t)((nw >> c) & 1ull) << b;
+  const unsigned long long nw = r ? lof_sir_col_ext<C>(col, eta) : 0ull;
+  if (__any_sync(0xffffffffu, nw != 0ull)) {
+    lo |= lof_bit_transpose32((uint32_t)nw, lane);
+    if (C > 32) hi |= lof_bit_transpose32((uint32_t)(nw >> 32), lane);
+    const uint32_t added = __reduce_add_sync(0xffffffffu, (uint32_t)__popcll(nw));
+    if (lane == 0) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[s].n_flagged), (unsigned long long)added);
   }
-#pragma unroll
-  for (int c = 0; c < C; ++c) co[(size_t)c * W] = v[c];
-  if (added) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[s].n_flagged), (unsigned long long)added);
+  if (lane < C) co[(size_t)lane * W] = lo;
+  if (C > 32) co[(size_t)(lane + 32) * W] = hi;
 }
 
 // Frequency direction, any channel count.  One thread per (stream, word column): the C words in[c][w] carry 32 time samples each.
