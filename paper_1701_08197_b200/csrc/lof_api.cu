@@ -430,6 +430,13 @@ static int flag_block_fused(lof_ctx*, const int16_t*, uint32_t*, cudaStream_t) {
 
 // ---- SIR operator on the packed mask (lof_sir.cuh): frequency, then time; ping-pong between the caller's
 // flags and the context's mask buffer
+// the shortest run that the operator grows: the smallest m <= limit with floor(eta * m) >= 1 (limit + 1 if none)
+static uint32_t sir_min_run(float eta, uint32_t limit) {
+  uint32_t m = 1;
+  while (m <= limit && (uint32_t)std::floor((double)eta * (double)m) == 0) ++m;
+  return m;
+}
+
 template <int G>
 static void sir_time_launch(const uint32_t* in, uint32_t* out, lof_ctx* c, cudaStream_t st) {
   const uint64_t rows = (uint64_t)c->prm.n_streams * c->prm.n_channels;
@@ -438,10 +445,10 @@ static void sir_time_launch(const uint32_t* in, uint32_t* out, lof_ctx* c, cudaS
   const size_t stage = (size_t)2 * (256 / G) * c->kp.W * 4;   // in and out copies of the CTA's rows
   if (stage <= 40 * 1024)
     lof_k_sir_time<G, true><<<grid, 256, stage, st>>>(in, out, c->d_stats, rows, c->prm.n_channels, c->kp.W,
-                                                      c->prm.n_time, c->prm.sir_eta);
+                                                      c->prm.n_time, c->prm.sir_eta, sir_min_run(c->prm.sir_eta, c->prm.n_time));
   else
     lof_k_sir_time<G, false><<<grid, 256, 0, st>>>(in, out, c->d_stats, rows, c->prm.n_channels, c->kp.W,
-                                                   c->prm.n_time, c->prm.sir_eta);
+                                                   c->prm.n_time, c->prm.sir_eta, sir_min_run(c->prm.sir_eta, c->prm.n_time));
 }
 
 static int sir_apply(lof_ctx* c, uint32_t* d_flags, cudaStream_t st) {
@@ -452,13 +459,12 @@ static int sir_apply(lof_ctx* c, uint32_t* d_flags, cudaStream_t st) {
   uint32_t* cur = d_flags;
   uint32_t* other = c->d_fmask;
   if (c->prm.directions & LOF_DIR_FREQ) {
-    uint32_t m_min = 1;                                  // shortest run that grows at all
-    while (m_min <= C && (uint32_t)std::floor((double)eta * (double)m_min) == 0) ++m_min;
+    const uint32_t m_min = sir_min_run(eta, C);          // shortest run that grows at all
     const uint64_t n_cols = (uint64_t)c->prm.n_streams * W;
-    const unsigned g8 = (unsigned)((n_cols + 7) / 8);          // a warp per word column
-    if (C == 64) lof_k_sir_freq_reg<64><<<g8, 256, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
-    else if (C == 32) lof_k_sir_freq_reg<32><<<g8, 256, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
-    else if (C == 16) lof_k_sir_freq_reg<16><<<g8, 256, 0, st>>>(cur, other, c->d_stats, n_cols, W, eta, m_min);
+    const dim3 g8(c->prm.n_streams, (W + 7) / 8);                // a warp per word column, 8 per CTA
+    if (C == 64) lof_k_sir_freq_reg<64><<<g8, 256, 0, st>>>(cur, other, c->d_stats, W, eta, m_min);
+    else if (C == 32) lof_k_sir_freq_reg<32><<<g8, 256, 0, st>>>(cur, other, c->d_stats, W, eta, m_min);
+    else if (C == 16) lof_k_sir_freq_reg<16><<<g8, 256, 0, st>>>(cur, other, c->d_stats, W, eta, m_min);
     else lof_k_sir_freq<<<(unsigned)((n_cols + 255) / 256), 256, 0, st>>>(cur, other, c->d_stats, n_cols, C, W, eta, m_min);
     c->launches += 1;
     uint32_t* t = cur; cur = other; other = t;
@@ -821,8 +827,9 @@ static void noalloc_sir_time(const uint32_t* in, uint32_t* out, lof_stream_stats
                              uint32_t W, uint32_t T, float eta, cudaStream_t st) {
   const unsigned grid = (unsigned)((rows * G + 255) / 256);
   const size_t stage = (size_t)2 * (256 / G) * W * 4;
-  if (stage <= 40 * 1024) lof_k_sir_time<G, true><<<grid, 256, stage, st>>>(in, out, d_stats, rows, C, W, T, eta);
-  else lof_k_sir_time<G, false><<<grid, 256, 0, st>>>(in, out, d_stats, rows, C, W, T, eta);
+  const uint32_t m_min = sir_min_run(eta, T);
+  if (stage <= 40 * 1024) lof_k_sir_time<G, true><<<grid, 256, stage, st>>>(in, out, d_stats, rows, C, W, T, eta, m_min);
+  else lof_k_sir_time<G, false><<<grid, 256, 0, st>>>(in, out, d_stats, rows, C, W, T, eta, m_min);
 }
 
 extern "C" int lof_sir_noalloc(uint32_t* d_flags, lof_stream_stats* d_stats, uint32_t n_streams, uint32_t n_channels,
@@ -845,13 +852,12 @@ extern "C" int lof_sir_noalloc(uint32_t* d_flags, lof_stream_stats* d_stats, uin
   uint32_t* cur = d_flags;
   uint32_t* other = scratch;
   if (directions & LOF_DIR_FREQ) {
-    uint32_t m_min = 1;                                  // shortest run that grows at all
-    while (m_min <= C && (uint32_t)std::floor((double)eta * (double)m_min) == 0) ++m_min;
+    const uint32_t m_min = sir_min_run(eta, C);          // shortest run that grows at all
     const uint64_t n_cols = (uint64_t)S * W;
-    const unsigned g8 = (unsigned)((n_cols + 7) / 8);          // a warp per word column
-    if (C == 64) lof_k_sir_freq_reg<64><<<g8, 256, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
-    else if (C == 32) lof_k_sir_freq_reg<32><<<g8, 256, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
-    else if (C == 16) lof_k_sir_freq_reg<16><<<g8, 256, 0, st>>>(cur, other, d_stats, n_cols, W, eta, m_min);
+    const dim3 g8(S, (W + 7) / 8);                             // a warp per word column, 8 per CTA
+    if (C == 64) lof_k_sir_freq_reg<64><<<g8, 256, 0, st>>>(cur, other, d_stats, W, eta, m_min);
+    else if (C == 32) lof_k_sir_freq_reg<32><<<g8, 256, 0, st>>>(cur, other, d_stats, W, eta, m_min);
+    else if (C == 16) lof_k_sir_freq_reg<16><<<g8, 256, 0, st>>>(cur, other, d_stats, W, eta, m_min);
     else lof_k_sir_freq<<<(unsigned)((n_cols + 255) / 256), 256, 0, st>>>(cur, other, d_stats, n_cols, C, W, eta, m_min);
     uint32_t* t = cur; cur = other; other = t;
   }

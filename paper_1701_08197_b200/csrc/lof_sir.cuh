@@ -59,9 +59,11 @@ __device__ __forceinline__ void lof_sir_set(uint32_t* __restrict__ w, uint32_t l
 // words [j*B, j*B+B) of the row wi[0..W) (B = ceil(W/G)); the output words go to wo (a different buffer).  Every
 // lane of the group must call it; `live` = false makes the group compute and write nothing.  Returns the number
 // of bits this lane's words gained.
+// m_min = the shortest run that grows at all (floor(eta * m_min) >= 1): shorter runs — most of them, single
+// noise flags — skip the fp64 product, and a lane whose block has nothing to extend copies its words.
 template <int G>
 __device__ __forceinline__ uint32_t lof_sir_time_row(const uint32_t* wi, uint32_t* wo, int j, unsigned gmask,
-                                                     uint32_t W, uint32_t T, float eta, bool live) {
+                                                     uint32_t W, uint32_t T, float eta, uint32_t m_min, bool live) {
   const uint32_t B = (W + G - 1) / G;
   const uint32_t p0 = min((uint32_t)j * B * 32u, T), p1 = min(((uint32_t)j + 1u) * B * 32u, T), len = p1 - p0;
   // 1. block summary and the carries
@@ -86,13 +88,15 @@ __device__ __forceinline__ uint32_t lof_sir_time_row(const uint32_t* wi, uint32_
   // 2. runs of the block, reaches
   int rmax = -1;                                          // exclusive end of the farthest right extension emitted here
   int lmin = 0x7FFFFFFF;                                  // start of the farthest left extension emitted here
+  bool grows = false;                                     // some run of this block has an extension
   for (uint32_t p = p0; p < p1;) {
     const uint32_t a = lof_sir_next(wi, p, p1, true);
     if (a >= p1) break;
     const uint32_t b = lof_sir_next(wi, a, p1, false);
     const bool starts = a > p0 || cin == 0, ends = b < p1 || cout == 0;
     const uint32_t n = (b - a) + (a == p0 ? cin : 0u) + (b == p1 ? cout : 0u);
-    const uint32_t e = lof_sir_ext(eta, n);
+    const uint32_t e = n >= m_min ? lof_sir_ext(eta, n) : 0u;
+    grows = grows || e != 0u;
     if (ends) rmax = max(rmax, (int)min(b + e, T));
     if (starts) lmin = min(lmin, (int)(a > e ? a - e : 0u));
     p = b;
@@ -113,13 +117,13 @@ __device__ __forceinline__ uint32_t lof_sir_time_row(const uint32_t* wi, uint32_
   const uint32_t w0 = (uint32_t)j * B, w1 = min(w0 + B, W);
   uint32_t before = 0, after = 0;
   for (uint32_t w = w0; w < w1; ++w) { const uint32_t v = wi[w]; wo[w] = v; before += __popc(v); }
-  for (uint32_t p = p0; p < p1;) {
+  if (grows) for (uint32_t p = p0; p < p1;) {
     const uint32_t a = lof_sir_next(wi, p, p1, true);
     if (a >= p1) break;
     const uint32_t b = lof_sir_next(wi, a, p1, false);
     const bool starts = a > p0 || cin == 0, ends = b < p1 || cout == 0;
     const uint32_t n = (b - a) + (a == p0 ? cin : 0u) + (b == p1 ? cout : 0u);
-    const uint32_t e = lof_sir_ext(eta, n);
+    const uint32_t e = n >= m_min ? lof_sir_ext(eta, n) : 0u;
     if (ends && e) lof_sir_set(wo, b, min(b + e, p1));
     if (starts && e) lof_sir_set(wo, max(a > e ? a - e : 0u, p0), a);
     p = b;
@@ -135,7 +139,7 @@ __device__ __forceinline__ uint32_t lof_sir_time_row(const uint32_t* wi, uint32_
 template <int G, bool STAGE>
 __global__ void __launch_bounds__(256)
 lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_stream_stats* __restrict__ stats,
-               uint64_t n_rows, uint32_t C, uint32_t W, uint32_t T, float eta) {
+               uint64_t n_rows, uint32_t C, uint32_t W, uint32_t T, float eta, uint32_t m_min) {
   extern __shared__ uint32_t sir_sh[];                    // STAGE: [2][256/G][W]
   const uint64_t gid = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / G;
   const int j = threadIdx.x % G;
@@ -154,7 +158,7 @@ lof_k_sir_time(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_
     wo = sir_sh + (RPB + lr) * W;
   }
   const unsigned gmask = (G == 32) ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
-  const uint32_t added = lof_sir_time_row<G>(wi, wo, j, gmask, W, T, eta, live);
+  const uint32_t added = lof_sir_time_row<G>(wi, wo, j, gmask, W, T, eta, m_min, live);
   if (added) atomicAdd(reinterpret_cast<unsigned long long*>(&stats[row / C].n_flagged), (unsigned long long)added);
   if (STAGE) {
     __syncthreads();
@@ -200,18 +204,17 @@ __device__ __forceinline__ uint32_t lof_bit_transpose32(uint32_t x, int lane) {
 // a bit, two more transposes bring the new bits back to the channel words.  (The first version was a thread per word
 // column with the C words in registers and a loop over the time samples with long runs: the lanes of a warp waited
 // for the one whose word lay inside a burst — 32 samples x 400 instructions — and the kernel took 150 us for the
-// 38 MB mask of config 2 x 64 subbands.)  grid.x = ceil(n_cols / 8), 256 threads.
+// 38 MB mask of config 2 x 64 subbands.)  grid = (S, ceil(W / 8)), 256 threads: a CTA takes 8 consecutive word
+// columns of one stream (one 32-byte sector per channel row).
 template <int C>
 __global__ void __launch_bounds__(256)
 lof_k_sir_freq_reg(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, lof_stream_stats* __restrict__ stats,
-                   uint64_t n_cols /* S*W */, uint32_t W, float eta, uint32_t m_min) {
+                   uint32_t W, float eta, uint32_t m_min) {
   const int lane = threadIdx.x & 31;
-  const uint64_t gw = (uint64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
-  if (gw >= n_cols) return;                               // whole warps leave together
-  const uint64_t s = gw / W;
-  const uint32_t w = (uint32_t)(gw - s * W);
-  const uint32_t* ci = in + s * C * W + w;
-  uint32_t* co = out + s * C * W + w;
+  const uint32_t s = blockIdx.x, w = blockIdx.y * 8u + (threadIdx.x >> 5);
+  if (w >= W) return;                                     // whole warps leave together
+  const uint32_t* ci = in + (size_t)s * C * W + w;
+  uint32_t* co = out + (size_t)s * C * W + w;
   uint32_t lo = lane < C ? __ldg(ci + (size_t)lane * W) : 0u;
   uint32_t hi = C > 32 ? __ldg(ci + (size_t)(lane + 32) * W) : 0u;
   const uint32_t tl = lof_bit_transpose32(lo, lane);
