@@ -268,7 +268,8 @@ __device__ __forceinline__ void lof_stat_row(const LofFusedSmem& sm, int c, cons
 // DESIGN.md S6); `median_out` is valid in every thread.
 template <int C, int L>
 __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& prm, const LofStatPlan& pl,
-                                      lof_stream_stats* out, float& median_out, unsigned long long* diag) {
+                                      lof_stream_stats* out, float& median_out, unsigned long long* diag,
+                                      uint64_t* nflag_prev = nullptr /* n_flagged of the stream just flagged */) {
   using Cfg = LofFusedCfg<C, L>;
   constexpr int N = Cfg::N, NT = Cfg::NT, NW = NT / 32;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -285,6 +286,7 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
     a = lof_warp_sum(a); q = lof_warp_sum(q);
     if (lane == 0) {
       sm.red[0] = a; sm.red[1] = q;
+      if (nflag_prev) *nflag_prev = sm.ctl[CT_NFLAG];     // (before the counter is reset for the next stream)
       sm.ctl[CT_NCAND] = 0; sm.ctl[CT_BAD] = 0; sm.ctl[CT_FOUND] = 0;
       sm.ctl[CT_NFLAG] = 0; sm.ctl[CT_ROW] = 0; sm.ctl[CT_COLGRP] = 0; sm.ctl[CT_SROW] = 0;
     }
@@ -491,14 +493,15 @@ __device__ uint32_t lof_stat_finalize(const LofFusedSmem& sm, const LofKParams& 
 // sample, every row through lof_stat_row, then lof_stat_finalize.
 template <int C, int L>
 __device__ uint32_t lof_stat_whole(const LofFusedSmem& sm, const LofKParams& prm, float sample,
-                                   lof_stream_stats* out, float& median_out, unsigned long long* diag) {
+                                   lof_stream_stats* out, float& median_out, unsigned long long* diag,
+                                   uint64_t* nflag_prev = nullptr) {
   using Cfg = LofFusedCfg<C, L>;
   constexpr int NT = Cfg::NT, NW = NT / 32;
   const LofStatPlan pl = lof_stat_plan<NT>(sample, reinterpret_cast<float*>(sm.red));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int c = warp; c < C; c += NW) lof_stat_row<C, L>(sm, c, pl, lane);
   __syncthreads();
-  return lof_stat_finalize<C, L>(sm, prm, pl, out, median_out, diag);
+  return lof_stat_finalize<C, L>(sm, prm, pl, out, median_out, diag, nflag_prev);
 }
 
 // Shared-memory layout of a row: float4 chunk g is stored at g ^ ((g >> 3) & 1): adjacent float4 pairs swapped in
@@ -728,13 +731,12 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
     lof_cp_async_wait_all();
     __syncthreads();
     LOF_PROF_T(t4);
-    if (tid == 0) stats[s].n_flagged = sm.ctl[CT_NFLAG];
-    __syncthreads();
+    // the stream's flag count: stored by the thread that resets the counter for the next stream (no barrier of its own)
     if (more) {
-      if (Cfg::OVL) n_bad = lof_stat_finalize<C, L>(sm, prm, plan_next, stats + s_next, median, diag);
-      else n_bad = lof_stat_whole<C, L>(sm, prm, sample_next, stats + s_next, median, diag);
+      if (Cfg::OVL) n_bad = lof_stat_finalize<C, L>(sm, prm, plan_next, stats + s_next, median, diag, &stats[s].n_flagged);
+      else n_bad = lof_stat_whole<C, L>(sm, prm, sample_next, stats + s_next, median, diag, &stats[s].n_flagged);
       ready = true;
-    }
+    } else if (tid == 0) stats[s].n_flagged = sm.ctl[CT_NFLAG];
     LOF_PROF_T(t5);
     LOF_PROF_ADD(0, t0, t1); LOF_PROF_ADD(1, t1, t2); LOF_PROF_ADD(2, t2, t3); LOF_PROF_ADD(3, t3, t4);
     LOF_PROF_ADD(4, t4, t5);
