@@ -24,10 +24,16 @@
 #define LOF_LR_CTA_LIST 1024       // candidates a gather CTA collects before it reserves list space
 #define LOF_LR_STAGE 8192          // ... of which this many can be selected from shared memory
 
+// Byte offset of x's bin in a histogram of LOF_LR_NBINS words: FFMA.SAT, FFMA, LOP (the fused kernel's
+// lof_stat_binoff).  t = x*scale + off in bin units, clamped to [0, NBINS-1]; adding 1.5*2^23 leaves round(4 t) in
+// the low mantissa bits, whose two lowest are masked off: bin b holds t in [b - 1/8, b + 7/8).  s1, o1 = scale, off
+// divided by NBINS - 1.  Monotone in x: bins are value-ordered.
+__device__ __forceinline__ uint32_t lof_lr_binoff(float x, float s1, float o1) {
+  const float y = __saturatef(fmaf(x, s1, o1));
+  return __float_as_uint(fmaf(y, 4.0f * (float)(LOF_LR_NBINS - 1), 12582912.0f)) & (uint32_t)(4 * LOF_LR_NBINS - 4);
+}
 __device__ __forceinline__ uint32_t lof_lr_bin(float x, float scale, float off) {
-  float yb = fmaf(x, scale, off);
-  yb = fminf(fmaxf(yb, 0.f), (float)(LOF_LR_NBINS - 1) + 0.4f);
-  return __float_as_uint(yb + 12582912.0f) & (uint32_t)(LOF_LR_NBINS - 1);
+  return lof_lr_binoff(x, scale * (1.0f / (float)(LOF_LR_NBINS - 1)), off * (1.0f / (float)(LOF_LR_NBINS - 1))) >> 2;
 }
 
 // The histogram placement of stream s, by all 256 threads of a CTA; K, scale, off valid in every thread.
@@ -92,12 +98,18 @@ lof_k_lr_hist(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_
   __syncthreads();
   uint32_t bad = 0;
   const uint32_t c_end = min(n_chunks, (blk + 1) * cpb);
+  const float s1 = scale * (1.0f / (float)(LOF_LR_NBINS - 1)), o1 = off * (1.0f / (float)(LOF_LR_NBINS - 1));
+  unsigned char* hb = reinterpret_cast<unsigned char*>(sh_hist);
+  const float2 nK = make_float2(-K, -K);
+  // the thread's sums over ALL of the CTA's chunks (fp32 over 8 samples per half of a pair, then fp64), reduced
+  // over the CTA once: a block reduction per chunk had cost two of the kernel's twenty instructions per sample
+  double sum = 0.0, sumsq = 0.0;
   for (uint32_t chunk = blk * cpb; chunk < c_end; ++chunk) {
     const uint64_t lo = (uint64_t)chunk * LOF_STATS_CHUNK;
     const uint64_t hi = min(N, lo + (uint64_t)LOF_STATS_CHUNK);
-    double sum = 0.0, sumsq = 0.0;
     if (((N | lo) & 3) == 0 && hi - lo == LOF_STATS_CHUNK) {
-      // full chunk, 16-byte aligned: 4 x 16-byte loads per thread in flight, two groups of 8 samples each
+      // full chunk, 16-byte aligned: 4 x 16-byte loads per thread in flight; packed fp32 pairs: .x and .y each take
+      // 8 of the 16 samples
 #pragma unroll 1
       for (int it = 0; it < LOF_STATS_PER_THREAD / 16; ++it) {
         float xv[16];
@@ -107,22 +119,21 @@ lof_k_lr_hist(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_
           in.ld4(base + lo + ((uint64_t)(it * 4 + r) * LOF_STATS_THREADS + threadIdx.x) * 4, t4);
           xv[4 * r] = t4[0]; xv[4 * r + 1] = t4[1]; xv[4 * r + 2] = t4[2]; xv[4 * r + 3] = t4[3];
         }
+        float2 ga = make_float2(0.f, 0.f), gq = make_float2(0.f, 0.f);
 #pragma unroll
-        for (int g = 0; g < 2; ++g) {
-          float ga = 0.f, gq = 0.f;
-#pragma unroll
-          for (int r = 0; r < 8; ++r) {
-            const float x = xv[8 * g + r], d = x - K;
-            ga += d; gq = fmaf(d, d, gq);
-            atomicAdd(&sh_hist[lof_lr_bin(x, scale, off)], 1u);
-          }
-          // a non-finite sample makes its group's sums non-finite: count exactly only then
-          if (!lof_finite(ga) || !lof_finite(gq)) {
-#pragma unroll
-            for (int r = 0; r < 8; ++r) bad += lof_finite(xv[8 * g + r]) ? 0u : 1u;
-          }
-          sum += (double)ga; sumsq += (double)gq;
+        for (int r = 0; r < 8; ++r) {
+          const float2 d = __fadd2_rn(make_float2(xv[2 * r], xv[2 * r + 1]), nK);
+          ga = __fadd2_rn(ga, d); gq = __ffma2_rn(d, d, gq);
+          atomicAdd(reinterpret_cast<uint32_t*>(hb + lof_lr_binoff(xv[2 * r], s1, o1)), 1u);
+          atomicAdd(reinterpret_cast<uint32_t*>(hb + lof_lr_binoff(xv[2 * r + 1], s1, o1)), 1u);
         }
+        const float gas = ga.x + ga.y, gqs = gq.x + gq.y;
+        // a non-finite sample makes its group's sums non-finite: count exactly only then
+        if (!lof_finite(gas) || !lof_finite(gqs)) {
+#pragma unroll
+          for (int r = 0; r < 16; ++r) bad += lof_finite(xv[r]) ? 0u : 1u;
+        }
+        sum += (double)ga.x + (double)ga.y; sumsq += (double)gq.x + (double)gq.y;
       }
     } else {
       for (uint64_t i0 = lo + threadIdx.x; i0 < hi; i0 += 8 * LOF_STATS_THREADS) {
@@ -140,11 +151,16 @@ lof_k_lr_hist(In in, LofKParams prm, LofStreamState* __restrict__ state, uint32_
         sum += (double)ga; sumsq += (double)gq;
       }
     }
+  }
+  {
+    // the CTA's sums go to the slot of its first chunk, zeros to its other chunks (lof_k_lr_select2 adds the chunk
+    // slots of a stream in chunk order)
     const double rs = lof_block_sum(sum, sh_red);
     const double rq = lof_block_sum(sumsq, sh_red);
-    if (threadIdx.x == 0) {
-      partial[((size_t)sl * n_chunks + chunk) * 2 + 0] = rs;
-      partial[((size_t)sl * n_chunks + chunk) * 2 + 1] = rq;
+    const uint32_t c0 = blk * cpb;
+    for (uint32_t chunk = c0 + threadIdx.x; chunk < c_end; chunk += LOF_STATS_THREADS) {
+      partial[((size_t)sl * n_chunks + chunk) * 2 + 0] = chunk == c0 ? rs : 0.0;
+      partial[((size_t)sl * n_chunks + chunk) * 2 + 1] = chunk == c0 ? rq : 0.0;
     }
   }
   __syncthreads();
@@ -204,7 +220,7 @@ lof_k_lr_gather(In in, LofKParams prm, LofStreamState* __restrict__ state, const
   lof_lr_find_bin(gh, (uint32_t)(N / 2), sh_cnt, sh_sel);
   const uint32_t bin = sh_sel[0], before = sh_sel[1], n_b = gh[bin], n_bad = ctr[2 * sl];
   const float scale = st.pl_scale, off = st.pl_off, inv = 1.0f / scale;
-  const float v0 = ((float)bin - 0.5f - off) * inv, v1 = ((float)bin + 0.5f - off) * inv;
+  const float v0 = ((float)bin - 0.5f - off) * inv, v1 = ((float)bin + 1.0f - off) * inv;   // (lof_lr_binoff: [b-1/8, b+7/8))
   const float eps = 8e-7f * (fabsf(v0) + fabsf(v1) + fabsf(off) * inv) + 8e-4f * inv;
   const float vmid = 0.5f * (v0 + v1), vhalf = 0.5f * (v1 - v0) + eps;
   const bool fallback = bin == 0 || bin >= LOF_LR_NBINS - 1 || n_b > LOF_LR_CAND || n_bad != 0;
