@@ -79,12 +79,14 @@ struct LofFusedSmem {
   }
 };
 // ctl slots
-enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS, CT_NFLAG, CT_BAD, CT_SELP, CT_SELACC, CT_PREFIX, CT_RANK, CT_FOUND, CT_SROW = 13 };
+enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS, CT_NFLAG, CT_BAD, CT_SELP, CT_SELACC, CT_PREFIX, CT_RANK, CT_FOUND, CT_SROW = 13, CT_TICKET = 14 /* and 15 */ };
 
 // Diagnostics live in a context-owned array `diag` (LOF_DIAG_WORDS words, lof_fused_counters): how the median of
 // each stream was found: [0] rank count among the samples of the median's bin, [1] radix select among them (a
 // crowded bin), [2] radix select over the whole stream, [3] stream with non-finite samples.
 #define LOF_DIAG_WORDS 16
+#define LOF_DIAG_TICKET 6         // work queue of the persistent CTAs: streams handed out / CTAs that have left
+#define LOF_DIAG_DONE 7
 // Find the bin holding `rank` in hist[NB] (NB a multiple of 1024, any blockDim that is a multiple of 32).
 // Results in ctl[CT_BIN] (bin) and ctl[CT_BEFORE] (number of entries in lower bins); rank beyond the total
 // gives the last bin.  Groups of 32 bins are summed by warps (one bin per lane: no bank conflicts), warp 0
@@ -687,9 +689,23 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
   unsigned bar_parity = 0;     // phase of the row barriers the next prefetch completes
   if (tid < C) lof_mbar_init(sm.rowbar + tid, 32);
   __syncthreads();
+  // Streams are handed out dynamically after the first two of a CTA (blockIdx.x and blockIdx.x + gridDim.x): a
+  // stream's cost depends on its content (restarts), and with ~42 streams per CTA in a fixed order the kernel waited
+  // for the unluckiest CTA.  Tickets come from diag[LOF_DIAG_TICKET]; a stream must be known one stream ahead (its
+  // rows are prefetched during the time pass of the one before), so the ticket for the stream AFTER NEXT is drawn at
+  // the top of an iteration and read after that iteration's first barrier (two slots by parity).  The last CTA to
+  // leave resets the counters for the next launch.
+  // (Measured: + 2 % with one CTA per SM, config 2; - 2.5 % with two CTAs per SM, config 3, whose CTAs then stay in
+  // a fixed order: DYN.)
+  constexpr bool DYN = Cfg::MINB == 1;
+  uint32_t s_nx = blockIdx.x + gridDim.x, it = 0;
 #pragma unroll 1
-  for (uint32_t s = blockIdx.x; s < prm.S; s += gridDim.x) {
+  for (uint32_t s = blockIdx.x; s < prm.S; ++it) {
     LOF_PROF_T(t0);
+    // (drawn here, put into shared memory only before the barrier that publishes it: the atomic's round trip to L2
+    // hides behind the frequency pass instead of holding warp 0 at the top of the iteration)
+    uint32_t ticket = 0;
+    if (DYN && tid == 0) ticket = 2u * gridDim.x + (uint32_t)atomicAdd(&diag[LOF_DIAG_TICKET], 1ull);
     if (!ready) {                                         // first stream of this CTA (or after a skipped one)
       const float* gs = power + (size_t)s * N;
       const float4* g4 = reinterpret_cast<const float4*>(gs);
@@ -706,11 +722,12 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
       // DESIGN.md S6: the whole stream is flagged
       for (int i = tid; i < C * W; i += NT) flags[(size_t)s * C * W + i] = 0xFFFFFFFFu;
       for (int i = tid; i < C; i += NT) { rowsum[(size_t)s * C + i] = 0.0; rowcnt[(size_t)s * C + i] = 0; }
-      if (tid == 0) atomicAdd(&diag[3], 1ull);
+      if (tid == 0) { atomicAdd(&diag[3], 1ull); sm.ctl[CT_TICKET + (it & 1u)] = ticket; }
       __syncthreads();
+      { const uint32_t nx2 = DYN ? sm.ctl[CT_TICKET + (it & 1u)] : s_nx + gridDim.x; s = s_nx; s_nx = nx2; }
       continue;
     }
-    const uint32_t s_next = s + gridDim.x;
+    const uint32_t s_next = s_nx;
     const bool more = s_next < prm.S;
     const float* next = more ? power + (size_t)s_next * N : nullptr;
     // issued here, consumed after the frequency pass: no select on the loaded value, or the wait moves up here
@@ -721,7 +738,9 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
       if constexpr (C == 64) lof_fused_freq_pair<C, L>(sm, prm.n_lev_f);
       else lof_fused_freq<C, L>(sm, prm.n_lev_f);
     }
+    if (tid == 0) sm.ctl[CT_TICKET + (it & 1u)] = ticket;
     __syncthreads();
+    const uint32_t s_nx2 = DYN ? sm.ctl[CT_TICKET + (it & 1u)] : s_nx + gridDim.x;
     LOF_PROF_T(t2);
     LofStatPlan plan_next;
     if (Cfg::OVL) plan_next = lof_stat_plan<NT>(sample_next, reinterpret_cast<float*>(sm.red));
@@ -740,6 +759,13 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
     LOF_PROF_T(t5);
     LOF_PROF_ADD(0, t0, t1); LOF_PROF_ADD(1, t1, t2); LOF_PROF_ADD(2, t2, t3); LOF_PROF_ADD(3, t3, t4);
     LOF_PROF_ADD(4, t4, t5);
+    s = s_nx; s_nx = s_nx2;
   }
   lof_cp_async_wait_all();
+  if (DYN && tid == 0) {
+    __threadfence();                                      // this CTA's last ticket was drawn before it is counted out
+    if (atomicAdd(&diag[LOF_DIAG_DONE], 1ull) == (unsigned long long)gridDim.x - 1ull) {
+      diag[LOF_DIAG_TICKET] = 0ull; diag[LOF_DIAG_DONE] = 0ull;
+    }
+  }
 }
