@@ -408,6 +408,9 @@ static cudaError_t fused_prepare_any(lof_ctx* c) {
 static int flag_block_fused(lof_ctx* c, const float* d_power, uint32_t* d_flags, cudaStream_t st) {
   const uint32_t C = c->prm.n_channels, T = c->prm.n_time;
   if (!c->fused_grid) return 0;
+  // the ticket counter of the kernel's dynamic hand-out of streams starts every launch at zero (reset here rather than
+  // by the last CTA to leave: a launch that died would otherwise leave the next one skipping streams)
+  LOF_CUDA(cudaMemsetAsync(c->d_diag + LOF_DIAG_TICKET, 0, sizeof(unsigned long long), st));
   bool done = false;
 #define X(CC, LL)                                                                                              \
   if (!done && C == CC && T == 32 * LL) {                                                                      \

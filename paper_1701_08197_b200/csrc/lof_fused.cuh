@@ -85,8 +85,7 @@ enum { CT_COLGRP = 12, CT_ROW = 11, CT_NCAND = 0, CT_BIN, CT_BEFORE, CT_MEDBITS,
 // each stream was found: [0] rank count among the samples of the median's bin, [1] radix select among them (a
 // crowded bin), [2] radix select over the whole stream, [3] stream with non-finite samples.
 #define LOF_DIAG_WORDS 16
-#define LOF_DIAG_TICKET 6         // work queue of the persistent CTAs: streams handed out / CTAs that have left
-#define LOF_DIAG_DONE 7
+#define LOF_DIAG_TICKET 6         // work queue of the persistent CTAs: streams handed out beyond the fixed first two
 // Find the bin holding `rank` in hist[NB] (NB a multiple of 1024, any blockDim that is a multiple of 32).
 // Results in ctl[CT_BIN] (bin) and ctl[CT_BEFORE] (number of entries in lower bins); rank beyond the total
 // gives the last bin.  Groups of 32 bins are summed by warps (one bin per lane: no bank conflicts), warp 0
@@ -693,8 +692,8 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
   // stream's cost depends on its content (restarts), and with ~42 streams per CTA in a fixed order the kernel waited
   // for the unluckiest CTA.  Tickets come from diag[LOF_DIAG_TICKET]; a stream must be known one stream ahead (its
   // rows are prefetched during the time pass of the one before), so the ticket for the stream AFTER NEXT is drawn at
-  // the top of an iteration and read after that iteration's first barrier (two slots by parity).  The last CTA to
-  // leave resets the counters for the next launch.
+  // the top of an iteration and read after that iteration's first barrier (two slots by parity).  The host zeroes
+  // the counter before every launch.
   // (Measured: + 2 % with one CTA per SM, config 2; - 2.5 % with two CTAs per SM, config 3, whose CTAs then stay in
   // a fixed order: DYN.)
   constexpr bool DYN = Cfg::MINB == 1;
@@ -762,10 +761,4 @@ lof_k_fused(const float* __restrict__ power, uint32_t* __restrict__ flags, lof_s
     s = s_nx; s_nx = s_nx2;
   }
   lof_cp_async_wait_all();
-  if (DYN && tid == 0) {
-    __threadfence();                                      // this CTA's last ticket was drawn before it is counted out
-    if (atomicAdd(&diag[LOF_DIAG_DONE], 1ull) == (unsigned long long)gridDim.x - 1ull) {
-      diag[LOF_DIAG_TICKET] = 0ull; diag[LOF_DIAG_DONE] = 0ull;
-    }
-  }
 }
